@@ -1,0 +1,260 @@
+"""Seeded synthetic inputs shaped like the paper's workloads (BASELINE.json configs 0-4).
+
+This module is the ONE thing the CPU oracle's tests and the CUDA path's tests share.  It holds input
+recipes only (numpy on the host) -- none of the step's arithmetic, no CUDA, no oracle import:
+  * a seeded Gaussian random field with P(k) = A k^-2 exp(-(k/k_c)^2), k_c = k_Nyq/2, rescaled to the stated rms
+    (stand-in for the paper's Eisenstein-Hu + LPT initial conditions; reading R19 in DESIGN.md);
+  * the Zel'dovich map  delta -> (gas, particles)  at the starting scale factor, and its transpose (used to
+    express "gradient w.r.t. the initial density field" for configs 0, 2, 3 on either side);
+  * the spherical Sod-type Riemann problem of config 1 and a 1-D Sod tube;
+  * the config table and the (a, dt) schedule in ln a for an EdS cosmology.
+Units (reading R18): length h^-1 Mpc, velocity km/s, H0 = 100, density in units of the mean comoving total
+matter density, positions in grid units [0, N).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+import numpy as np
+
+KB_OVER_MP = 8.2544e-3   # (km/s)^2 / K
+MU = 0.59
+
+
+@dataclass
+class Config:
+    name: str
+    N: int
+    box: float
+    gamma: float
+    static_mode: int = 0
+    gravity_on: int = 1
+    n_part_side: int = -1          # -1: N
+    H0: float = 100.0
+    Omega_m: float = 1.0
+    Omega_b: float = 0.16
+    Omega_L: float = 0.0
+    a0: float = 0.01
+    a1: float = 0.1
+    n_steps: int = 20
+    rms_delta: float = 0.02
+    seed: int = 1000
+    target_seed: int = 0
+    T0: float = 1.0e4
+    checkpoint_stride: int = 0
+    lim_eps: float = 1e-20
+    e_floor_rel: float = 1e-3      # e_floor = e_floor_rel * initial e~  (R17)
+    extra: dict = field(default_factory=dict)
+
+    @property
+    def n_side(self):
+        return self.N if self.n_part_side < 0 else self.n_part_side
+
+    @property
+    def f_b(self):
+        return self.Omega_b / self.Omega_m
+
+    def e_tilde0(self):
+        """a0^2 e(T0): initial thermal energy per unit mass in tilde variables (R18, R27)."""
+        return self.a0 ** 2 * KB_OVER_MP * self.T0 / ((self.gamma - 1.0) * MU)
+
+    def e_floor(self):
+        return 1e-12 if self.static_mode else self.e_floor_rel * self.e_tilde0()
+
+
+CONFIGS = {
+    0: Config("cfg0_32_coupled", 32, 20.0, 5.0 / 3.0, a1=0.1, n_steps=20, rms_delta=0.02, seed=1000),
+    1: Config("cfg1_128_hydro", 128, 1.0, 1.4, static_mode=1, gravity_on=0, n_part_side=0, n_steps=0),
+    2: Config("cfg2_64_coupled", 64, 50.0, 5.0 / 3.0, a1=0.33, n_steps=100, rms_delta=0.01, seed=1002,
+              target_seed=2002),
+    3: Config("cfg3_256_coupled", 256, 100.0, 5.0 / 3.0, a1=0.33, n_steps=200, rms_delta=0.01, seed=1003,
+              target_seed=2003, checkpoint_stride=10),
+    4: Config("cfg4_512_coupled", 512, 200.0, 5.0 / 3.0, a1=0.33, n_steps=50, rms_delta=0.01, seed=1004,
+              checkpoint_stride=5),
+}
+
+
+def scaled_config(base: int, N: int, **kw) -> Config:
+    """A config with the recipe of `base` on an N^3 grid (same cell size), for small parity cases."""
+    import copy
+    c = copy.deepcopy(CONFIGS[base])
+    c.box = c.box * N / c.N
+    c.N = N
+    c.name = f"{c.name}_at{N}"
+    for k, v in kw.items():
+        setattr(c, k, v)
+    return c
+
+
+# ------------------------------------------------------------------ schedule -------
+def eds_schedule(cfg: Config):
+    """a_k = a0 exp(k r) (k = 0..n), dt_k = t(a_{k+1}) - t(a_k) with the EdS closed form t = 2/(3 H0) a^{3/2}."""
+    n = cfg.n_steps
+    r = np.log(cfg.a1 / cfg.a0) / n
+    a = cfg.a0 * np.exp(r * np.arange(n + 1))
+    a[-1] = cfg.a1
+    t = 2.0 / (3.0 * cfg.H0) * a ** 1.5
+    return a, np.diff(t)
+
+
+# ------------------------------------------------------------ Gaussian field -------
+def _kgrid(N, L):
+    kf = 2.0 * np.pi / L
+    n1 = np.fft.fftfreq(N, d=1.0 / N)             # integers, Nyquist = -N/2
+    nz = n1[:, None, None]; ny = n1[None, :, None]; nx = np.arange(N // 2 + 1)[None, None, :]
+    return kf, nx, ny, nz
+
+
+def gaussian_field(N: int, L: float, seed: int, rms: float) -> np.ndarray:
+    """Real N^3 field, zero mean, P(k) ~ k^-2 exp(-(k/k_c)^2) with k_c = pi N / (2 L), rms exactly `rms`."""
+    rng = np.random.default_rng(seed)
+    white = rng.standard_normal((N, N, N))
+    kf, nx, ny, nz = _kgrid(N, L)
+    k2 = kf * kf * (nx * nx + ny * ny + nz * nz)
+    kc = np.pi * N / (2.0 * L)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        P = np.where(k2 > 0, np.exp(-k2 / kc ** 2) / k2, 0.0)
+    d = np.fft.irfftn(np.fft.rfftn(white) * np.sqrt(P), s=(N, N, N), axes=(0, 1, 2))
+    d -= d.mean()
+    d *= rms / np.sqrt(np.mean(d * d))
+    return d
+
+
+def _psi_operator(N, L):
+    """Fourier multipliers i k~_d / k^2 (d = x, y, z) on the rfftn layout; k~_d = 0 on its Nyquist plane."""
+    kf, nx, ny, nz = _kgrid(N, L)
+    k2 = kf * kf * (nx * nx + ny * ny + nz * nz) + 0.0 * (nx + ny + nz)
+    inv = np.zeros_like(k2)
+    inv[k2 > 0] = 1.0 / k2[k2 > 0]
+    comps = []
+    for n in (nx, ny, nz):
+        nt = np.where(np.abs(n) == N // 2, 0.0, n) + 0.0 * k2
+        comps.append(1j * kf * nt * inv)
+    return comps
+
+
+def displacement(delta: np.ndarray, L: float) -> np.ndarray:
+    """Zel'dovich displacement psi (3,N,N,N) in h^-1 Mpc with div psi = -delta."""
+    N = delta.shape[0]
+    dh = np.fft.rfftn(delta)
+    return np.stack([np.fft.irfftn(op * dh, s=(N, N, N), axes=(0, 1, 2)) for op in _psi_operator(N, L)])
+
+
+def displacement_T(psib: np.ndarray, L: float) -> np.ndarray:
+    """Transpose of `displacement` (the multipliers are odd and imaginary, so each is antisymmetric)."""
+    N = psib.shape[1]
+    acc = 0.0
+    for d, op in enumerate(_psi_operator(N, L)):
+        acc = acc - np.fft.irfftn(op * np.fft.rfftn(psib[d]), s=(N, N, N), axes=(0, 1, 2))
+    return acc
+
+
+def velocity_factor(cfg: Config, a: float) -> float:
+    """w = a^2 H(a) f(a) psi; EdS: H0 sqrt(a)."""
+    assert cfg.Omega_L == 0.0 and abs(cfg.Omega_m - 1.0) < 1e-15, "only EdS ICs are provided"
+    return cfg.H0 * np.sqrt(a)
+
+
+def zeldovich_state(delta: np.ndarray, cfg: Config):
+    """delta (N^3, at a0) -> gas (5,N,N,N), part (6,N^3), float64.  Reading R19."""
+    N, L, a = cfg.N, cfg.box, cfg.a0
+    assert cfg.n_side == N, "one particle per cell"
+    dx = L / N
+    psi = displacement(delta, L)
+    vf = velocity_factor(cfg, a)
+    q = np.arange(N) + 0.5
+    Q = np.stack(np.meshgrid(q, q, q, indexing="ij")[::-1])     # (x,y,z) components on the [z][y][x] grid
+    pos = (Q + psi / dx).reshape(3, -1)
+    pos = pos - N * np.floor(pos / N)
+    w = (vf * psi).reshape(3, -1)
+    part = np.concatenate([pos, w], axis=0)
+    rho = cfg.f_b * (1.0 + delta)
+    v = vf * psi
+    e0 = cfg.e_tilde0()
+    gas = np.empty((5, N, N, N))
+    gas[0] = rho
+    gas[1:4] = rho[None] * v
+    gas[4] = rho * (e0 + 0.5 * np.sum(v * v, axis=0))
+    return gas, part
+
+
+def zeldovich_state_vjp(delta: np.ndarray, cfg: Config, cot_gas: np.ndarray, cot_part: np.ndarray) -> np.ndarray:
+    """Transpose of d(zeldovich_state)/d(delta) applied to (cot_gas, cot_part) -> cotangent of delta."""
+    N, L, a = cfg.N, cfg.box, cfg.a0
+    dx = L / N
+    psi = displacement(delta, L)
+    vf = velocity_factor(cfg, a)
+    rho = cfg.f_b * (1.0 + delta)
+    v = vf * psi
+    e0 = cfg.e_tilde0()
+    cg = np.asarray(cot_gas, dtype=np.float64).reshape(5, N, N, N)
+    cp = np.asarray(cot_part, dtype=np.float64).reshape(6, N, N, N)
+    rho_b = cg[0] + np.sum(cg[1:4] * v, axis=0) + cg[4] * (e0 + 0.5 * np.sum(v * v, axis=0))
+    v_b = cg[1:4] * rho[None] + cg[4][None] * rho[None] * v
+    psi_b = vf * v_b + cp[0:3] / dx + vf * cp[3:6]
+    return cfg.f_b * rho_b + displacement_T(psi_b, L)
+
+
+def coupled_ic(cfg: Config, seed=None):
+    """Seeded IC of a coupled config.  Returns (delta f64, gas f32, part f32) -- the fp32 arrays are THE inputs
+    both the oracle (promoted to fp64) and the CUDA path receive (reading R24)."""
+    delta = gaussian_field(cfg.N, cfg.box, cfg.seed if seed is None else seed, cfg.rms_delta)
+    gas, part = zeldovich_state(delta, cfg)
+    return delta, gas.astype(np.float32), part.astype(np.float32)
+
+
+# ------------------------------------------------------------------ hydro ICs ------
+def sod_sphere(N: int, gamma: float = 1.4, r0: float = 0.2):
+    """Config 1: rho, p = 1, 1 inside r < r0 L about the box centre, else 0.125, 0.1; v = 0.  gas (5,N,N,N) f32."""
+    c = (np.arange(N) + 0.5) / N - 0.5
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+    inside = (x * x + y * y + z * z) < r0 * r0
+    rho = np.where(inside, 1.0, 0.125)
+    p = np.where(inside, 1.0, 0.1)
+    gas = np.zeros((5, N, N, N))
+    gas[0] = rho
+    gas[4] = p / (gamma - 1.0)
+    return gas.astype(np.float32)
+
+
+def sod_tube(nx: int, gamma: float = 1.4, axis: int = 0, ny: int = 1, nz: int = 1, mirror: bool = False):
+    """Two back-to-back Sod tubes on a periodic line: left state (1, 1) on the middle half, right state
+    (0.125, 0.1) outside, so each discontinuity is a Sod problem until the waves meet.  f64."""
+    shape = [nz, ny, nx]
+    n = shape[2 - axis]
+    i = (np.arange(n) + 0.5) / n
+    hi = (i > 0.25) & (i < 0.75)
+    if mirror:
+        hi = ~hi
+    prof_rho = np.where(hi, 1.0, 0.125)
+    prof_p = np.where(hi, 1.0, 0.1)
+    sh = [1, 1, 1]; sh[2 - axis] = n
+    gas = np.zeros((5, nz, ny, nx))
+    gas[0] = prof_rho.reshape(sh)
+    gas[4] = prof_p.reshape(sh) / (gamma - 1.0)
+    return gas
+
+
+def smooth_random_state(N: int, seed: int, amp: float = 0.1, n_part_side=None, mach: float = 0.5):
+    """Smooth, kink-free random gas + particle state on an N^3 grid for derivative tests (low modes only)."""
+    rng = np.random.default_rng(seed)
+    c = (np.arange(N) + 0.5) / N
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+
+    def field():
+        f = np.zeros((N, N, N))
+        for _ in range(4):
+            kx, ky, kz = rng.integers(-2, 3, size=3)
+            f += rng.standard_normal() * np.cos(2 * np.pi * (kx * x + ky * y + kz * z) + rng.uniform(0, 2 * np.pi))
+        return f / 2.0
+    rho = 1.0 + amp * field()
+    v = np.stack([mach * (0.3 + amp * field()) for _ in range(3)])   # offset keeps v away from the |v| kink
+    e = 1.0 + amp * field()
+    gas = np.empty((5, N, N, N))
+    gas[0] = rho; gas[1:4] = rho * v; gas[4] = rho * (e + 0.5 * np.sum(v * v, axis=0))
+    ns = N if n_part_side is None else n_part_side
+    q = (np.arange(ns) + 0.5) * N / ns
+    Q = np.stack(np.meshgrid(q, q, q, indexing="ij")[::-1]).reshape(3, -1)
+    pos = Q + 0.2 * rng.uniform(-1, 1, size=Q.shape) + 0.013
+    pos = pos - N * np.floor(pos / N)
+    w = 0.1 * rng.standard_normal(Q.shape)
+    return gas, np.concatenate([pos, w], axis=0)
