@@ -1,0 +1,174 @@
+/* diffhydro.h -- C ABI of the B200-native diffHydro hot path.
+ *
+ * One coupled time step of the relaxing-TVD finite-volume Euler solver and the dark-matter particle-mesh gravity
+ * solver of Horowitz & Lukic, arXiv 2502.02294 (section 2.2 Eq. 2-3, section 2.3 Eq. 4-20), and that
+ * step's reverse-mode adjoint (section 2.3.5, :198-220), as hand-written CUDA kernels for sm_100a.
+ * cuFFT is used for the 3-D real transforms only.  There is no CPU fallback: dh_init fails with DH_ERR_NO_DEVICE
+ * when no sm_100 device is present.
+ *
+ * Conventions
+ *   - Every entry point returns int: DH_OK (0) or a negative DH_ERR_* code; dh_last_error() gives a thread-local
+ *     message.  No exception crosses this boundary.
+ *   - "device pointer" = CUDA global memory owned by the CALLER (e.g. a torch tensor); the library never frees
+ *     it.  "host pointer" = ordinary host memory.  The context owns cuFFT plans, scratch meshes and snapshots.
+ *   - Grids are N^3 fp32, C order [z][y][x], x fastest.  Gas state = 5 conserved fields in the paper's variables
+ *     (PAPER.md:95-97): gas[0] = rho_b, gas[1..3] = a rho_b U_{x,y,z}, gas[4] = a^2 rho_b E.  Particles are
+ *     structure-of-arrays: part[0..2] = comoving position in GRID UNITS [0, N), part[3..5] = w = a u = a^2 dx/dt in
+ *     km/s (Eq. 2-3).  Density unit = mean comoving total matter density; length h^-1 Mpc; velocity
+ *     km/s; time (h^-1 Mpc)/(km/s).
+ *   - All work is issued on the one CUDA stream given at dh_init (NULL: the legacy default stream) and is asynchronous
+ *     unless stated; calls that return host scalars synchronise that stream.
+ *   - Readings of the paper where it is silent or garbled (R1..R27) are listed in DESIGN.md.
+ */
+#ifndef DIFFHYDRO_H
+#define DIFFHYDRO_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DH_OK 0
+#define DH_ERR_INVALID (-1)    /* bad argument / unsupported size */
+#define DH_ERR_NO_DEVICE (-2)  /* no CUDA device of compute capability 10.x */
+#define DH_ERR_CUDA (-3)
+#define DH_ERR_CUFFT (-4)
+#define DH_ERR_NONFINITE (-5)  /* the CFL reduction saw NaN/Inf */
+#define DH_ERR_OOM (-6)
+#define DH_ERR_STATE (-7)      /* call order (e.g. dh_run_vjp without a checkpointed dh_run) */
+
+typedef struct dh_ctx dh_ctx;
+
+/* Flat matter + Lambda background.  static_mode = 1: a == 1 for all time (non-cosmological runs, config 1). */
+typedef struct {
+    double H0;       /* km/s per h^-1 Mpc (100) */
+    double Omega_m;  /* total matter */
+    double Omega_b;  /* baryons; f_b = Omega_b / Omega_m sets the particle mass (1 - f_b) N^3 / N_p */
+    double Omega_L;
+    int32_t static_mode;
+} dh_cosmology;
+
+typedef struct {
+    int32_t n_part_side;          /* particles per side, N_p = n_part_side^3; 0 = no particles */
+    int32_t gravity_on;           /* 0: no Poisson solve, g' = 0 */
+    int32_t hydro_on;             /* 0: particles only */
+    int32_t gas_sources_gravity;  /* 1: delta_tot includes rho_gas (reading R12) */
+    double e_floor;               /* floor of the DERIVED thermal energy e~ used in fluxes (reading R17), > 0 */
+    double lim_eps;               /* epsilon of the altered Van Leer limiter, Eq. 18 (reading R8) */
+    void* cuda_stream;            /* cudaStream_t to issue all work on; NULL = the legacy default stream */
+    int32_t want_dA;              /* 1: dh_step_vjp also accumulates dparams.dA (one extra pass over g') */
+} dh_options;
+
+/* State of the simulation.  gas/part: caller-owned DEVICE pointers (N^3 and N_p floats each).
+ * a, dt_prev, step: host scalars the library updates (S5 of the step: a <- a_next, dt_prev <- dt, step++). */
+typedef struct {
+    float* gas[5];
+    float* part[6];
+    double a;        /* scale factor of this state (1 in static mode) */
+    double dt_prev;  /* cosmic-time length of the previous step; 0 before the first step (reading R15) */
+    int64_t step;    /* step counter; step mod 6 selects the Strang order (reading R9) */
+} dh_state;
+
+/* Cotangent of a state: same 11 arrays, caller-owned DEVICE pointers. */
+typedef struct {
+    float* gas[5];
+    float* part[6];
+} dh_cot;
+
+/* Gradients w.r.t. the scalars of the scheme, ACCUMULATED (+=) by the VJP calls (host struct, fp64).
+ * dgamma: adiabatic index (through p~ and c~_s; reading R20).  dDtau, dkappa, dK: the per-step factors
+ * Dtau = dt/a_h^2 (drift and hydro), kappa = dt/a_h (gas gravity), K = (dt_prev+dt)/(2 a_i) (particle kick), summed
+ * over steps (reading R15).  dA: Poisson amplitude A = 1.5 Omega_m H0^2 (reading R12). */
+typedef struct {
+    double dgamma, dDtau, dkappa, dK, dA;
+} dh_dparams;
+
+/* ---- the four calls of the north star (+ dh_run_vjp, which consumes dh_run's checkpoints) ------------------- */
+
+/* Create a context for an N^3 grid in a periodic box of side `box` (h^-1 Mpc) with adiabatic index gamma.
+ * Builds the cuFFT R2C/C2R plans and scratch meshes.  grid_n must be a multiple of 4, 8 <= grid_n <= 1024.
+ * Errors: DH_ERR_INVALID, DH_ERR_NO_DEVICE, DH_ERR_CUFFT, DH_ERR_OOM. */
+int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmology* cosmo, const dh_options* opt);
+int dh_free(dh_ctx* ctx);
+
+/* One coupled step in place (Eq. 2-3, 8-18):
+ *   S1 delta_tot = rho_gas - rho_bar + CIC deposit of the particles
+ *   S2 g'_d = IFFT( i k_d A delta^ / k^2 )
+ *   S3 w += K g'(x);  x += w Dtau/dx, wrapped                            (Eq. 2-3)
+ *   S4 three 1-D relaxing-TVD sweeps in Strang order, each with its gravity source (Eq. 8-18)
+ * dt = cosmic-time length of the step, a = scale factor at the END of the step.
+ * cfl_cmax_out: DEVICE pointer to 3 floats (or NULL): max freezing speed |v~_d| + c~_s over the input of each of
+ * the three sweeps, in sweep order (Eq. 19-20).  Asynchronous. */
+int dh_step(dh_ctx* ctx, dh_state* state, double dt, double a, float* cfl_cmax_out);
+
+/* Reverse-mode adjoint of dh_step.  state_checkpoint: the step's INPUT state (its a, dt_prev, step are used; its
+ * arrays are read only); intermediates are recomputed.  cotangent_out: cotangent of the step's OUTPUT state (read
+ * only).  cotangent_in: receives the cotangent of the INPUT state (overwritten; may alias cotangent_out).
+ * dparams: accumulated.  Synchronises the stream (host scalars are returned). */
+int dh_step_vjp(dh_ctx* ctx, const dh_state* state_checkpoint, double dt, double a, const dh_cot* cotangent_out,
+                dh_cot* cotangent_in, dh_dparams* dparams);
+
+/* n_steps forward steps; a_sched[k] = scale factor at the END of step k, dt_sched[k] = its cosmic-time length (host
+ * arrays).  checkpoint_stride > 0: a snapshot of the state is stored in the context before steps 0, stride,
+ * 2 stride, ... for dh_run_vjp; <= 0: none.  The per-sweep CFL maxima are kept in the context
+ * (dh_get_cmax).  Synchronises at the end and returns DH_ERR_NONFINITE if any maximum is NaN/Inf. */
+int dh_run(dh_ctx* ctx, dh_state* state, const double* a_sched, const double* dt_sched, int n_steps,
+           int checkpoint_stride);
+
+/* Reverse sweep over the last checkpointed dh_run: for each segment (last first) re-run the forward from its
+ * snapshot keeping every step's input, then apply the step VJP in reverse (recompute-from-checkpoint schedule).
+ * cot_final: cotangent of the final state (read only); cot_initial: cotangent of the initial state (overwritten; may
+ * alias cot_final); dparams accumulated.  Synchronises. */
+int dh_run_vjp(dh_ctx* ctx, const dh_cot* cot_final, dh_cot* cot_initial, dh_dparams* dparams);
+
+/* ---- host-buffer variants (end-to-end path: host <-> device copies inside the call) ------------------------- */
+
+/* gas_host: 5 N^3 floats, part_host: 6 N_p floats (HOST, pinned or pageable), updated in place with the final state.
+ * a, dt_prev, step: host scalars of the state, updated. */
+int dh_run_host(dh_ctx* ctx, float* gas_host, float* part_host, double* a, double* dt_prev, int64_t* step,
+                const double* a_sched, const double* dt_sched, int n_steps, int checkpoint_stride);
+/* cot_gas_host / cot_part_host: cotangent of the final state on entry, of the initial state on exit (HOST). */
+int dh_run_vjp_host(dh_ctx* ctx, float* cot_gas_host, float* cot_part_host, dh_dparams* dparams);
+
+/* ---- helpers ------------------------------------------------------------------------------------------------ */
+const char* dh_last_error(void);
+/* out (HOST): 3 * n floats, the CFL maxima of the last dh_run's first n steps. */
+int dh_get_cmax(dh_ctx* ctx, float* out, int n);
+/* Uniform-in-ln(a) schedule: a_out[0..n] = a0 exp(k r), dt_out[k] = t(a_{k+1}) - t(a_k); EdS closed form, else
+ * Simpson quadrature of dt = da / (a H(a)).  HOST arrays. */
+int dh_schedule_lna(const dh_cosmology* cosmo, double a0, double a1, int n, double* a_out, double* dt_out);
+/* Per-step factors of reading R15: out[4] = (Dtau, kappa, K, A).  HOST. */
+int dh_step_scalars(const dh_cosmology* cosmo, double a_i, double a_next, double dt, double dt_prev, double* out);
+/* CIC cell indices of n fp32 positions (DEVICE in, DEVICE out): i0 = floor(x - 1/2) mod N, i1 = (i0 + 1) mod N, the
+ * very function the deposit / gather kernels use (bit-exact test, reading R22). */
+int dh_debug_cell_index(dh_ctx* ctx, const float* x_dev, int64_t n, int32_t* i0_dev, int32_t* i1_dev);
+/* Bytes of device memory the context currently holds (scratch + snapshots). */
+int64_t dh_device_bytes(dh_ctx* ctx);
+/* Number of kernels this library has launched on the context since dh_init (the gpu_launches count of bench.py);
+ * cuFFT's internal kernels are not counted. */
+int64_t dh_launch_count(dh_ctx* ctx);
+int dh_sync(dh_ctx* ctx);
+
+/* ---- single kernels of the path (same kernels dh_step / dh_step_vjp launch; for parity tests and profiling) --
+ * All pointers DEVICE.  d = sweep axis 0/1/2 = x/y/z.  lam = Dtau/dx, kap = kappa. */
+/* SWEEP_d: gas_out = sweep(gas_in, g) (g may be NULL: no source); cmax_out: 1 float, max-combined (caller zeroes). */
+int dh_sweep(dh_ctx* ctx, int d, float* const gas_in[5], const float* g, double lam, double kap, float* const gas_out[5],
+             float* cmax_out);
+/* Adjoint of SWEEP_d: cot_in overwritten, g_bar overwritten (may be NULL iff g is NULL);
+ * scal_bar: DEVICE double[3] += (lam_bar, kap_bar, gamma_bar). */
+int dh_sweep_vjp(dh_ctx* ctx, int d, float* const gas_in[5], const float* g, double lam, double kap,
+                 float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar);
+/* delta_tot = [gas_sources_gravity] rho_gas - rho_bar + m_p CIC(pos) (rho_gas may be NULL). */
+int dh_deposit(dh_ctx* ctx, const float* rho_gas, float* const pos[3], float* delta_out);
+/* g'_d (3 meshes) from delta (delta is not modified). */
+int dh_poisson(dh_ctx* ctx, const float* delta, double A, float* const g_out[3]);
+/* delta_bar = sum_d G_d^T g_bar_d. */
+int dh_poisson_vjp(dh_ctx* ctx, float* const g_bar[3], double A, float* delta_bar_out);
+/* S3 in place on part[6]. */
+int dh_kick_drift(dh_ctx* ctx, float* const g[3], float* const part[6], double K, double dtau_over_dx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DIFFHYDRO_H */

@@ -1,0 +1,550 @@
+// api.cu -- the C ABI of libdiffhydro (include/diffhydro.h): context, step scheduler, step VJP, checkpointed run.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "dh_internal.cuh"
+
+namespace dh {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int dev_alloc(dh_ctx* c, void** p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) return DH_OK;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+        return DH_ERR_OOM;
+    }
+    c->bytes += (int64_t)bytes;
+    return DH_OK;
+}
+
+void dev_free(dh_ctx* c, void* p, size_t bytes) {
+    if (p) {
+        cudaFree(p);
+        c->bytes -= (int64_t)bytes;
+    }
+}
+
+// Per-step factors (reading R15): midpoint rule at a_h = sqrt(a_i a_next) for drift int dt/a^2 and kick int dt/a of
+// Eq. 2-3; K is centred on a_i (staggered leapfrog, the first step is the opening half kick).
+StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, double dt, double dt_prev) {
+    StepScalars s;
+    if (co.static_mode) {
+        s.dtau = dt; s.kappa = dt; s.K = 0.5 * (dt_prev + dt);
+    } else {
+        const double ah = std::sqrt(a_i * a_next);
+        s.dtau = dt / (ah * ah);
+        s.kappa = dt / ah;
+        s.K = (dt_prev + dt) / (2.0 * a_i);
+    }
+    s.A = 1.5 * co.Omega_m * co.H0 * co.H0;
+    return s;
+}
+
+static int alloc_fields(dh_ctx* c, float** arr, int n, size_t count) {
+    for (int i = 0; i < n; ++i) DH_TRY(dev_alloc(c, (void**)&arr[i], count * sizeof(float)));
+    return DH_OK;
+}
+
+static int ensure_adjoint_scratch(dh_ctx* c) {
+    if (c->adj_alloc) return DH_OK;
+    if (c->opt.hydro_on) {
+        DH_TRY(alloc_fields(c, c->sw_in[0], 5, c->n3));
+        DH_TRY(alloc_fields(c, c->sw_in[1], 5, c->n3));
+        DH_TRY(alloc_fields(c, c->cot_tmp, 5, c->n3));
+    }
+    if (c->opt.gravity_on) DH_TRY(alloc_fields(c, c->gpb, 3, c->n3));
+    c->adj_alloc = true;
+    return DH_OK;
+}
+
+static size_t state_floats(const dh_ctx* c) { return (size_t)(5 * c->n3 + 6 * c->np); }
+
+static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st) {
+    if (!s.buf) DH_TRY(dev_alloc(c, (void**)&s.buf, state_floats(c) * sizeof(float)));
+    for (int k = 0; k < 5; ++k)
+        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)k * c->n3, st->gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    for (int k = 0; k < 6 && c->np > 0; ++k)
+        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)5 * c->n3 + (size_t)k * c->np, st->part[k], c->np * sizeof(float),
+                                cudaMemcpyDeviceToDevice, c->stream));
+    s.a = st->a; s.dt_prev = st->dt_prev; s.step = st->step;
+    return DH_OK;
+}
+
+static void snapshot_view(const dh_ctx* c, const Snapshot& s, dh_state* st) {
+    for (int k = 0; k < 5; ++k) st->gas[k] = s.buf + (size_t)k * c->n3;
+    for (int k = 0; k < 6; ++k) st->part[k] = s.buf + (size_t)5 * c->n3 + (size_t)k * c->np;
+    st->a = s.a; st->dt_prev = s.dt_prev; st->step = s.step;
+}
+
+static void free_snaps(dh_ctx* c, std::vector<Snapshot>& v) {
+    for (auto& s : v) dev_free(c, s.buf, state_floats(c) * sizeof(float));
+    v.clear();
+}
+
+// S1 + S2: delta_tot and g' from the state's gas density and particle positions.
+static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A) {
+    DH_TRY(launch_deposit(c, gas[0], part[0], part[1], part[2], c->delta));
+    DH_TRY(poisson_forward(c, c->delta, A, c->gp));
+    return DH_OK;
+}
+
+// The forward step on explicit arrays.  If sweep_inputs != nullptr the inputs of sweeps 2 and 3 are kept there and the
+// particle update is skipped when `skip_particles` (the reverse pass only needs g' and the sweep inputs).
+static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], const StepScalars& s, int64_t step,
+                       float* cmax3, bool skip_particles, float* (*sweep_inputs)[5], bool last_sweep_needed) {
+    const bool grav = c->opt.gravity_on != 0;
+    if (grav) DH_TRY(compute_gravity(c, gas, part, (float)s.A));
+    if (c->np > 0 && !skip_particles)
+        DH_TRY(launch_kick_drift(c, grav ? c->gp : nullptr, part, (float)s.K, (float)(s.dtau / c->dx)));
+    if (c->opt.hydro_on) {
+        const int* order = STRANG[((step % 6) + 6) % 6];
+        const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
+        // gas -> tmp -> tmp2 -> gas: every sweep reads and writes each field once, no copy back; the reverse pass keeps
+        // the two intermediate states (inputs of sweeps 2 and 3) in its own buffers instead
+        float* cur[5]; float* nxt[5];
+        for (int k = 0; k < 5; ++k) cur[k] = gas[k];
+        for (int sidx = 0; sidx < 3; ++sidx) {
+            if (sidx == 2 && !last_sweep_needed) break;
+            const int d = order[sidx];
+            for (int k = 0; k < 5; ++k)
+                nxt[k] = sidx == 2 ? gas[k] : (sweep_inputs ? sweep_inputs[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
+            DH_TRY(launch_sweep(c, d, cur, grav ? c->gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr));
+            for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
+        }
+    }
+    return DH_OK;
+}
+
+static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_in[6], const StepScalars& s, int64_t step,
+                           float* const cot_gas_out[5], float* const cot_part_out[6], float* const cot_gas_in[5],
+                           float* const cot_part_in[6]) {
+    DH_TRY(ensure_adjoint_scratch(c));
+    const bool grav = c->opt.gravity_on != 0;
+    const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
+    // ---- recompute: g' and the inputs of sweeps 2 and 3 (the third sweep's output is not needed)
+    float* (*swin)[5] = c->sw_in;
+    DH_TRY(step_arrays(c, gas_in, part_in, s, step, nullptr, true, c->opt.hydro_on ? swin : nullptr, false));
+    // ---- S4 reversed
+    if (c->opt.hydro_on) {
+        const int* order = STRANG[((step % 6) + 6) % 6];
+        float* cur[5]; float* nxt[5];
+        for (int k = 0; k < 5; ++k) cur[k] = cot_gas_out[k];
+        for (int sidx = 2; sidx >= 0; --sidx) {
+            const int d = order[sidx];
+            float* const* src = (sidx == 0) ? gas_in : swin[sidx - 1];
+            // the last adjoint sweep writes the caller's cot_gas_in; the others alternate between the two scratch sets
+            if (sidx == 0) for (int k = 0; k < 5; ++k) nxt[k] = cot_gas_in[k];
+            else if (sidx == 2) for (int k = 0; k < 5; ++k) nxt[k] = c->cot_tmp[k];
+            else for (int k = 0; k < 5; ++k) nxt[k] = c->gas_tmp[k];
+            DH_TRY(launch_sweep_vjp(c, d, src, grav ? c->gp[d] : nullptr, lam, kap, cur, nxt, grav ? c->gpb[d] : nullptr,
+                                    c->scal_dev));
+            for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
+        }
+    } else {
+        for (int k = 0; k < 5; ++k)
+            if (cot_gas_in[k] != cot_gas_out[k])
+                DH_CUDA(cudaMemcpyAsync(cot_gas_in[k], cot_gas_out[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+        if (grav) for (int d = 0; d < 3; ++d) DH_TRY(launch_fill(c, c->gpb[d], c->n3, 0.f));
+    }
+    // ---- S3 reversed (vector deposit adds to the g'_bar the sweeps wrote)
+    if (c->np > 0) {
+        DH_TRY(launch_kick_drift_vjp(c, grav ? c->gp : nullptr, part_in, cot_part_out, cot_part_in, c->gpb, (float)s.K,
+                                     (float)(s.dtau / c->dx), c->scal_dev));
+    }
+    // ---- S2, S1 reversed
+    if (grav) {
+        if (c->opt.want_dA) DH_TRY(launch_dot3(c, c->gpb, c->gp, 1.0 / s.A, c->scal_dev + 5));
+        DH_TRY(poisson_adjoint(c, c->gpb, (float)s.A, c->delta));
+        DH_TRY(launch_deposit_vjp(c, c->delta, part_in, cot_gas_in[0], cot_part_in));
+    }
+    return DH_OK;
+}
+
+// fold the device scalar accumulators into dparams: scal = (lam_b, kap_b, gamma_b, K_b, (dtau/dx)_b, A_b)
+static int harvest_scalars(dh_ctx* c, dh_dparams* dp) {
+    double h[8];
+    DH_CUDA(cudaMemcpyAsync(h, c->scal_dev, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    if (dp) {
+        dp->dgamma += h[2];
+        dp->dDtau += (h[0] + h[4]) / c->dx;
+        dp->dkappa += h[1];
+        dp->dK += h[3];
+        dp->dA += h[5];
+    }
+    DH_CUDA(cudaMemsetAsync(c->scal_dev, 0, 8 * sizeof(double), c->stream));
+    return DH_OK;
+}
+
+static int check_state(const dh_ctx* c, const float* const gas[5], const float* const part[6]) {
+    for (int k = 0; k < 5; ++k) if (!gas[k]) { set_error("null gas pointer %d", k); return DH_ERR_INVALID; }
+    if (c->np > 0) for (int k = 0; k < 6; ++k) if (!part[k]) { set_error("null particle pointer %d", k); return DH_ERR_INVALID; }
+    return DH_OK;
+}
+
+}  // namespace dh
+
+using namespace dh;
+
+extern "C" {
+
+const char* dh_last_error(void) { return g_err; }
+
+int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmology* cosmo, const dh_options* opt) {
+    if (!out || !cosmo || !opt) { set_error("dh_init: null argument"); return DH_ERR_INVALID; }
+    *out = nullptr;
+    if (grid_n < 32 || grid_n > 1024 || grid_n % 32 != 0) {
+        set_error("dh_init: grid_n must be a multiple of 32 in [32, 1024], got %d", grid_n);
+        return DH_ERR_INVALID;
+    }
+    if (!(box > 0) || !(gamma > 1.0) || !(opt->e_floor > 0) || opt->n_part_side < 0) {
+        set_error("dh_init: need box > 0, gamma > 1, e_floor > 0, n_part_side >= 0");
+        return DH_ERR_INVALID;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        set_error("dh_init: no CUDA device (this library has no CPU fallback)");
+        return DH_ERR_NO_DEVICE;
+    }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    DH_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) {
+        set_error("dh_init: device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
+        return DH_ERR_NO_DEVICE;
+    }
+    dh_ctx* c = new (std::nothrow) dh_ctx();
+    if (!c) return DH_ERR_OOM;
+    c->N = grid_n;
+    c->n3 = (int64_t)grid_n * grid_n * grid_n;
+    c->nps = opt->n_part_side;
+    c->np = (int64_t)c->nps * c->nps * c->nps;
+    c->box = box; c->gamma = gamma; c->dx = box / grid_n;
+    c->cosmo = *cosmo; c->opt = *opt;
+    c->f_b = cosmo->Omega_m > 0 ? cosmo->Omega_b / cosmo->Omega_m : 0.0;
+    c->m_p = c->np > 0 ? (1.0 - c->f_b) * (double)c->n3 / (double)c->np : 0.0;
+    c->rho_bar = (c->np > 0 ? 1.0 - c->f_b : 0.0) + (opt->gas_sources_gravity ? c->f_b : 0.0);
+    c->sm_count = prop.multiProcessorCount;
+    // NULL = the legacy default stream, which orders with the caller's default-stream work (torch's current stream is
+    // stream 0 unless the caller changed it); a private non-blocking stream would race with it.
+    c->stream = (cudaStream_t)opt->cuda_stream;
+    int rc = DH_OK;
+    auto fail = [&](int code) { dh_free(c); return code; };
+    if (opt->gravity_on) {
+        const size_t nspec = (size_t)grid_n * grid_n * (grid_n / 2 + 1);
+        if ((rc = dev_alloc(c, (void**)&c->delta, c->n3 * sizeof(float))) != DH_OK) return fail(rc);
+        for (int i = 0; i < 4; ++i)
+            if ((rc = dev_alloc(c, (void**)&c->spec[i], nspec * sizeof(float2))) != DH_OK) return fail(rc);
+        if ((rc = alloc_fields(c, c->gp, 3, c->n3)) != DH_OK) return fail(rc);
+        // cuFFT plans share one work area
+        size_t w1 = 0, w2 = 0;
+        if (cufftCreate(&c->plan_r2c) != CUFFT_SUCCESS || cufftCreate(&c->plan_c2r) != CUFFT_SUCCESS) {
+            set_error("cufftCreate failed"); return fail(DH_ERR_CUFFT);
+        }
+        c->plans = true;
+        cufftSetAutoAllocation(c->plan_r2c, 0);
+        cufftSetAutoAllocation(c->plan_c2r, 0);
+        if (cufftMakePlan3d(c->plan_r2c, grid_n, grid_n, grid_n, CUFFT_R2C, &w1) != CUFFT_SUCCESS ||
+            cufftMakePlan3d(c->plan_c2r, grid_n, grid_n, grid_n, CUFFT_C2R, &w2) != CUFFT_SUCCESS) {
+            set_error("cufftMakePlan3d(%d^3) failed", grid_n); return fail(DH_ERR_CUFFT);
+        }
+        c->fft_work_bytes = w1 > w2 ? w1 : w2;
+        if (c->fft_work_bytes > 0) {
+            if ((rc = dev_alloc(c, &c->fft_work, c->fft_work_bytes)) != DH_OK) return fail(rc);
+            cufftSetWorkArea(c->plan_r2c, c->fft_work);
+            cufftSetWorkArea(c->plan_c2r, c->fft_work);
+        }
+        if (cufftSetStream(c->plan_r2c, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_c2r, c->stream) != CUFFT_SUCCESS) {
+            set_error("cufftSetStream failed"); return fail(DH_ERR_CUFFT);
+        }
+    }
+    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp, 5, c->n3)) != DH_OK) return fail(rc);
+    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp2, 5, c->n3)) != DH_OK) return fail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->cmax_step, 3 * sizeof(float))) != DH_OK) return fail(rc);
+    if ((rc = dev_alloc(c, (void**)&c->scal_dev, 8 * sizeof(double))) != DH_OK) return fail(rc);
+    if (cudaMemsetAsync(c->scal_dev, 0, 8 * sizeof(double), c->stream) != cudaSuccess) return fail(DH_ERR_CUDA);
+    *out = c;
+    return DH_OK;
+}
+
+int dh_free(dh_ctx* c) {
+    if (!c) return DH_OK;
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    if (c->plans) { cufftDestroy(c->plan_r2c); cufftDestroy(c->plan_c2r); }
+    cudaFree(c->fft_work);
+    cudaFree(c->delta);
+    for (auto p : c->spec) cudaFree(p);
+    for (auto p : c->gp) cudaFree(p);
+    for (auto p : c->gas_tmp) cudaFree(p);
+    for (auto p : c->gas_tmp2) cudaFree(p);
+    for (int i = 0; i < 2; ++i) for (auto p : c->sw_in[i]) cudaFree(p);
+    for (auto p : c->gpb) cudaFree(p);
+    for (auto p : c->cot_tmp) cudaFree(p);
+    for (auto p : c->part_tmp) cudaFree(p);
+    cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev);
+    cudaFree(c->hv_state); cudaFree(c->hv_cot);
+    for (auto& s : c->snaps) cudaFree(s.buf);
+    for (auto& s : c->seg) cudaFree(s.buf);
+    if (c->own_stream) cudaStreamDestroy(c->stream);
+    cudaGetLastError();
+    delete c;
+    return DH_OK;
+}
+
+int dh_sync(dh_ctx* c) {
+    if (!c) return DH_ERR_INVALID;
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    return DH_OK;
+}
+
+int64_t dh_device_bytes(dh_ctx* c) { return c ? c->bytes : 0; }
+int64_t dh_launch_count(dh_ctx* c) { return c ? c->launches : 0; }
+
+int dh_step_scalars(const dh_cosmology* cosmo, double a_i, double a_next, double dt, double dt_prev, double* out) {
+    if (!cosmo || !out) return DH_ERR_INVALID;
+    StepScalars s = step_scalars(*cosmo, a_i, a_next, dt, dt_prev);
+    out[0] = s.dtau; out[1] = s.kappa; out[2] = s.K; out[3] = s.A;
+    return DH_OK;
+}
+
+int dh_schedule_lna(const dh_cosmology* co, double a0, double a1, int n, double* a_out, double* dt_out) {
+    if (!co || !a_out || !dt_out || n <= 0 || !(a0 > 0) || !(a1 > a0)) { set_error("dh_schedule_lna: bad argument"); return DH_ERR_INVALID; }
+    const double r = std::log(a1 / a0) / n;
+    for (int k = 0; k <= n; ++k) a_out[k] = a0 * std::exp(k * r);
+    a_out[n] = a1;
+    const bool eds = co->Omega_L == 0.0 && std::fabs(co->Omega_m - 1.0) < 1e-15;
+    for (int k = 0; k < n; ++k) {
+        const double lo = a_out[k], hi = a_out[k + 1];
+        if (eds) {
+            // t = 2 / (3 H0) a^{3/2}
+            dt_out[k] = (2.0 / (3.0 * co->H0)) * (hi * std::sqrt(hi) - lo * std::sqrt(lo));
+        } else {
+            // dt = d ln a / H(a): composite Simpson in ln a
+            const int M = 2048;
+            const double h = std::log(hi / lo) / M, Ok = 1.0 - co->Omega_m - co->Omega_L;
+            double acc = 0.0;
+            for (int j = 0; j <= M; ++j) {
+                const double a = lo * std::exp(j * h);
+                const double H = co->H0 * std::sqrt(co->Omega_m / (a * a * a) + Ok / (a * a) + co->Omega_L);
+                acc += ((j == 0 || j == M) ? 1.0 : ((j & 1) ? 4.0 : 2.0)) / H;
+            }
+            dt_out[k] = acc * h / 3.0;
+        }
+    }
+    return DH_OK;
+}
+
+int dh_step(dh_ctx* c, dh_state* st, double dt, double a, float* cfl_cmax_out) {
+    if (!c || !st) { set_error("dh_step: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(check_state(c, st->gas, st->part));
+    const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
+    float* cm = cfl_cmax_out ? cfl_cmax_out : c->cmax_step;
+    DH_CUDA(cudaMemsetAsync(cm, 0, 3 * sizeof(float), c->stream));
+    DH_TRY(step_arrays(c, st->gas, st->part, s, st->step, cm, false, nullptr, true));
+    st->a = c->cosmo.static_mode ? 1.0 : a;
+    st->dt_prev = dt;
+    st->step += 1;
+    return DH_OK;
+}
+
+int dh_step_vjp(dh_ctx* c, const dh_state* st, double dt, double a, const dh_cot* cot_out, dh_cot* cot_in, dh_dparams* dp) {
+    if (!c || !st || !cot_out || !cot_in) { set_error("dh_step_vjp: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(check_state(c, st->gas, st->part));
+    DH_TRY(check_state(c, cot_out->gas, cot_out->part));
+    DH_TRY(check_state(c, cot_in->gas, cot_in->part));
+    const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
+    DH_TRY(step_vjp_arrays(c, st->gas, st->part, s, st->step, cot_out->gas, cot_out->part, cot_in->gas, cot_in->part));
+    return harvest_scalars(c, dp);
+}
+
+int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sched, int n_steps, int stride) {
+    if (!c || !st || !a_sched || !dt_sched || n_steps < 0) { set_error("dh_run: bad argument"); return DH_ERR_INVALID; }
+    DH_TRY(check_state(c, st->gas, st->part));
+    if (n_steps > c->cmax_cap) {
+        dev_free(c, c->cmax_log, (size_t)3 * c->cmax_cap * sizeof(float));
+        c->cmax_log = nullptr; c->cmax_cap = 0;
+        DH_TRY(dev_alloc(c, (void**)&c->cmax_log, (size_t)3 * n_steps * sizeof(float)));
+        c->cmax_cap = n_steps;
+    }
+    if (n_steps > 0) DH_CUDA(cudaMemsetAsync(c->cmax_log, 0, (size_t)3 * n_steps * sizeof(float), c->stream));
+    c->cmax_n = n_steps;
+    c->run_valid = false;
+    const int nseg = stride > 0 ? (n_steps + stride - 1) / stride : 0;
+    if ((int)c->snaps.size() > nseg) {
+        for (size_t i = nseg; i < c->snaps.size(); ++i) dev_free(c, c->snaps[i].buf, state_floats(c) * sizeof(float));
+    }
+    c->snaps.resize(nseg);
+    c->run_a.assign(a_sched, a_sched + n_steps);
+    c->run_dt.assign(dt_sched, dt_sched + n_steps);
+    c->run_n = n_steps; c->run_stride = stride;
+    for (int k = 0; k < n_steps; ++k) {
+        if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
+        const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
+        DH_TRY(step_arrays(c, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, false, nullptr, true));
+        st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
+        st->dt_prev = dt_sched[k];
+        st->step += 1;
+    }
+    // one synchronisation per run: fetch the CFL log and look for NaN/Inf
+    if (n_steps > 0) {
+        std::vector<float> h((size_t)3 * n_steps);
+        DH_CUDA(cudaMemcpyAsync(h.data(), c->cmax_log, h.size() * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+        DH_CUDA(cudaStreamSynchronize(c->stream));
+        for (size_t i = 0; i < h.size(); ++i)
+            if (!std::isfinite(h[i])) {
+                set_error("dh_run: non-finite CFL maximum at step %zu, sweep %zu", i / 3, i % 3);
+                return DH_ERR_NONFINITE;
+            }
+    }
+    c->run_valid = stride > 0;
+    return DH_OK;
+}
+
+int dh_get_cmax(dh_ctx* c, float* out, int n) {
+    if (!c || !out || n < 0 || n > c->cmax_n) { set_error("dh_get_cmax: bad argument"); return DH_ERR_INVALID; }
+    if (n == 0) return DH_OK;
+    DH_CUDA(cudaMemcpyAsync(out, c->cmax_log, (size_t)3 * n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    return DH_OK;
+}
+
+int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dparams* dp) {
+    if (!c || !cot_final || !cot_initial) { set_error("dh_run_vjp: null argument"); return DH_ERR_INVALID; }
+    if (!c->run_valid) { set_error("dh_run_vjp: no checkpointed dh_run to differentiate"); return DH_ERR_STATE; }
+    DH_TRY(check_state(c, cot_final->gas, cot_final->part));
+    DH_TRY(check_state(c, cot_initial->gas, cot_initial->part));
+    const int n = c->run_n, stride = c->run_stride;
+    const int nseg = (n + stride - 1) / stride;
+    // cot_initial doubles as the running cotangent
+    for (int k = 0; k < 5; ++k)
+        if (cot_initial->gas[k] != cot_final->gas[k])
+            DH_CUDA(cudaMemcpyAsync(cot_initial->gas[k], cot_final->gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    for (int k = 0; k < 6 && c->np > 0; ++k)
+        if (cot_initial->part[k] != cot_final->part[k])
+            DH_CUDA(cudaMemcpyAsync(cot_initial->part[k], cot_final->part[k], c->np * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    if ((int)c->seg.size() < stride) c->seg.resize(stride);
+    for (int sgi = nseg - 1; sgi >= 0; --sgi) {
+        const int k0 = sgi * stride, k1 = (k0 + stride < n) ? k0 + stride : n;
+        // ---- re-run the segment from its snapshot, keeping every step's input (seg[0] aliases the snapshot itself)
+        dh_state cur;
+        snapshot_view(c, c->snaps[sgi], &cur);
+        for (int k = k0; k < k1 - 1; ++k) {
+            Snapshot& nx = c->seg[k - k0 + 1];
+            DH_TRY(snapshot_store(c, nx, &cur));          // copy, then advance the copy in place
+            dh_state adv;
+            snapshot_view(c, nx, &adv);
+            const StepScalars s = step_scalars(c->cosmo, adv.a, c->run_a[k], c->run_dt[k], adv.dt_prev);
+            DH_TRY(step_arrays(c, adv.gas, adv.part, s, adv.step, nullptr, false, nullptr, true));
+            nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
+            nx.dt_prev = c->run_dt[k];
+            nx.step = adv.step + 1;
+            snapshot_view(c, nx, &cur);
+        }
+        // ---- step VJPs, last step of the segment first
+        for (int k = k1 - 1; k >= k0; --k) {
+            dh_state in;
+            snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
+            const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
+            DH_TRY(step_vjp_arrays(c, in.gas, in.part, s, in.step, cot_initial->gas, cot_initial->part, cot_initial->gas,
+                                   cot_initial->part));
+        }
+    }
+    return harvest_scalars(c, dp);
+}
+
+// ---------------------------------------------------------------------------------------------- host variants ----
+static int hv_ensure(dh_ctx* c, float** buf) {
+    if (!*buf) DH_TRY(dev_alloc(c, (void**)buf, state_floats(c) * sizeof(float)));
+    return DH_OK;
+}
+
+int dh_run_host(dh_ctx* c, float* gas_host, float* part_host, double* a, double* dt_prev, int64_t* step,
+                const double* a_sched, const double* dt_sched, int n_steps, int stride) {
+    if (!c || !gas_host || !a || !dt_prev || !step || (c->np > 0 && !part_host)) { set_error("dh_run_host: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(hv_ensure(c, &c->hv_state));
+    dh_state st;
+    for (int k = 0; k < 5; ++k) st.gas[k] = c->hv_state + (size_t)k * c->n3;
+    for (int k = 0; k < 6; ++k) st.part[k] = c->hv_state + (size_t)5 * c->n3 + (size_t)k * c->np;
+    st.a = *a; st.dt_prev = *dt_prev; st.step = *step;
+    DH_CUDA(cudaMemcpyAsync(st.gas[0], gas_host, (size_t)5 * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    if (c->np > 0) DH_CUDA(cudaMemcpyAsync(st.part[0], part_host, (size_t)6 * c->np * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    DH_TRY(dh_run(c, &st, a_sched, dt_sched, n_steps, stride));
+    DH_CUDA(cudaMemcpyAsync(gas_host, st.gas[0], (size_t)5 * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    if (c->np > 0) DH_CUDA(cudaMemcpyAsync(part_host, st.part[0], (size_t)6 * c->np * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    *a = st.a; *dt_prev = st.dt_prev; *step = st.step;
+    return DH_OK;
+}
+
+int dh_run_vjp_host(dh_ctx* c, float* cot_gas_host, float* cot_part_host, dh_dparams* dp) {
+    if (!c || !cot_gas_host || (c->np > 0 && !cot_part_host)) { set_error("dh_run_vjp_host: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(hv_ensure(c, &c->hv_cot));
+    dh_cot ct;
+    for (int k = 0; k < 5; ++k) ct.gas[k] = c->hv_cot + (size_t)k * c->n3;
+    for (int k = 0; k < 6; ++k) ct.part[k] = c->hv_cot + (size_t)5 * c->n3 + (size_t)k * c->np;
+    DH_CUDA(cudaMemcpyAsync(ct.gas[0], cot_gas_host, (size_t)5 * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    if (c->np > 0) DH_CUDA(cudaMemcpyAsync(ct.part[0], cot_part_host, (size_t)6 * c->np * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    DH_TRY(dh_run_vjp(c, &ct, &ct, dp));
+    DH_CUDA(cudaMemcpyAsync(cot_gas_host, ct.gas[0], (size_t)5 * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    if (c->np > 0) DH_CUDA(cudaMemcpyAsync(cot_part_host, ct.part[0], (size_t)6 * c->np * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    return DH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- single kernels ----
+int dh_debug_cell_index(dh_ctx* c, const float* x_dev, int64_t n, int32_t* i0_dev, int32_t* i1_dev) {
+    if (!c || !x_dev || !i0_dev || !i1_dev || n < 0) { set_error("dh_debug_cell_index: bad argument"); return DH_ERR_INVALID; }
+    return launch_cell_index(c, x_dev, n, i0_dev, i1_dev);
+}
+
+int dh_sweep(dh_ctx* c, int d, float* const gas_in[5], const float* g, double lam, double kap, float* const gas_out[5],
+             float* cmax_out) {
+    if (!c || d < 0 || d > 2 || !gas_in || !gas_out) { set_error("dh_sweep: bad argument"); return DH_ERR_INVALID; }
+    return launch_sweep(c, d, gas_in, g, (float)lam, (float)kap, gas_out, cmax_out);
+}
+
+int dh_sweep_vjp(dh_ctx* c, int d, float* const gas_in[5], const float* g, double lam, double kap,
+                 float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar) {
+    if (!c || d < 0 || d > 2 || !gas_in || !cot_out || !cot_in || !scal_bar || (g && !g_bar)) {
+        set_error("dh_sweep_vjp: bad argument"); return DH_ERR_INVALID;
+    }
+    return launch_sweep_vjp(c, d, gas_in, g, (float)lam, (float)kap, cot_out, cot_in, g_bar, scal_bar);
+}
+
+int dh_deposit(dh_ctx* c, const float* rho_gas, float* const pos[3], float* delta_out) {
+    if (!c || !delta_out || (c->np > 0 && !pos)) { set_error("dh_deposit: bad argument"); return DH_ERR_INVALID; }
+    return launch_deposit(c, rho_gas, pos ? pos[0] : nullptr, pos ? pos[1] : nullptr, pos ? pos[2] : nullptr, delta_out);
+}
+
+int dh_poisson(dh_ctx* c, const float* delta, double A, float* const g_out[3]) {
+    if (!c || !delta || !g_out || !c->plans) { set_error("dh_poisson: bad argument or gravity off"); return DH_ERR_INVALID; }
+    return poisson_forward(c, delta, (float)A, g_out);
+}
+
+int dh_poisson_vjp(dh_ctx* c, float* const g_bar[3], double A, float* delta_bar_out) {
+    if (!c || !g_bar || !delta_bar_out || !c->plans) { set_error("dh_poisson_vjp: bad argument or gravity off"); return DH_ERR_INVALID; }
+    return poisson_adjoint(c, g_bar, (float)A, delta_bar_out);
+}
+
+int dh_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], double K, double dtau_over_dx) {
+    if (!c || !part) { set_error("dh_kick_drift: bad argument"); return DH_ERR_INVALID; }
+    return launch_kick_drift(c, g, part, (float)K, (float)dtau_over_dx);
+}
+
+}  // extern "C"

@@ -1,0 +1,133 @@
+// dh_internal.cuh -- context, error plumbing and launch declarations shared by the .cu files of libdiffhydro.
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <vector>
+
+#include "../../include/diffhydro.h"
+
+namespace dh {
+
+void set_error(const char* fmt, ...);
+
+#define DH_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            dh::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? DH_ERR_OOM : DH_ERR_CUDA;               \
+        }                                                                                      \
+    } while (0)
+
+#define DH_CUFFT(call)                                                              \
+    do {                                                                            \
+        cufftResult r_ = (call);                                                    \
+        if (r_ != CUFFT_SUCCESS) {                                                  \
+            dh::set_error("%s:%d: %s -> cufft error %d", __FILE__, __LINE__, #call, (int)r_); \
+            return DH_ERR_CUFFT;                                                    \
+        }                                                                           \
+    } while (0)
+
+#define DH_TRY(call)            \
+    do {                        \
+        int rc_ = (call);       \
+        if (rc_ != DH_OK) return rc_; \
+    } while (0)
+
+// Strang table (reading R9): step n uses STRANG[n mod 6].
+static const int STRANG[6][3] = {{0, 1, 2}, {2, 1, 0}, {2, 0, 1}, {1, 0, 2}, {1, 2, 0}, {0, 2, 1}};
+
+struct StepScalars { double dtau, kappa, K, A; };
+
+struct Snapshot {
+    float* buf = nullptr;   // 5 N^3 + 6 N_p floats
+    double a = 0, dt_prev = 0;
+    int64_t step = 0;
+};
+
+}  // namespace dh
+
+struct dh_ctx {
+    int N = 0;
+    int64_t n3 = 0, np = 0;
+    int nps = 0;
+    double box = 0, gamma = 0, dx = 0;
+    dh_cosmology cosmo{};
+    dh_options opt{};
+    double f_b = 0, m_p = 0, rho_bar = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    int sm_count = 148;
+    int64_t launches = 0;
+    int64_t bytes = 0;
+
+    cufftHandle plan_r2c = 0, plan_c2r = 0;
+    bool plans = false;
+    void* fft_work = nullptr;
+    size_t fft_work_bytes = 0;
+
+    // scratch
+    float* delta = nullptr;        // N^3 real (Poisson source / delta_bar)
+    float2* spec[4] = {nullptr, nullptr, nullptr, nullptr};   // half spectra: [0] delta^, [1..3] g^_d
+    float* gp[3] = {nullptr, nullptr, nullptr};               // g'_d
+    float* gas_tmp[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // output of sweep 1
+    float* gas_tmp2[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // output of sweep 2 (sweep 3 writes the state)
+    float* cmax_step = nullptr;    // 3 floats (device) for dh_step when the caller passes NULL
+    float* cmax_log = nullptr;     // 3 * cmax_cap floats
+    int cmax_cap = 0;
+    int cmax_n = 0;
+    double* scal_dev = nullptr;    // 8 doubles: (lam_b, kap_b, gamma_b, K_b, dtau_drift_b, A_b, spare, spare)
+
+    // adjoint scratch (allocated on first use)
+    float* sw_in[2][5] = {};       // inputs of sweeps 2 and 3
+    float* gpb[3] = {nullptr, nullptr, nullptr};   // cotangent of g'
+    float* cot_tmp[5] = {};        // cotangent ping-pong
+    float* part_tmp[6] = {};       // particle scratch for the recompute
+    bool adj_alloc = false;
+
+    // checkpoints of the last dh_run
+    std::vector<dh::Snapshot> snaps;     // segment snapshots
+    std::vector<dh::Snapshot> seg;       // per-step inputs inside one segment (reverse pass)
+    std::vector<double> run_a, run_dt;
+    int run_n = 0, run_stride = 0;
+    double run_a0 = 0, run_dtprev0 = 0;
+    int64_t run_step0 = 0;
+    bool run_valid = false;
+
+    // host-variant device buffers
+    float* hv_state = nullptr;     // 5 N^3 + 6 N_p
+    float* hv_cot = nullptr;
+};
+
+namespace dh {
+
+int dev_alloc(dh_ctx* c, void** p, size_t bytes);
+void dev_free(dh_ctx* c, void* p, size_t bytes);
+
+StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, double dt, double dt_prev);
+
+// ---- kernels (sweep.cu) ----
+int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
+                 float* cmax);
+int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap,
+                     float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar);
+// ---- kernels (pm.cu) ----
+int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta);
+int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]);
+int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat);
+int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float K, float dtau_dx);
+int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6], float* const cot_out[6],
+                          float* const cot_in[6], float* const gbar[3], float K, float dtau_dx, double* scal_bar);
+int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6], float* rho_bar_gas,
+                       float* const xbar[3]);
+int launch_dot3(dh_ctx* c, float* const a[3], float* const b[3], double scale, double* out);
+int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t* i1);
+int launch_fill(dh_ctx* c, float* p, int64_t n, float v);
+
+int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]);
+int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar);
+
+}  // namespace dh

@@ -1,0 +1,509 @@
+// pm.cu -- particle-mesh kernels (forward and adjoint) for sm_100a.
+//
+//   deposit      : delta_tot = [gas] rho_gas - rho_bar + m_p sum_p W(x_p - cell)      cloud in cell
+//   green        : g^_d(k) = i k~_d A delta^(k) / (k^2 N^3)                            PAPER.md:71, :83, reading R12
+//   kick_drift   : w += K g'(x);  x += w Dtau/dx, wrapped to [0, N)                    Eq. 2-3
+// and their transposes.  CIC convention (reading R13): mesh values live at cell centres (i + 1/2), so s = x - 1/2,
+// i0 = floor(s), f = s - i0, i1 = i0 + 1, both wrapped mod N, weights (1-f | f) per axis; the same (i0, f) serve
+// deposit and gather, so there is no self-force.  cuFFT does the 3-D R2C / C2R transforms only.
+#include "dh_internal.cuh"
+
+namespace dh {
+
+// ------------------------------------------------------------------------------------------------- CIC index ----
+struct Cic {
+    int i0[3], i1[3];
+    float f[3];
+};
+
+// i0 = floor(x - 0.5) mod N.  x - 0.5f is exact in fp32 for x >= 0.25 and cannot round across an integer below that,
+// so this integer is bit-identical to the fp64 evaluation on the same fp32 input (reading R22).
+__device__ __forceinline__ void cic_axis(float x, int N, int& i0, int& i1, float& f) {
+    const float s = x - 0.5f;
+    const float fl = floorf(s);
+    f = s - fl;
+    int i = (int)fl;
+    i = i < 0 ? i + N : i;
+    i = i >= N ? i - N : i;
+    i0 = i;
+    i1 = (i + 1 == N) ? 0 : i + 1;
+}
+
+__device__ __forceinline__ Cic cic_of(float x, float y, float z, int N) {
+    Cic c;
+    cic_axis(x, N, c.i0[0], c.i1[0], c.f[0]);
+    cic_axis(y, N, c.i0[1], c.i1[1], c.f[1]);
+    cic_axis(z, N, c.i0[2], c.i1[2], c.f[2]);
+    return c;
+}
+
+__global__ void cell_index_kernel(const float* __restrict__ x, int64_t n, int N, int32_t* i0, int32_t* i1) {
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    int a, b; float f;
+    cic_axis(x[p], N, a, b, f);
+    i0[p] = a; i1[p] = b;
+}
+
+__global__ void fill_kernel(float* p, int64_t n, float v) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; i < n; i += stride) p[i] = v;
+}
+
+// --------------------------------------------------------------------------------------------------- deposit ----
+// delta = flag * rho_gas - rho_bar  (replaces the memset of the mesh)
+__global__ void source_init_kernel(const float4* __restrict__ rho, float4* __restrict__ delta, int64_t n4, float flag,
+                                   float rho_bar) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; i < n4; i += stride) {
+        float4 r = rho ? __ldg(rho + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+        delta[i] = make_float4(fmaf(flag, r.x, -rho_bar), fmaf(flag, r.y, -rho_bar), fmaf(flag, r.z, -rho_bar),
+                               fmaf(flag, r.w, -rho_bar));
+    }
+}
+
+// Particles are stored in lattice order (particle p started at lattice site p) and move only a few cells over a run,
+// so a block of consecutive particles touches a compact brick of the mesh.  Each block accumulates its particles
+// into a shared-memory brick [BZ][BY][BX] anchored at the brick's first lattice site (red.shared), flushes the brick
+// with one red.global per non-zero cell, and sends the rare particle that left the brick straight to global memory.
+// Block = one PX x PY x PZ brick of lattice sites, 256 threads (see launch_deposit for the geometry).
+template <int PX, int PY, int PZ, int M>
+__global__ void __launch_bounds__(256)
+deposit_brick_kernel(const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z, int nps,
+                     int N, float mp, float cell_per_part, float* __restrict__ delta) {
+    // brick of lattice sites [PZ][PY][PX]; mesh tile with margin M cells each side (in mesh cells)
+    constexpr int TX = PX + 2 * M, TY = PY + 2 * M, TZ = PZ + 2 * M;
+    __shared__ float tile[TZ * TY * TX];
+    const int nthr = blockDim.x;
+    for (int i = threadIdx.x; i < TZ * TY * TX; i += nthr) tile[i] = 0.f;
+    __syncthreads();
+    const int nbx = (nps + PX - 1) / PX, nby = (nps + PY - 1) / PY;
+    const int bx = blockIdx.x % nbx, by = (blockIdx.x / nbx) % nby, bz = blockIdx.x / (nbx * nby);
+    // mesh cell of the brick's first lattice site (lattice site q sits at (q + 1/2) * cell_per_part)
+    const int ox = (int)floorf((bx * PX + 0.5f) * cell_per_part - 0.5f) - M;
+    const int oy = (int)floorf((by * PY + 0.5f) * cell_per_part - 0.5f) - M;
+    const int oz = (int)floorf((bz * PZ + 0.5f) * cell_per_part - 0.5f) - M;
+    for (int l = threadIdx.x; l < PX * PY * PZ; l += nthr) {
+        const int lx = l % PX, ly = (l / PX) % PY, lz = l / (PX * PY);
+        const int qx = bx * PX + lx, qy = by * PY + ly, qz = bz * PZ + lz;
+        if (qx >= nps || qy >= nps || qz >= nps) continue;
+        const int64_t p = ((int64_t)qz * nps + qy) * nps + qx;
+        const Cic c = cic_of(__ldg(x + p), __ldg(y + p), __ldg(z + p), N);
+        // tile-relative coordinates of i0 (minimum image with respect to the tile origin)
+        int rx = c.i0[0] - ox, ry = c.i0[1] - oy, rz = c.i0[2] - oz;
+        rx -= N * (int)floorf((float)rx / (float)N);
+        ry -= N * (int)floorf((float)ry / (float)N);
+        rz -= N * (int)floorf((float)rz / (float)N);
+        const bool inside = rx < TX - 1 && ry < TY - 1 && rz < TZ - 1;
+        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {mp * (1.f - c.f[2]), mp * c.f[2]};
+#pragma unroll
+        for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+            for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+                for (int cx = 0; cx < 2; ++cx) {
+                    const float w = wz[cz] * wy[cy] * wx[cx];
+                    if (inside) {
+                        atomicAdd(&tile[((rz + cz) * TY + (ry + cy)) * TX + (rx + cx)], w);
+                    } else {
+                        const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
+                                             (cx ? c.i1[0] : c.i0[0]);
+                        atomicAdd(delta + cell, w);
+                    }
+                }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < TZ * TY * TX; i += nthr) {
+        const float v = tile[i];
+        if (v != 0.f) {
+            int tx = i % TX, ty = (i / TX) % TY, tz = i / (TX * TY);
+            int gx = ox + tx, gy = oy + ty, gz = oz + tz;
+            gx -= N * (int)floorf((float)gx / (float)N);
+            gy -= N * (int)floorf((float)gy / (float)N);
+            gz -= N * (int)floorf((float)gz / (float)N);
+            atomicAdd(delta + ((int64_t)gz * N + gy) * N + gx, v);
+        }
+    }
+}
+
+// ----------------------------------------------------------------------------------------- Green's function ----
+__device__ __forceinline__ int kint(int j, int N) { return j <= N / 2 ? j : j - N; }
+
+// one thread per complex element of the half spectrum [z][y][x <= N/2]
+__device__ __forceinline__ void green_symbol(int64_t c, int N, int nxh, float coef, float& sx, float& sy, float& sz) {
+    const int ix = (int)(c % nxh);
+    const int64_t r = c / nxh;
+    const int iy = (int)(r % N), iz = (int)(r / N);
+    const int nx = ix, ny = kint(iy, N), nz = kint(iz, N);
+    const int n2 = nx * nx + ny * ny + nz * nz;
+    // i k~_d A / k^2 = i n~_d (A L / 2 pi) / n^2 ;  0 at k = 0 ;  n~_d = 0 on the axis-d Nyquist plane
+    const float s = n2 > 0 ? coef / (float)n2 : 0.f;
+    sx = (nx == N / 2) ? 0.f : s * nx;
+    sy = (ny == N / 2) ? 0.f : s * ny;
+    sz = (nz == N / 2) ? 0.f : s * nz;
+}
+
+__global__ void __launch_bounds__(256) green_kernel(const float2* __restrict__ dh, float2* __restrict__ gx,
+                                                    float2* __restrict__ gy, float2* __restrict__ gz, int N,
+                                                    int64_t nspec, float coef /* A L / (2 pi N^3) */) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nspec) return;
+    float sx, sy, sz;
+    green_symbol(c, N, N / 2 + 1, coef, sx, sy, sz);
+    const float2 d = __ldg(dh + c);
+    gx[c] = make_float2(-sx * d.y, sx * d.x);
+    gy[c] = make_float2(-sy * d.y, sy * d.x);
+    gz[c] = make_float2(-sz * d.y, sz * d.x);
+}
+
+// delta_bar^ = sum_d conj(i s_d) g_bar^_d = sum_d s_d (im, -re)
+__global__ void __launch_bounds__(256) green_adj_kernel(const float2* __restrict__ gx, const float2* __restrict__ gy,
+                                                        const float2* __restrict__ gz, float2* __restrict__ db, int N,
+                                                        int64_t nspec, float coef) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nspec) return;
+    float sx, sy, sz;
+    green_symbol(c, N, N / 2 + 1, coef, sx, sy, sz);
+    const float2 a = __ldg(gx + c), b = __ldg(gy + c), e = __ldg(gz + c);
+    db[c] = make_float2(sx * a.y + sy * b.y + sz * e.y, -(sx * a.x + sy * b.x + sz * e.x));
+}
+
+// ------------------------------------------------------------------------------------------- gather helpers ----
+__device__ __forceinline__ float gather8(const float* __restrict__ m, const Cic& c, int N, const float (&wx)[2],
+                                         const float (&wy)[2], const float (&wz)[2]) {
+    float acc = 0.f;
+#pragma unroll
+    for (int cz = 0; cz < 2; ++cz) {
+        const int64_t bz = (int64_t)(cz ? c.i1[2] : c.i0[2]) * N;
+#pragma unroll
+        for (int cy = 0; cy < 2; ++cy) {
+            const int64_t row = (bz + (cy ? c.i1[1] : c.i0[1])) * N;
+            const float wzy = wz[cz] * wy[cy];
+            acc = fmaf(wzy * wx[0], __ldg(m + row + c.i0[0]), acc);
+            acc = fmaf(wzy * wx[1], __ldg(m + row + c.i1[0]), acc);
+        }
+    }
+    return acc;
+}
+
+// ---------------------------------------------------------------------------------------------- kick + drift ----
+__device__ __forceinline__ float wrap_pos(float x, float fN) {
+    x -= fN * floorf(x / fN);
+    return x >= fN ? x - fN : x;
+}
+
+__global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
+                                                         const float* __restrict__ gz, float* __restrict__ px,
+                                                         float* __restrict__ py, float* __restrict__ pz,
+                                                         float* __restrict__ wx_, float* __restrict__ wy_,
+                                                         float* __restrict__ wz_, int64_t np, int N, float K,
+                                                         float dtau_dx, int gravity) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    float x = px[p], y = py[p], z = pz[p];
+    float ux = wx_[p], uy = wy_[p], uz = wz_[p];
+    if (gravity) {
+        const Cic c = cic_of(x, y, z, N);
+        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
+        ux = fmaf(K, gather8(gx, c, N, wx, wy, wz), ux);
+        uy = fmaf(K, gather8(gy, c, N, wx, wy, wz), uy);
+        uz = fmaf(K, gather8(gz, c, N, wx, wy, wz), uz);
+    }
+    const float fN = (float)N;
+    px[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN);
+    py[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN);
+    pz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN);
+    wx_[p] = ux; wy_[p] = uy; wz_[p] = uz;
+}
+
+__device__ __forceinline__ void block_sum2_to_global(float a, float b, double* outa, double* outb, float* sm /*64*/) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+    }
+    const int t = threadIdx.x, w = t >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((t & 31) == 0) { sm[w] = a; sm[32 + w] = b; }
+    __syncthreads();
+    if (t < 32) {
+        double da = t < nw ? (double)sm[t] : 0.0, db = t < nw ? (double)sm[32 + t] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            da += __shfl_xor_sync(0xffffffffu, da, o);
+            db += __shfl_xor_sync(0xffffffffu, db, o);
+        }
+        if (t == 0) { atomicAdd(outa, da); if (outb) atomicAdd(outb, db); }
+    }
+}
+
+// Adjoint of kick + drift + gather.  Forward: w' = w + K g_p(x); x' = wrap(x + w' dtau/dx).
+//   wt_b = w'_b + (dtau/dx) x'_b;  w_b = wt_b;  x_b = x'_b + K sum_d wt_b,d d g_p,d / dx;
+//   g'_b(cell) += W K wt_b (vector deposit);  K_b += wt_b . g_p;  (dtau/dx)_b += x'_b . w'
+__global__ void __launch_bounds__(256) kick_drift_adj_kernel(
+    const float* __restrict__ gx, const float* __restrict__ gy, const float* __restrict__ gz,
+    const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
+    const float* __restrict__ wx_, const float* __restrict__ wy_, const float* __restrict__ wz_,
+    const float* __restrict__ xbo, const float* __restrict__ ybo, const float* __restrict__ zbo,
+    const float* __restrict__ wxbo, const float* __restrict__ wybo, const float* __restrict__ wzbo,
+    float* __restrict__ xbi, float* __restrict__ ybi, float* __restrict__ zbi,
+    float* __restrict__ wxbi, float* __restrict__ wybi, float* __restrict__ wzbi,
+    float* __restrict__ gbx, float* __restrict__ gby, float* __restrict__ gbz,
+    int64_t np, int N, float K, float dtau_dx, int gravity, double* K_b, double* dtdx_b) {
+    __shared__ float sm[64];
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float kacc = 0.f, dacc = 0.f;
+    if (p < np) {
+        const float x = px[p], y = py[p], z = pz[p];
+        const float xb[3] = {xbo[p], ybo[p], zbo[p]};
+        float wt[3] = {fmaf(dtau_dx, xb[0], wxbo[p]), fmaf(dtau_dx, xb[1], wybo[p]), fmaf(dtau_dx, xb[2], wzbo[p])};
+        float gp[3] = {0.f, 0.f, 0.f};
+        float xo[3] = {xb[0], xb[1], xb[2]};
+        if (gravity) {
+            const Cic c = cic_of(x, y, z, N);
+            const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
+            const float dm[2] = {-1.f, 1.f};
+            const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
+#pragma unroll
+            for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+                for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+                    for (int cx = 0; cx < 2; ++cx) {
+                        const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
+                                             (cx ? c.i1[0] : c.i0[0]);
+                        const float g0 = __ldg(gx + cell), g1 = __ldg(gy + cell), g2 = __ldg(gz + cell);
+                        const float w = wz[cz] * wy[cy] * wx[cx];
+                        gp[0] = fmaf(w, g0, gp[0]); gp[1] = fmaf(w, g1, gp[1]); gp[2] = fmaf(w, g2, gp[2]);
+                        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
+                        const float s = kw[0] * g0 + kw[1] * g1 + kw[2] * g2;
+                        xo[0] = fmaf(dm[cx] * wy[cy] * wz[cz], s, xo[0]);
+                        xo[1] = fmaf(wx[cx] * dm[cy] * wz[cz], s, xo[1]);
+                        xo[2] = fmaf(wx[cx] * wy[cy] * dm[cz], s, xo[2]);
+                        atomicAdd(gbx + cell, w * kw[0]);
+                        atomicAdd(gby + cell, w * kw[1]);
+                        atomicAdd(gbz + cell, w * kw[2]);
+                    }
+        }
+        const float wn[3] = {fmaf(K, gp[0], wx_[p]), fmaf(K, gp[1], wy_[p]), fmaf(K, gp[2], wz_[p])};
+        kacc = wt[0] * gp[0] + wt[1] * gp[1] + wt[2] * gp[2];
+        dacc = xb[0] * wn[0] + xb[1] * wn[1] + xb[2] * wn[2];
+        xbi[p] = xo[0]; ybi[p] = xo[1]; zbi[p] = xo[2];
+        wxbi[p] = wt[0]; wybi[p] = wt[1]; wzbi[p] = wt[2];
+    }
+    block_sum2_to_global(kacc, dacc, K_b, dtdx_b, sm);
+}
+
+// Adjoint of the deposit: x_b += m_p sum_cells delta_b(cell) dW/dx_p
+__global__ void __launch_bounds__(256) deposit_adj_kernel(const float* __restrict__ db, const float* __restrict__ px,
+                                                          const float* __restrict__ py, const float* __restrict__ pz,
+                                                          float* __restrict__ xb, float* __restrict__ yb,
+                                                          float* __restrict__ zb, int64_t np, int N, float mp) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    const Cic c = cic_of(px[p], py[p], pz[p], N);
+    const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
+    const float dm[2] = {-1.f, 1.f};
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+#pragma unroll
+    for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+        for (int cy = 0; cy < 2; ++cy)
+#pragma unroll
+            for (int cx = 0; cx < 2; ++cx) {
+                const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
+                                     (cx ? c.i1[0] : c.i0[0]);
+                const float v = __ldg(db + cell);
+                a0 = fmaf(dm[cx] * wy[cy] * wz[cz], v, a0);
+                a1 = fmaf(wx[cx] * dm[cy] * wz[cz], v, a1);
+                a2 = fmaf(wx[cx] * wy[cy] * dm[cz], v, a2);
+            }
+    xb[p] = fmaf(mp, a0, xb[p]);
+    yb[p] = fmaf(mp, a1, yb[p]);
+    zb[p] = fmaf(mp, a2, zb[p]);
+}
+
+// y += a * x  (float4)
+__global__ void axpy_kernel(const float4* __restrict__ x, float4* __restrict__ y, int64_t n4, float a) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; i < n4; i += stride) {
+        const float4 u = __ldg(x + i);
+        float4 v = y[i];
+        v.x = fmaf(a, u.x, v.x); v.y = fmaf(a, u.y, v.y); v.z = fmaf(a, u.z, v.z); v.w = fmaf(a, u.w, v.w);
+        y[i] = v;
+    }
+}
+
+// out += scale * sum_d <a_d, b_d>   (fp64 accumulation across blocks)
+__global__ void __launch_bounds__(256) dot3_kernel(const float4* __restrict__ a0, const float4* __restrict__ a1,
+                                                   const float4* __restrict__ a2, const float4* __restrict__ b0,
+                                                   const float4* __restrict__ b1, const float4* __restrict__ b2,
+                                                   int64_t n4, double scale, double* out) {
+    __shared__ float sm[64];
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (; i < n4; i += stride) {
+        float s = 0.f;
+        float4 u = __ldg(a0 + i), v = __ldg(b0 + i);
+        s = fmaf(u.x, v.x, s); s = fmaf(u.y, v.y, s); s = fmaf(u.z, v.z, s); s = fmaf(u.w, v.w, s);
+        u = __ldg(a1 + i); v = __ldg(b1 + i);
+        s = fmaf(u.x, v.x, s); s = fmaf(u.y, v.y, s); s = fmaf(u.z, v.z, s); s = fmaf(u.w, v.w, s);
+        u = __ldg(a2 + i); v = __ldg(b2 + i);
+        s = fmaf(u.x, v.x, s); s = fmaf(u.y, v.y, s); s = fmaf(u.z, v.z, s); s = fmaf(u.w, v.w, s);
+        acc += (double)s;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    double* smd = reinterpret_cast<double*>(sm);
+    const int t = threadIdx.x;
+    if ((t & 31) == 0) smd[t >> 5] = acc;
+    __syncthreads();
+    if (t < 32) {
+        double v = t < (int)(blockDim.x >> 5) ? smd[t] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (t == 0) atomicAdd(out, scale * v);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ launchers ----
+static inline unsigned grid_for(int64_t n, int block, int sm_count, int per_sm) {
+    int64_t g = (n + block - 1) / block;
+    int64_t cap = (int64_t)sm_count * per_sm;
+    return (unsigned)(g < cap ? (g > 0 ? g : 1) : cap);
+}
+
+int launch_fill(dh_ctx* c, float* p, int64_t n, float v) {
+    fill_kernel<<<grid_for(n, 256, c->sm_count, 8), 256, 0, c->stream>>>(p, n, v);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t* i1) {
+    if (n <= 0) return DH_OK;
+    cell_index_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, n, c->N, i0, i1);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta) {
+    const float flag = (c->opt.gas_sources_gravity && rho_gas) ? 1.f : 0.f;
+    const int64_t n4 = c->n3 / 4;
+    source_init_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
+        reinterpret_cast<const float4*>(flag != 0.f ? rho_gas : nullptr), reinterpret_cast<float4*>(delta), n4, flag,
+        (float)c->rho_bar);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    if (c->np > 0) {
+        constexpr int PX = 32, PY = 8, PZ = 8, M = 2;   // 2048 particles per block, 36x12x12 mesh brick (20 KB)
+        const int nps = c->nps;
+        const int nbx = (nps + PX - 1) / PX, nby = (nps + PY - 1) / PY, nbz = (nps + PZ - 1) / PZ;
+        deposit_brick_kernel<PX, PY, PZ, M><<<(unsigned)((int64_t)nbx * nby * nbz), 256, 0, c->stream>>>(
+            x, y, z, nps, c->N, (float)c->m_p, (float)c->N / (float)nps, delta);
+        c->launches++;
+        DH_CUDA(cudaGetLastError());
+    }
+    return DH_OK;
+}
+
+static float green_coef(const dh_ctx* c, float A) {
+    // i k_d A / k^2 with k = (2 pi / L) n  ->  i n_d (A L / 2 pi) / n^2 ; the 1/N^3 normalises the unnormalised cuFFT pair
+    return (float)((double)A * c->box / (2.0 * M_PI) / (double)c->n3);
+}
+
+int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]) {
+    const int64_t nspec = (int64_t)c->N * c->N * (c->N / 2 + 1);
+    green_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, c->stream>>>(dhat, ghat[0], ghat[1], ghat[2], c->N, nspec,
+                                                                          green_coef(c, A));
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat) {
+    const int64_t nspec = (int64_t)c->N * c->N * (c->N / 2 + 1);
+    green_adj_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, c->stream>>>(gbhat[0], gbhat[1], gbhat[2], dbhat, c->N,
+                                                                              nspec, green_coef(c, A));
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]) {
+    DH_CUFFT(cufftExecR2C(c->plan_r2c, const_cast<float*>(delta), reinterpret_cast<cufftComplex*>(c->spec[0])));
+    float2* gh[3] = {c->spec[1], c->spec[2], c->spec[3]};
+    DH_TRY(launch_green(c, c->spec[0], A, gh));
+    for (int d = 0; d < 3; ++d)
+        DH_CUFFT(cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(gh[d]), g_out[d]));
+    return DH_OK;
+}
+
+int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar) {
+    float2* gh[3] = {c->spec[1], c->spec[2], c->spec[3]};
+    for (int d = 0; d < 3; ++d)
+        DH_CUFFT(cufftExecR2C(c->plan_r2c, g_bar[d], reinterpret_cast<cufftComplex*>(gh[d])));
+    DH_TRY(launch_green_adj(c, gh, A, c->spec[0]));
+    DH_CUFFT(cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->spec[0]), delta_bar));
+    return DH_OK;
+}
+
+int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float K, float dtau_dx) {
+    if (c->np <= 0) return DH_OK;
+    const int grav = c->opt.gravity_on && g && g[0];
+    kick_drift_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+        grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
+        part[5], c->np, c->N, K, dtau_dx, grav);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6], float* const cot_out[6],
+                          float* const cot_in[6], float* const gbar[3], float K, float dtau_dx, double* scal_bar) {
+    if (c->np <= 0) return DH_OK;
+    const int grav = c->opt.gravity_on && g && g[0];
+    kick_drift_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+        grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part_in[0], part_in[1], part_in[2],
+        part_in[3], part_in[4], part_in[5], cot_out[0], cot_out[1], cot_out[2], cot_out[3], cot_out[4], cot_out[5],
+        cot_in[0], cot_in[1], cot_in[2], cot_in[3], cot_in[4], cot_in[5], grav ? gbar[0] : nullptr,
+        grav ? gbar[1] : nullptr, grav ? gbar[2] : nullptr, c->np, c->N, K, dtau_dx, grav, scal_bar + 3, scal_bar + 4);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6], float* rho_bar_gas,
+                       float* const xbar[3]) {
+    if (c->opt.gas_sources_gravity && rho_bar_gas) {
+        const int64_t n4 = c->n3 / 4;
+        axpy_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
+            reinterpret_cast<const float4*>(delta_bar), reinterpret_cast<float4*>(rho_bar_gas), n4, 1.f);
+        c->launches++;
+        DH_CUDA(cudaGetLastError());
+    }
+    if (c->np > 0) {
+        deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+            delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], c->np, c->N, (float)c->m_p);
+        c->launches++;
+        DH_CUDA(cudaGetLastError());
+    }
+    return DH_OK;
+}
+
+int launch_dot3(dh_ctx* c, float* const a[3], float* const b[3], double scale, double* out) {
+    const int64_t n4 = c->n3 / 4;
+    dot3_kernel<<<grid_for(n4, 256, c->sm_count, 4), 256, 0, c->stream>>>(
+        reinterpret_cast<const float4*>(a[0]), reinterpret_cast<const float4*>(a[1]), reinterpret_cast<const float4*>(a[2]),
+        reinterpret_cast<const float4*>(b[0]), reinterpret_cast<const float4*>(b[1]), reinterpret_cast<const float4*>(b[2]),
+        n4, scale, out);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+}  // namespace dh

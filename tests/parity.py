@@ -1,0 +1,39 @@
+"""Error norms of the parity protocol (reading R25 in DESIGN.md) and small helpers shared by the GPU tests."""
+import numpy as np
+
+
+def field_err(got, ref):
+    """max |got - ref| / max |ref| per gas field; the three momentum components are normalised jointly."""
+    got = np.asarray(got, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
+    e = {}
+    e["rho"] = np.max(np.abs(got[0] - ref[0])) / np.max(np.abs(ref[0]))
+    mscale = max(np.max(np.abs(ref[1:4])), 1e-300)
+    e["mom"] = np.max(np.abs(got[1:4] - ref[1:4])) / mscale
+    e["eps"] = np.max(np.abs(got[4] - ref[4])) / np.max(np.abs(ref[4]))
+    return e
+
+
+def part_err(got, ref, N):
+    got = np.asarray(got, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
+    d = got[:3] - ref[:3]
+    d -= N * np.round(d / N)
+    e = {"x": np.max(np.abs(d)) / N if d.size else 0.0}
+    e["w"] = (np.max(np.abs(got[3:] - ref[3:])) / max(np.max(np.abs(ref[3:])), 1e-300)) if d.size else 0.0
+    return e
+
+
+def rel_l2(got, ref):
+    got = np.asarray(got, dtype=np.float64).ravel(); ref = np.asarray(ref, dtype=np.float64).ravel()
+    return np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)
+
+
+def max_rel(got, ref):
+    got = np.asarray(got, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
+    return np.max(np.abs(got - ref)) / max(np.max(np.abs(ref)), 1e-300)
+
+
+def oracle_params(O, cfg, **kw):
+    args = dict(n_part_side=cfg.n_side, H0=cfg.H0, Omega_m=cfg.Omega_m, Omega_b=cfg.Omega_b, Omega_L=cfg.Omega_L,
+                static_mode=cfg.static_mode, gravity_on=cfg.gravity_on, e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+    args.update(kw)
+    return O.make_params(cfg.N, cfg.box, cfg.gamma, **args)
