@@ -122,6 +122,10 @@ int dh_run(dh_ctx* ctx, dh_state* state, const double* a_sched, const double* dt
  * alias cot_final); dparams accumulated.  Synchronises. */
 int dh_run_vjp(dh_ctx* ctx, const dh_cot* cot_final, dh_cot* cot_initial, dh_dparams* dparams);
 
+/* Optional: allocate now everything a dh_run(n_steps, checkpoint_stride) + dh_run_vjp pair will need (snapshot pool,
+ * in-segment states, adjoint scratch, CFL log), so that neither call allocates.  Errors: DH_ERR_OOM. */
+int dh_reserve(dh_ctx* ctx, int n_steps, int checkpoint_stride);
+
 /* ---- host-buffer variants (end-to-end path: host <-> device copies inside the call) ------------------------- */
 
 /* gas_host: 5 N^3 floats, part_host: 6 N_p floats (HOST, pinned or pageable), updated in place with the final state.
@@ -149,6 +153,14 @@ int64_t dh_device_bytes(dh_ctx* ctx);
  * cuFFT's internal kernels are not counted. */
 int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
+/* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of
+ * CUDA events on the context's stream.  dh_profile_read synchronises, adds the elapsed milliseconds and launch counts
+ * per category into ms_out / count_out (HOST arrays of dh_profile_categories() entries, overwritten) and clears the
+ * record.  dh_profile_name(i): static string, NULL when i is out of range. */
+int dh_profile_enable(dh_ctx* ctx, int on);
+int dh_profile_categories(void);
+const char* dh_profile_name(int i);
+int dh_profile_read(dh_ctx* ctx, double* ms_out, int64_t* count_out);
 
 /* ---- single kernels of the path (same kernels dh_step / dh_step_vjp launch; for parity tests and profiling) --
  * All pointers DEVICE.  d = sweep axis 0/1/2 = x/y/z.  lam = Dtau/dx, kap = kappa. */

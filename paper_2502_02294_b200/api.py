@@ -27,7 +27,8 @@ ERRORS = {-1: "DH_ERR_INVALID", -2: "DH_ERR_NO_DEVICE", -3: "DH_ERR_CUDA", -4: "
 EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp", "dh_run_host", "dh_run_vjp_host",
            "dh_last_error", "dh_get_cmax", "dh_schedule_lna", "dh_step_scalars", "dh_debug_cell_index",
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
-           "dh_poisson_vjp", "dh_kick_drift"]
+           "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
+           "dh_profile_read", "dh_reserve"]
 
 
 class DhError(RuntimeError):
@@ -68,6 +69,10 @@ class dh_dparams(C.Structure):
 _lib.dh_last_error.restype = C.c_char_p
 _lib.dh_device_bytes.restype = C.c_int64
 _lib.dh_launch_count.restype = C.c_int64
+_lib.dh_profile_name.restype = C.c_char_p
+_lib.dh_profile_name.argtypes = [C.c_int]
+_lib.dh_profile_enable.argtypes = [C.c_void_p, C.c_int]
+_lib.dh_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
 _lib.dh_device_bytes.argtypes = [C.c_void_p]
 _lib.dh_launch_count.argtypes = [C.c_void_p]
 _dp = C.POINTER(C.c_double)
@@ -83,6 +88,7 @@ _lib.dh_run_vjp.argtypes = [C.c_void_p, C.POINTER(dh_cot), C.POINTER(dh_cot), C.
 _lib.dh_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, _dp, _dp, C.POINTER(C.c_int64), _dp, _dp, C.c_int,
                              C.c_int]
 _lib.dh_run_vjp_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(dh_dparams)]
+_lib.dh_reserve.argtypes = [C.c_void_p, C.c_int, C.c_int]
 _lib.dh_get_cmax.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
 _lib.dh_schedule_lna.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_int, _dp, _dp]
 _lib.dh_step_scalars.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_double, C.c_double, _dp]
@@ -201,6 +207,9 @@ class Context:
         st.a, st.dt_prev, st.step = cs.a, cs.dt_prev, cs.step
         _check(rc, "dh_run")
 
+    def dh_reserve(self, n_steps, checkpoint_stride):
+        _check(_lib.dh_reserve(self._h, int(n_steps), int(checkpoint_stride)), "dh_reserve")
+
     def dh_run_vjp(self, cot_final: Cot, cot_initial: Cot, dparams: dh_dparams | None = None):
         dparams = dparams if dparams is not None else dh_dparams()
         cf, ci = cot_final.c_struct(), cot_initial.c_struct()
@@ -239,6 +248,17 @@ class Context:
 
     def dh_launch_count(self):
         return int(_lib.dh_launch_count(self._h))
+
+    def dh_profile_enable(self, on=True):
+        _check(_lib.dh_profile_enable(self._h, int(bool(on))), "dh_profile_enable")
+
+    def dh_profile_read(self):
+        """{category: (milliseconds, launches)} since the last read (CUDA events around every launch)."""
+        n = _lib.dh_profile_categories()
+        ms = (C.c_double * n)()
+        cnt = (C.c_int64 * n)()
+        _check(_lib.dh_profile_read(self._h, ms, cnt), "dh_profile_read")
+        return {_lib.dh_profile_name(i).decode(): (ms[i], cnt[i]) for i in range(n) if cnt[i]}
 
     def dh_debug_cell_index(self, x: torch.Tensor):
         x = x.contiguous()

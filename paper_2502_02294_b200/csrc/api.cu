@@ -75,6 +75,7 @@ static size_t state_floats(const dh_ctx* c) { return (size_t)(5 * c->n3 + 6 * c-
 
 static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st) {
     if (!s.buf) DH_TRY(dev_alloc(c, (void**)&s.buf, state_floats(c) * sizeof(float)));
+    Prof prof(c, PROF_COPY);
     for (int k = 0; k < 5; ++k)
         DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)k * c->n3, st->gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     for (int k = 0; k < 6 && c->np > 0; ++k)
@@ -301,6 +302,7 @@ int dh_free(dh_ctx* c) {
     cudaFree(c->hv_state); cudaFree(c->hv_cot);
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
+    for (auto e : c->prof_ev) cudaEventDestroy(e);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     cudaGetLastError();
     delete c;
@@ -310,6 +312,34 @@ int dh_free(dh_ctx* c) {
 int dh_sync(dh_ctx* c) {
     if (!c) return DH_ERR_INVALID;
     DH_CUDA(cudaStreamSynchronize(c->stream));
+    return DH_OK;
+}
+
+static const char* const PROF_NAMES[PROF_N] = {
+    "source_init", "deposit", "fft_r2c", "green", "fft_c2r", "kick_drift", "sweep_x", "sweep_y", "sweep_z",
+    "sweep_x_adj", "sweep_y_adj", "sweep_z_adj", "kick_drift_adj", "green_adj", "deposit_adj", "axpy", "dot3", "fill",
+    "copy"};
+
+int dh_profile_enable(dh_ctx* c, int on) {
+    if (!c) return DH_ERR_INVALID;
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    c->prof_on = on != 0;
+    c->prof_used = 0;
+    return DH_OK;
+}
+int dh_profile_categories(void) { return PROF_N; }
+const char* dh_profile_name(int i) { return (i >= 0 && i < PROF_N) ? PROF_NAMES[i] : nullptr; }
+int dh_profile_read(dh_ctx* c, double* ms_out, int64_t* count_out) {
+    if (!c || !ms_out || !count_out) { set_error("dh_profile_read: null argument"); return DH_ERR_INVALID; }
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < PROF_N; ++i) { ms_out[i] = 0.0; count_out[i] = 0; }
+    for (size_t s = 0; s < c->prof_used; ++s) {
+        float ms = 0.f;
+        DH_CUDA(cudaEventElapsedTime(&ms, c->prof_ev[2 * s], c->prof_ev[2 * s + 1]));
+        ms_out[c->prof_cat[s]] += ms;
+        count_out[c->prof_cat[s]] += 1;
+    }
+    c->prof_used = 0;
     return DH_OK;
 }
 
@@ -386,10 +416,7 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     c->cmax_n = n_steps;
     c->run_valid = false;
     const int nseg = stride > 0 ? (n_steps + stride - 1) / stride : 0;
-    if ((int)c->snaps.size() > nseg) {
-        for (size_t i = nseg; i < c->snaps.size(); ++i) dev_free(c, c->snaps[i].buf, state_floats(c) * sizeof(float));
-    }
-    c->snaps.resize(nseg);
+    if ((int)c->snaps.size() < nseg) c->snaps.resize(nseg);     // the pool only grows (dh_free releases it)
     c->run_a.assign(a_sched, a_sched + n_steps);
     c->run_dt.assign(dt_sched, dt_sched + n_steps);
     c->run_n = n_steps; c->run_stride = stride;
@@ -413,6 +440,29 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
             }
     }
     c->run_valid = stride > 0;
+    return DH_OK;
+}
+
+int dh_reserve(dh_ctx* c, int n_steps, int stride) {
+    if (!c || n_steps < 0) { set_error("dh_reserve: bad argument"); return DH_ERR_INVALID; }
+    if (n_steps > c->cmax_cap) {
+        dev_free(c, c->cmax_log, (size_t)3 * c->cmax_cap * sizeof(float));
+        c->cmax_log = nullptr; c->cmax_cap = 0;
+        DH_TRY(dev_alloc(c, (void**)&c->cmax_log, (size_t)3 * n_steps * sizeof(float)));
+        c->cmax_cap = n_steps;
+    }
+    if (stride <= 0) return DH_OK;
+    const size_t bytes = state_floats(c) * sizeof(float);
+    const int nseg = (n_steps + stride - 1) / stride;
+    if ((int)c->snaps.size() < nseg) c->snaps.resize(nseg);
+    for (int i = 0; i < nseg; ++i)
+        if (!c->snaps[i].buf) DH_TRY(dev_alloc(c, (void**)&c->snaps[i].buf, bytes));
+    const int in_seg = stride < n_steps ? stride : n_steps;
+    if ((int)c->seg.size() < in_seg) c->seg.resize(in_seg);
+    for (int i = 1; i < in_seg; ++i)
+        if (!c->seg[i].buf) DH_TRY(dev_alloc(c, (void**)&c->seg[i].buf, bytes));
+    DH_TRY(ensure_adjoint_scratch(c));
+    c->run_valid = false;
     return DH_OK;
 }
 

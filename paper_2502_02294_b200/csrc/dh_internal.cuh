@@ -42,6 +42,13 @@ static const int STRANG[6][3] = {{0, 1, 2}, {2, 1, 0}, {2, 0, 1}, {1, 0, 2}, {1,
 
 struct StepScalars { double dtau, kappa, K, A; };
 
+// Per-kernel timing categories of dh_profile_* (names in api.cu, same order).
+enum ProfCat {
+    PROF_SOURCE_INIT = 0, PROF_DEPOSIT, PROF_FFT_R2C, PROF_GREEN, PROF_FFT_C2R, PROF_KICK_DRIFT,
+    PROF_SWEEP_X, PROF_SWEEP_Y, PROF_SWEEP_Z, PROF_SWEEP_X_ADJ, PROF_SWEEP_Y_ADJ, PROF_SWEEP_Z_ADJ,
+    PROF_KICK_DRIFT_ADJ, PROF_GREEN_ADJ, PROF_DEPOSIT_ADJ, PROF_AXPY, PROF_DOT3, PROF_FILL, PROF_COPY, PROF_N
+};
+
 struct Snapshot {
     float* buf = nullptr;   // 5 N^3 + 6 N_p floats
     double a = 0, dt_prev = 0;
@@ -97,12 +104,37 @@ struct dh_ctx {
     int64_t run_step0 = 0;
     bool run_valid = false;
 
+    // optional per-kernel CUDA-event timing (dh_profile_enable): pairs of events around every launch
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev;    // 2 per recorded launch
+    std::vector<int> prof_cat;
+    size_t prof_used = 0;                // launches recorded since the last read
+
     // host-variant device buffers
     float* hv_state = nullptr;     // 5 N^3 + 6 N_p
     float* hv_cot = nullptr;
 };
 
 namespace dh {
+
+// RAII timing scope: records an event pair on the context's stream around whatever is launched inside it.
+struct Prof {
+    dh_ctx* c; size_t slot; bool on;
+    Prof(dh_ctx* ctx, int cat) : c(ctx), slot(0), on(ctx->prof_on) {
+        if (!on) return;
+        slot = c->prof_used;
+        if (c->prof_ev.size() < 2 * (slot + 1)) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { on = false; return; }
+            c->prof_ev.push_back(a); c->prof_ev.push_back(b);
+            c->prof_cat.push_back(cat);
+        }
+        c->prof_cat[slot] = cat;
+        c->prof_used = slot + 1;
+        cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+    }
+    ~Prof() { if (on) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
+};
 
 int dev_alloc(dh_ctx* c, void** p, size_t bytes);
 void dev_free(dh_ctx* c, void* p, size_t bytes);

@@ -377,6 +377,7 @@ static inline unsigned grid_for(int64_t n, int block, int sm_count, int per_sm) 
 }
 
 int launch_fill(dh_ctx* c, float* p, int64_t n, float v) {
+    Prof prof(c, PROF_FILL);
     fill_kernel<<<grid_for(n, 256, c->sm_count, 8), 256, 0, c->stream>>>(p, n, v);
     c->launches++;
     DH_CUDA(cudaGetLastError());
@@ -394,12 +395,16 @@ int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t
 int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta) {
     const float flag = (c->opt.gas_sources_gravity && rho_gas) ? 1.f : 0.f;
     const int64_t n4 = c->n3 / 4;
-    source_init_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
-        reinterpret_cast<const float4*>(flag != 0.f ? rho_gas : nullptr), reinterpret_cast<float4*>(delta), n4, flag,
-        (float)c->rho_bar);
+    {
+        Prof prof(c, PROF_SOURCE_INIT);
+        source_init_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
+            reinterpret_cast<const float4*>(flag != 0.f ? rho_gas : nullptr), reinterpret_cast<float4*>(delta), n4, flag,
+            (float)c->rho_bar);
+    }
     c->launches++;
     DH_CUDA(cudaGetLastError());
     if (c->np > 0) {
+        Prof prof(c, PROF_DEPOSIT);
         constexpr int PX = 32, PY = 8, PZ = 8, M = 2;   // 2048 particles per block, 36x12x12 mesh brick (20 KB)
         const int nps = c->nps;
         const int nbx = (nps + PX - 1) / PX, nby = (nps + PY - 1) / PY, nbz = (nps + PZ - 1) / PZ;
@@ -418,6 +423,7 @@ static float green_coef(const dh_ctx* c, float A) {
 
 int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]) {
     const int64_t nspec = (int64_t)c->N * c->N * (c->N / 2 + 1);
+    Prof prof(c, PROF_GREEN);
     green_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, c->stream>>>(dhat, ghat[0], ghat[1], ghat[2], c->N, nspec,
                                                                           green_coef(c, A));
     c->launches++;
@@ -427,6 +433,7 @@ int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]) 
 
 int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat) {
     const int64_t nspec = (int64_t)c->N * c->N * (c->N / 2 + 1);
+    Prof prof(c, PROF_GREEN_ADJ);
     green_adj_kernel<<<(unsigned)((nspec + 255) / 256), 256, 0, c->stream>>>(gbhat[0], gbhat[1], gbhat[2], dbhat, c->N,
                                                                               nspec, green_coef(c, A));
     c->launches++;
@@ -435,26 +442,37 @@ int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat) 
 }
 
 int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]) {
-    DH_CUFFT(cufftExecR2C(c->plan_r2c, const_cast<float*>(delta), reinterpret_cast<cufftComplex*>(c->spec[0])));
+    {
+        Prof prof(c, PROF_FFT_R2C);
+        DH_CUFFT(cufftExecR2C(c->plan_r2c, const_cast<float*>(delta), reinterpret_cast<cufftComplex*>(c->spec[0])));
+    }
     float2* gh[3] = {c->spec[1], c->spec[2], c->spec[3]};
     DH_TRY(launch_green(c, c->spec[0], A, gh));
-    for (int d = 0; d < 3; ++d)
+    for (int d = 0; d < 3; ++d) {
+        Prof prof(c, PROF_FFT_C2R);
         DH_CUFFT(cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(gh[d]), g_out[d]));
+    }
     return DH_OK;
 }
 
 int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar) {
     float2* gh[3] = {c->spec[1], c->spec[2], c->spec[3]};
-    for (int d = 0; d < 3; ++d)
+    for (int d = 0; d < 3; ++d) {
+        Prof prof(c, PROF_FFT_R2C);
         DH_CUFFT(cufftExecR2C(c->plan_r2c, g_bar[d], reinterpret_cast<cufftComplex*>(gh[d])));
+    }
     DH_TRY(launch_green_adj(c, gh, A, c->spec[0]));
-    DH_CUFFT(cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->spec[0]), delta_bar));
+    {
+        Prof prof(c, PROF_FFT_C2R);
+        DH_CUFFT(cufftExecC2R(c->plan_c2r, reinterpret_cast<cufftComplex*>(c->spec[0]), delta_bar));
+    }
     return DH_OK;
 }
 
 int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float K, float dtau_dx) {
     if (c->np <= 0) return DH_OK;
     const int grav = c->opt.gravity_on && g && g[0];
+    Prof prof(c, PROF_KICK_DRIFT);
     kick_drift_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
         grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
         part[5], c->np, c->N, K, dtau_dx, grav);
@@ -467,6 +485,7 @@ int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6],
                           float* const cot_in[6], float* const gbar[3], float K, float dtau_dx, double* scal_bar) {
     if (c->np <= 0) return DH_OK;
     const int grav = c->opt.gravity_on && g && g[0];
+    Prof prof(c, PROF_KICK_DRIFT_ADJ);
     kick_drift_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
         grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part_in[0], part_in[1], part_in[2],
         part_in[3], part_in[4], part_in[5], cot_out[0], cot_out[1], cot_out[2], cot_out[3], cot_out[4], cot_out[5],
@@ -481,12 +500,14 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
                        float* const xbar[3]) {
     if (c->opt.gas_sources_gravity && rho_bar_gas) {
         const int64_t n4 = c->n3 / 4;
+        Prof prof(c, PROF_AXPY);
         axpy_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
             reinterpret_cast<const float4*>(delta_bar), reinterpret_cast<float4*>(rho_bar_gas), n4, 1.f);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }
     if (c->np > 0) {
+        Prof prof(c, PROF_DEPOSIT_ADJ);
         deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
             delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], c->np, c->N, (float)c->m_p);
         c->launches++;
@@ -497,6 +518,7 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
 
 int launch_dot3(dh_ctx* c, float* const a[3], float* const b[3], double scale, double* out) {
     const int64_t n4 = c->n3 / 4;
+    Prof prof(c, PROF_DOT3);
     dot3_kernel<<<grid_for(n4, 256, c->sm_count, 4), 256, 0, c->stream>>>(
         reinterpret_cast<const float4*>(a[0]), reinterpret_cast<const float4*>(a[1]), reinterpret_cast<const float4*>(a[2]),
         reinterpret_cast<const float4*>(b[0]), reinterpret_cast<const float4*>(b[1]), reinterpret_cast<const float4*>(b[2]),

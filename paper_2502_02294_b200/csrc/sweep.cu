@@ -729,6 +729,7 @@ static int yz_chain_threads(int N, int K, int halo, int max_c) {
 int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
                  float* cmax) {
     const int N = c->N;
+    Prof prof(c, PROF_SWEEP_X + d);
     SweepConst sc = make_const(c, lam, kap);
     Ptr5 pin; MPtr5 pout;
     const float* tmp[5];
@@ -763,6 +764,7 @@ int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam
 int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap,
                      float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar) {
     const int N = c->N;
+    Prof prof(c, PROF_SWEEP_X_ADJ + d);
     SweepConst sc = make_const(c, lam, kap);
     Ptr5 pin, pco; MPtr5 pci;
     const float* tmp[5];

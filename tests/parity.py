@@ -27,6 +27,18 @@ def rel_l2(got, ref):
     return np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)
 
 
+def rel_l2_trimmed(got, ref, frac=2e-4):
+    """rel_l2 after dropping the `frac` largest-error entries.  The limiter gate (ab > 0), the energy floor and |v| make
+    the step's derivative piecewise: a difference whose sign is decided at fp32 rounding level switches a few O(1)
+    entries of the VJP (the fp64 oracle shows the same jumps when its input is perturbed by 1e-7).  Those entries are
+    compared through the untrimmed north-star bound (<= 1e-3); everything else must agree tightly."""
+    got = np.asarray(got, dtype=np.float64).ravel(); ref = np.asarray(ref, dtype=np.float64).ravel()
+    err = np.abs(got - ref)
+    k = int(np.ceil(frac * err.size))
+    keep = np.argsort(err)[: err.size - k]
+    return np.linalg.norm(err[keep]) / max(np.linalg.norm(ref), 1e-300)
+
+
 def max_rel(got, ref):
     got = np.asarray(got, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
     return np.max(np.abs(got - ref)) / max(np.max(np.abs(ref)), 1e-300)
