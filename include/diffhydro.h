@@ -153,6 +153,11 @@ int64_t dh_device_bytes(dh_ctx* ctx);
  * cuFFT's internal kernels are not counted. */
 int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
+/* Launch-geometry knobs (performance only; results stay within the parity tolerances).  key (HOST string):
+ *   "march_s_fwd", "march_s_adj": cells per thread segment of the marching y/z sweeps (0 = built-in choice);
+ *   "yz_chain": 1 routes the y/z sweeps through the shared-memory chain kernels the x sweep uses.
+ * Unknown key: DH_ERR_INVALID. */
+int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of
  * CUDA events on the context's stream.  dh_profile_read synchronises, adds the elapsed milliseconds and launch counts
  * per category into ms_out / count_out (HOST arrays of dh_profile_categories() entries, overwritten) and clears the

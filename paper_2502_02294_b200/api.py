@@ -28,7 +28,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_last_error", "dh_get_cmax", "dh_schedule_lna", "dh_step_scalars", "dh_debug_cell_index",
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
-           "dh_profile_read", "dh_reserve"]
+           "dh_profile_read", "dh_reserve", "dh_tune"]
 
 
 class DhError(RuntimeError):
@@ -89,6 +89,7 @@ _lib.dh_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, _dp, _dp, C.POI
                              C.c_int]
 _lib.dh_run_vjp_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(dh_dparams)]
 _lib.dh_reserve.argtypes = [C.c_void_p, C.c_int, C.c_int]
+_lib.dh_tune.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
 _lib.dh_get_cmax.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
 _lib.dh_schedule_lna.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_int, _dp, _dp]
 _lib.dh_step_scalars.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_double, C.c_double, _dp]
@@ -242,6 +243,9 @@ class Context:
 
     def dh_sync(self):
         _check(_lib.dh_sync(self._h), "dh_sync")
+
+    def dh_tune(self, key: str, value: int):
+        _check(_lib.dh_tune(self._h, key.encode(), int(value)), "dh_tune")
 
     def dh_device_bytes(self):
         return int(_lib.dh_device_bytes(self._h))

@@ -343,6 +343,15 @@ int dh_profile_read(dh_ctx* c, double* ms_out, int64_t* count_out) {
     return DH_OK;
 }
 
+int dh_tune(dh_ctx* c, const char* key, int value) {
+    if (!c || !key) { set_error("dh_tune: null argument"); return DH_ERR_INVALID; }
+    if (!strcmp(key, "march_s_fwd")) c->tune_march_s_fwd = value;
+    else if (!strcmp(key, "march_s_adj")) c->tune_march_s_adj = value;
+    else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
+    else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
+    return DH_OK;
+}
+
 int64_t dh_device_bytes(dh_ctx* c) { return c ? c->bytes : 0; }
 int64_t dh_launch_count(dh_ctx* c) { return c ? c->launches : 0; }
 

@@ -70,6 +70,9 @@ struct dh_ctx {
     int sm_count = 148;
     int64_t launches = 0;
     int64_t bytes = 0;
+    // tuning knobs (dh_tune): 0 = built-in choice
+    int tune_march_s_fwd = 0, tune_march_s_adj = 0;   // segment length of the marching y/z sweeps
+    int tune_yz_chain = 0;                            // 1: y/z sweeps through the chain kernels of sweep.cu
 
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans = false;

@@ -1,0 +1,197 @@
+// sweep_common.cuh -- device functions shared by the sweep kernels (sweep.cu: x chain kernels; sweep_march.cu: y/z
+// marching kernels): the flux split P(u), its transpose, the limiter, block reductions.  Product code: shares nothing
+// with oracle/.
+#pragma once
+#include "dh_internal.cuh"
+
+namespace dh {
+
+struct SweepConst {
+    float lam, kap;
+    float gm1;       // gamma - 1
+    float ggm1;      // gamma (gamma - 1)
+    float gamma;
+    float e_floor;
+    float eps4;      // 4 * lim_eps
+    float inv_lam;   // 1 / lam (0 when lam == 0): the marching adjoint forms lam_b from u* - u
+    int N;
+};
+
+__device__ __forceinline__ float rcp_fast(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// (G, H, c) = P(u)
+__device__ __forceinline__ void prim_GH(const float (&u)[5], const SweepConst& sc, float (&G)[5], float (&H)[5], float& c) {
+    const float rinv = rcp_fast(u[0]);
+    const float v = u[1] * rinv;
+    const float ke = 0.5f * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) * rinv;
+    const float e = (u[4] - ke) * rinv;
+    const float ep = !(e <= sc.e_floor) ? e : sc.e_floor;   // NaN passes through to the CFL check
+    const float p = sc.gm1 * u[0] * ep;
+    const float cs = sqrt_fast(sc.ggm1 * ep);
+    c = fabsf(v) + cs;
+    float F[5];
+    F[0] = u[1];
+    F[1] = fmaf(u[1], v, p);
+    F[2] = u[2] * v;
+    F[3] = u[3] * v;
+    F[4] = (u[4] + p) * v;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        G[k] = fmaf(c, u[k], F[k]);
+        H[k] = fmaf(c, u[k], -F[k]);
+    }
+}
+
+// Transpose of P at u: given cotangents Gb, Hb returns the cotangent of u and adds to gamma_b.
+__device__ __forceinline__ void prim_GH_vjp(const float (&u)[5], const SweepConst& sc, const float (&Gb)[5],
+                                            const float (&Hb)[5], float (&ub)[5], float& gamma_b) {
+    const float rinv = rcp_fast(u[0]);
+    const float v = u[1] * rinv;
+    const float m2 = u[1] * u[1] + u[2] * u[2] + u[3] * u[3];
+    const float ke = 0.5f * m2 * rinv;
+    const float e = (u[4] - ke) * rinv;
+    const bool active = !(e <= sc.e_floor);
+    const float ep = active ? e : sc.e_floor;
+    const float p = sc.gm1 * u[0] * ep;
+    const float cs = sqrt_fast(sc.ggm1 * ep);
+    const float c = fabsf(v) + cs;
+    float cub[5], Fb[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) { cub[k] = Gb[k] + Hb[k]; Fb[k] = Gb[k] - Hb[k]; }
+    float cb = 0.f;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) { cb = fmaf(cub[k], u[k], cb); ub[k] = c * cub[k]; }
+    // F = (m_n, m_n v + p, m_t1 v, m_t2 v, (eps + p) v)
+    float mnb = fmaf(Fb[1], v, Fb[0]);
+    float vb = Fb[1] * u[1] + Fb[2] * u[2] + Fb[3] * u[3] + Fb[4] * (u[4] + p);
+    const float pb = fmaf(Fb[4], v, Fb[1]);
+    float epsb = Fb[4] * v;
+    // c = |v| + cs   (d|v|/dv = sign(v), sign(0) = 0: R26)
+    const float sgn = (v > 0.f) ? 1.f : ((v < 0.f) ? -1.f : 0.f);
+    vb = fmaf(sgn, cb, vb);
+    // cs = sqrt(gamma (gamma-1) e+)
+    const float half_cs_inv = 0.5f * rcp_fast(cs);
+    float epb = cb * sc.ggm1 * half_cs_inv;
+    gamma_b = fmaf(cb * (2.f * sc.gamma - 1.f) * ep, half_cs_inv, gamma_b);
+    // p = (gamma - 1) rho e+
+    gamma_b = fmaf(pb * u[0], ep, gamma_b);
+    float rhob = pb * sc.gm1 * ep;
+    epb = fmaf(pb * sc.gm1, u[0], epb);
+    // e+ = max(e, floor);  e = (eps - ke)/rho, ke = m2/(2 rho)
+    const float eb = active ? epb : 0.f;
+    const float ebr = eb * rinv;
+    epsb += ebr;
+    rhob += ebr * (2.f * ke * rinv - u[4] * rinv);       // eb * (-eps/rho^2 + m2/rho^3)
+    const float mcoef = -ebr * rinv;                       // -eb / rho^2
+    mnb = fmaf(mcoef, u[1], mnb);
+    // v = m_n / rho
+    mnb = fmaf(vb, rinv, mnb);
+    rhob -= vb * v * rinv;
+    ub[0] += rhob;
+    ub[1] += mnb;
+    ub[2] += fmaf(mcoef, u[2], Fb[2] * v);
+    ub[3] += fmaf(mcoef, u[3], Fb[3] * v);
+    ub[4] += epsb;
+}
+
+// L(A,B) = AB / (A + B + sign(A) eps4) if AB > 0 else 0
+__device__ __forceinline__ float limL(float A, float B, float eps4) {
+    const float t = A * B;
+    const float den = (A + B) + copysignf(eps4, A);
+    const float r = t * rcp_fast(den);
+    return t > 0.f ? r : 0.f;
+}
+// value and both partials:  L_A = B (B + s eps4)/den^2,  L_B = A (A + s eps4)/den^2
+__device__ __forceinline__ float limL_grad(float A, float B, float eps4, float& LA, float& LB) {
+    const float t = A * B;
+    const float s = copysignf(eps4, A);
+    const float den = (A + B) + s;
+    const float rd = rcp_fast(den);
+    const bool on = t > 0.f;
+    const float rd2 = rd * rd;
+    LA = on ? B * (B + s) * rd2 : 0.f;
+    LB = on ? A * (A + s) * rd2 : 0.f;
+    return on ? t * rd : 0.f;
+}
+
+// Marching-kernel forms of the limiter.  EPS = false drops the sign(A) 4 eps term of the denominator: for
+// 4 eps <= 4e-18 it changes L by at most 2 eps in absolute value (L = AB/(A+B) <= min(|A|,|B|)), far below one fp32
+// rounding of any flux the scheme produces; launchers pick EPS = true whenever lim_eps > 1e-18.
+// The gate AB > 0 is applied to the reciprocal, so value and partials all vanish with one select.
+template <bool EPS>
+__device__ __forceinline__ float limM(float A, float B, float eps4) {
+    const float t = A * B;
+    float den = A + B;
+    if (EPS) den += copysignf(eps4, A);
+    const float r = t > 0.f ? rcp_fast(den) : 0.f;
+    return t * r;
+}
+// value and partials: with w = 1/den (0 when gated off), L = A B w, L_A = B (B + s) w^2, L_B = A (A + s) w^2
+template <bool EPS>
+__device__ __forceinline__ float limM_grad(float A, float B, float eps4, float& LA, float& LB) {
+    const float t = A * B;
+    const float s = EPS ? copysignf(eps4, A) : 0.f;
+    const float den = (A + B) + s;
+    const float r = t > 0.f ? rcp_fast(den) : 0.f;
+    const float wA = A * r, wB = B * r;
+    if (EPS) {
+        LA = wB * ((B + s) * r);
+        LB = wA * ((A + s) * r);
+    } else {
+        LA = wB * wB;
+        LB = wA * wA;
+    }
+    return A * wB;
+}
+
+struct Ptr5 { const float* p[5]; };
+struct MPtr5 { float* p[5]; };
+
+__device__ __forceinline__ void block_max_to_global(float v, float* out, int* smem_slot) {
+    // all values are >= 0 or NaN: compare as ints (NaN = 0x7fc00000 wins, which is what the NONFINITE check wants)
+    int iv = __float_as_int(v) & 0x7fffffff;
+    iv = __reduce_max_sync(0xffffffffu, iv);
+    if ((threadIdx.x + threadIdx.y * blockDim.x) % 32 == 0) atomicMax(smem_slot, iv);
+    __syncthreads();
+    if (threadIdx.x == 0 && threadIdx.y == 0) atomicMax(reinterpret_cast<int*>(out), *smem_slot);
+}
+
+__device__ __forceinline__ void block_sum3_to_global(float a, float b, float c, double* out, float* sm /*3*32*/) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+        c += __shfl_xor_sync(0xffffffffu, c, o);
+    }
+    const int t = threadIdx.x + threadIdx.y * blockDim.x;
+    const int w = t >> 5, nw = (blockDim.x * blockDim.y + 31) >> 5;
+    if ((t & 31) == 0) { sm[w] = a; sm[32 + w] = b; sm[64 + w] = c; }
+    __syncthreads();
+    if (t < 32) {
+        double da = t < nw ? (double)sm[t] : 0.0, db = t < nw ? (double)sm[32 + t] : 0.0, dc = t < nw ? (double)sm[64 + t] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            da += __shfl_xor_sync(0xffffffffu, da, o);
+            db += __shfl_xor_sync(0xffffffffu, db, o);
+            dc += __shfl_xor_sync(0xffffffffu, dc, o);
+        }
+        if (t == 0) { atomicAdd(out + 0, da); atomicAdd(out + 1, db); atomicAdd(out + 2, dc); }
+    }
+}
+
+// marching y/z kernels (sweep_march.cu); the field pointers are already permuted to (rho, m_n, m_t1, m_t2, eps)
+int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
+                       const SweepConst& sc);
+int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, const Ptr5& pco, const MPtr5& pci,
+                           float* gbar, double* scal, const SweepConst& sc);
+
+}  // namespace dh

@@ -1,0 +1,391 @@
+// sweep_march.cu -- y and z sweeps of the relaxing-TVD scheme (forward and adjoint) as register-streaming
+// ("marching") kernels for sm_100a.
+//
+// The scheme is the one stated at the top of sweep.cu (section 2.3.1-2.3.2, Eq. 9-18, :105-150; readings
+// R3-R8, R11, R17 of DESIGN.md).  Layout: a warp's 32 lanes are 32 consecutive x (every load and store is one
+// coalesced 128-byte row segment); a thread owns ONE pencil segment of `S` cells along the sweep axis and marches
+// along it.  Everything the two Runge-Kutta stages need from neighbouring cells is carried in registers from one
+// iteration to the next, so there is no shared-memory exchange, no barrier, and nothing is computed twice except the
+// HALO cells at the two ends of a segment (3 forward, 4 adjoint).
+//
+// Forward pipeline, iteration that loads cell q (delay 3: it finishes cell q-3):
+//   P(u_q) -> G_q, H_q ; D_{q-1} = G_{q-1} - H_q ; u*_{q-1} ; P(u*_{q-1}) -> G*_{q-1}, H*_{q-1}
+//   PsiG_{q-2} = G*_{q-2} + L(dG_{q-3}, dG_{q-2})        dG_n = G*_{n+1} - G*_n
+//   PsiH_{q-3} = H*_{q-2} - L(dH_{q-3}, dH_{q-2})        dH_n = H*_{n+1} - H*_n
+//   Psi_{q-3}  = PsiG_{q-3} - PsiH_{q-3} ;  u'_{q-3} = R_{q-3} - (lam/2)(Psi_{q-3} - Psi_{q-4}),  R_n = u_n + kap S(u*_n, g_n)
+// Adjoint pipeline (delay 4: the iteration that loads u_q, g_q and the output cotangent ob_{q-1} finishes u_b of cell
+// q-4 and g_b of cell q-3): the forward recompute above, then with Psi_b_n = -(lam/2)(ob_n - ob_{n+1})
+//   G-limiter of interface q-2 and H-limiter of interface q-3 -> G*_b, H*_b of cell q-3 complete
+//   u*_b_{q-3} = P^T(u*_{q-3})(G*_b, H*_b) + source terms ;  D_b_{q-4} = -(lam/4)(u*_b_{q-4} - u*_b_{q-3})
+//   u_b_{q-4} = ob + u*_b + (kap/2) source^T + P^T(u_{q-4})(D_b_{q-4}, -D_b_{q-5})
+// lam_b is formed without carrying D or Psi:  stage B by summation by parts, sum_n Psi_n Psi_b_n / lam; stage A from
+// u*_n - u_n - (kap/2) S = -(lam/4)(D_n - D_{n-1}).
+#include "sweep_common.cuh"
+
+namespace dh {
+
+// wrapped running offset along the sweep axis: off = base + p * stride, p in [0, N)
+struct AxisPos {
+    int p, off;
+    __device__ __forceinline__ void set(int p_unwrapped, int N, int base, int stride) {
+        p = p_unwrapped < 0 ? p_unwrapped + N : (p_unwrapped >= N ? p_unwrapped - N : p_unwrapped);
+        off = base + p * stride;
+    }
+    __device__ __forceinline__ void next(int N, int base, int stride) {
+        ++p; off += stride;
+        if (p == N) { p = 0; off = base; }
+    }
+};
+
+// ------------------------------------------------------------------------------------------------- forward ----
+template <bool HAS_G, bool EPS>
+struct FwdPipe {
+    float u1[5], g1, G1[5], D2[5];       // u_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
+    float R1[5], R2[5];                  // R_{q-2}, R_{q-3}
+    float Gs[5], dGs[5], Hs[5], dHs[5];  // G*_{q-2}, dG_{q-3}, H*_{q-2}, dH_{q-3}
+    float PG[5], Psi[5];                 // PsiG_{q-3}, Psi_{q-4}
+
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            u1[k] = 1.f; G1[k] = 0.f; D2[k] = 0.f; R1[k] = 0.f; R2[k] = 0.f; Gs[k] = 0.f; dGs[k] = 0.f; Hs[k] = 0.f;
+            dHs[k] = 0.f; PG[k] = 0.f; Psi[k] = 0.f;
+        }
+        g1 = 0.f;
+    }
+
+    // take cell q; out = u'_{q-3}; c0 = freezing speed of cell q
+    __device__ __forceinline__ void push(const float (&u0)[5], float g0, const SweepConst& sc, float (&out)[5], float& c0) {
+        float G0[5], H0[5];
+        prim_GH(u0, sc, G0, H0, c0);
+        float us[5], D1[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            D1[k] = G1[k] - H0[k];
+            us[k] = fmaf(-0.25f * sc.lam, D1[k] - D2[k], u1[k]);
+        }
+        float R0[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) R0[k] = u1[k];
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * g1;
+            us[1] = fmaf(hk, u1[0], us[1]);
+            us[4] = fmaf(hk, u1[1], us[4]);
+            const float kg = sc.kap * g1;
+            R0[1] = fmaf(kg, us[0], R0[1]);
+            R0[4] = fmaf(kg, us[1], R0[4]);
+        }
+        float Gs0[5], Hs0[5], cdummy;
+        prim_GH(us, sc, Gs0, Hs0, cdummy);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const float dG0 = Gs0[k] - Gs[k];
+            const float dH0 = Hs0[k] - Hs[k];
+            const float PG0 = Gs[k] + limM<EPS>(dGs[k], dG0, sc.eps4);
+            const float PH = Hs[k] - limM<EPS>(dHs[k], dH0, sc.eps4);
+            const float Psi0 = PG[k] - PH;
+            out[k] = fmaf(-0.5f * sc.lam, Psi0 - Psi[k], R2[k]);
+            // rotate
+            Psi[k] = Psi0; PG[k] = PG0;
+            Gs[k] = Gs0[k]; dGs[k] = dG0; Hs[k] = Hs0[k]; dHs[k] = dH0;
+            R2[k] = R1[k]; R1[k] = R0[k];
+            u1[k] = u0[k]; G1[k] = G0[k]; D2[k] = D1[k];
+        }
+        g1 = g0;
+    }
+};
+
+// block = (BX lanes along x, BY pencils); grid = (N / BX, N / BY, segments along the sweep axis)
+template <int DIR, bool HAS_G, bool EPS>
+__global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const float* __restrict__ gfield, MPtr5 outp,
+                                                                 float* cmax, SweepConst sc, int S) {
+    constexpr int HALO = 3;
+    __shared__ int s_max;
+    if (threadIdx.x == 0 && threadIdx.y == 0) s_max = 0;
+    __syncthreads();
+    const int N = sc.N;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int o = blockIdx.y * blockDim.y + threadIdx.y;
+    const int p0 = blockIdx.z * S;
+    const int len = min(S, N - p0);
+    const int stride = DIR == 1 ? N : N * N;
+    const int base = DIR == 1 ? o * N * N + x : o * N + x;
+    AxisPos ld;
+    ld.set(p0 - HALO, N, base, stride);
+    int off_out = base + p0 * stride;
+    FwdPipe<HAS_G, EPS> pipe;
+    pipe.init();
+    float un[5], gn = 0.f;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) un[k] = __ldg(in.p[k] + ld.off);
+    if (HAS_G) gn = __ldg(gfield + ld.off);
+    float cm = 0.f;
+    const int niter = len + 2 * HALO;
+#pragma unroll 2
+    for (int i = 0; i < niter; ++i) {
+        float u0[5], g0 = gn;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) u0[k] = un[k];
+        if (i + 1 < niter) {                        // prefetch the next cell
+            ld.next(N, base, stride);
+#pragma unroll
+            for (int k = 0; k < 5; ++k) un[k] = __ldg(in.p[k] + ld.off);
+            if (HAS_G) gn = __ldg(gfield + ld.off);
+        }
+        float out[5], c0;
+        pipe.push(u0, g0, sc, out, c0);
+        cm = (c0 > cm || c0 != c0) ? c0 : cm;
+        if (i >= 2 * HALO) {
+#pragma unroll
+            for (int k = 0; k < 5; ++k) outp.p[k][off_out] = out[k];
+            off_out += stride;
+        }
+    }
+    if (cmax) block_max_to_global(cm, cmax, &s_max);
+}
+
+// ------------------------------------------------------------------------------------------------- adjoint ----
+template <bool HAS_G, bool EPS>
+struct AdjPipe {
+    // forward recompute
+    float u1[5], g1, G1[5], D2[5];         // u_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
+    float us1[5], us2[5];                  // u*_{q-2}, u*_{q-3}
+    float Gs[5], dGs[5], Hs[5], dHs[5];    // G*_{q-2}, dG_{q-3}, H*_{q-2}, dH_{q-3}
+    // cotangents in flight
+    float ob1[5], ob2[5];                  // ob_{q-2}, ob_{q-3}
+    float GB0[5], GB1[5];                  // partial G*_b of cells q-3 (interfaces q-4, q-3) and q-2 (interface q-3)
+    float HB0[5], HB1[5];                  // partial H*_b of cells q-3 (interfaces q-5, q-4) and q-2 (interface q-4)
+    float uR[5], accR[5], usbR[5], DbR[5]; // u_{q-4}, ob + u*_b + source^T of cell q-4, u*_b_{q-4}, D_b_{q-5}
+
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            u1[k] = 1.f; G1[k] = 0.f; D2[k] = 0.f; us1[k] = 1.f; us2[k] = 1.f; Gs[k] = 0.f; dGs[k] = 0.f; Hs[k] = 0.f;
+            dHs[k] = 0.f; ob1[k] = 0.f; ob2[k] = 0.f; GB0[k] = 0.f; GB1[k] = 0.f; HB0[k] = 0.f; HB1[k] = 0.f;
+            uR[k] = 1.f; accR[k] = 0.f; usbR[k] = 0.f; DbR[k] = 0.f;
+        }
+        g1 = 0.f;
+    }
+
+    // Takes u_q, g_q, ob_{q-1} and the re-read u_{q-3}, g_{q-3}.  Returns ub = u_b of cell q-4, gb = g_b of cell q-3,
+    // and the scalar-cotangent terms of this iteration, split by the cell / interface they belong to so the caller
+    // can count each once: lamG (interface q-2), lamH (interface q-3), and for cell q-3: lamA, kapM, gamM; for cell
+    // q-4: gamR.
+    __device__ __forceinline__ void push(const float (&u0)[5], float g0, const float (&ob0)[5], const float (&uM)[5],
+                                         float gM, const SweepConst& sc, float (&ub)[5], float& gb, float& lamG,
+                                         float& lamH, float& lamA, float& kapM, float& gamM, float& gamR) {
+        // ---- forward recompute: P(u_q), u*_{q-1}, P(u*_{q-1})
+        float G0[5], H0[5], cdummy;
+        prim_GH(u0, sc, G0, H0, cdummy);
+        float us0[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const float D1 = G1[k] - H0[k];
+            us0[k] = fmaf(-0.25f * sc.lam, D1 - D2[k], u1[k]);
+            D2[k] = D1;
+        }
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * g1;
+            us0[1] = fmaf(hk, u1[0], us0[1]);
+            us0[4] = fmaf(hk, u1[1], us0[4]);
+        }
+        float Gs0[5], Hs0[5];
+        prim_GH(us0, sc, Gs0, Hs0, cdummy);
+        // ---- limiters: G side of interface q-2, H side of interface q-3; G*_b, H*_b of cell q-3 complete
+        float GsB[5], HsB[5];
+        float lg = 0.f, lh = 0.f;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const float dG0 = Gs0[k] - Gs[k];
+            const float dH0 = Hs0[k] - Hs[k];
+            float LA, LB, MA, MB;
+            const float L = limM_grad<EPS>(dGs[k], dG0, sc.eps4, LA, LB);
+            const float M = limM_grad<EPS>(dHs[k], dH0, sc.eps4, MA, MB);
+            const float dob0 = ob1[k] - ob0[k];           // ob_{q-2} - ob_{q-1}
+            const float dob1 = ob2[k] - ob1[k];           // ob_{q-3} - ob_{q-2}
+            const float pb0 = -0.5f * sc.lam * dob0;      // Psi_b of interface q-2
+            const float pb1 = -0.5f * sc.lam * dob1;      // Psi_b of interface q-3
+            lg = fmaf(Gs[k] + L, dob0, lg);               // PsiG_{q-2} (ob_{q-2} - ob_{q-1})
+            lh = fmaf(Hs[k] - M, dob1, lh);               // PsiH_{q-3} (ob_{q-3} - ob_{q-2})
+            GsB[k] = fmaf(-LA, pb0, GB0[k]);
+            GB0[k] = fmaf(1.f + LA - LB, pb0, GB1[k]);
+            GB1[k] = LB * pb0;
+            HsB[k] = fmaf(-MA, pb1, HB0[k]);
+            HB0[k] = fmaf(-1.f + MA - MB, pb1, HB1[k]);
+            HB1[k] = MB * pb1;
+            Gs[k] = Gs0[k]; dGs[k] = dG0; Hs[k] = Hs0[k]; dHs[k] = dH0;
+        }
+        lamG = -0.5f * lg;
+        lamH = 0.5f * lh;
+        // ---- cell m = q-3: u*_b, g_b, the additive part of u_b
+        float usb[5];
+        gamM = 0.f;
+        prim_GH_vjp(us2, sc, GsB, HsB, usb, gamM);
+        float acc[5];
+        gb = 0.f; kapM = 0.f;
+        if (HAS_G) {
+            const float kg = sc.kap * gM;
+            usb[0] = fmaf(kg, ob2[1], usb[0]);
+            usb[1] = fmaf(kg, ob2[4], usb[1]);
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k) acc[k] = ob2[k] + usb[k];
+        float dA = 0.f;                                   // sum_k u*_b (u - u* + (kap/2) g S(u))
+#pragma unroll
+        for (int k = 0; k < 5; ++k) dA = fmaf(usb[k], uM[k] - us2[k], dA);
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * gM;
+            acc[0] = fmaf(hk, usb[1], acc[0]);
+            acc[1] = fmaf(hk, usb[4], acc[1]);
+            const float tB = us2[0] * ob2[1] + us2[1] * ob2[4];
+            const float tA = uM[0] * usb[1] + uM[1] * usb[4];
+            const float t = fmaf(0.5f, tA, tB);
+            gb = sc.kap * t;
+            kapM = gM * t;
+            dA = fmaf(hk, tA, dA);
+        }
+        lamA = -sc.inv_lam * dA;
+        // ---- cell r = q-4: stage-A transpose
+        float Gb[5], Hb[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const float Db = -0.25f * sc.lam * (usbR[k] - usb[k]);
+            Gb[k] = Db;
+            Hb[k] = -DbR[k];
+            DbR[k] = Db;
+            usbR[k] = usb[k];
+        }
+        gamR = 0.f;
+        prim_GH_vjp(uR, sc, Gb, Hb, ub, gamR);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            ub[k] += accR[k];
+            accR[k] = acc[k];
+            uR[k] = uM[k];
+            // rotate the rest
+            us2[k] = us1[k]; us1[k] = us0[k];
+            ob2[k] = ob1[k]; ob1[k] = ob0[k];
+            u1[k] = u0[k]; G1[k] = G0[k];
+        }
+        g1 = g0;
+    }
+};
+
+template <int DIR, bool HAS_G, bool EPS>
+__global__ void __launch_bounds__(128, 3) sweep_march_adj_kernel(Ptr5 in, const float* __restrict__ gfield, Ptr5 cot_out,
+                                                                 MPtr5 cot_in, float* __restrict__ gbar, double* scal,
+                                                                 SweepConst sc, int S) {
+    constexpr int HALO = 4;
+    __shared__ float s_red[96];
+    const int N = sc.N;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int o = blockIdx.y * blockDim.y + threadIdx.y;
+    const int p0 = blockIdx.z * S;
+    const int len = min(S, N - p0);
+    const int stride = DIR == 1 ? N : N * N;
+    const int base = DIR == 1 ? o * N * N + x : o * N + x;
+    AxisPos ldq, ldo, ldm;                       // cells q (u, g), q-1 (ob), q-3 (re-read u, g; g_b store)
+    ldq.set(p0 - HALO, N, base, stride);
+    ldo.set(p0 - HALO - 1, N, base, stride);
+    ldm.set(p0 - HALO - 3, N, base, stride);
+    int off_r = base + p0 * stride;              // cell q-4 once it is owned
+    AdjPipe<HAS_G, EPS> pipe;
+    pipe.init();
+    float lacc = 0.f, kacc = 0.f, gacc = 0.f;
+    const int niter = len + 2 * HALO;
+#pragma unroll 1
+    for (int i = 0; i < niter; ++i) {
+        float u0[5], ob0[5], uM[5], g0 = 0.f, gM = 0.f;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            u0[k] = __ldg(in.p[k] + ldq.off);
+            ob0[k] = __ldg(cot_out.p[k] + ldo.off);
+            uM[k] = __ldg(in.p[k] + ldm.off);
+        }
+        if (HAS_G) { g0 = __ldg(gfield + ldq.off); gM = __ldg(gfield + ldm.off); }
+        float ub[5], gb, lamG, lamH, lamA, kapM, gamM, gamR;
+        pipe.push(u0, g0, ob0, uM, gM, sc, ub, gb, lamG, lamH, lamA, kapM, gamM, gamR);
+        // interface q-2 = p0 + i - 6, cell / interface q-3 = p0 + i - 7, cell q-4 = p0 + i - 8
+        if (i >= 6 && i < len + 6) lacc += lamG;
+        if (i >= 7 && i < len + 7) {
+            lacc += lamH + lamA; kacc += kapM; gacc += gamM;
+            if (HAS_G) gbar[ldm.off] = gb;
+        }
+        if (i >= 8) {
+            gacc += gamR;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) cot_in.p[k][off_r] = ub[k];
+            off_r += stride;
+        }
+        ldq.next(N, base, stride);
+        ldo.next(N, base, stride);
+        ldm.next(N, base, stride);
+    }
+    block_sum3_to_global(lacc, kacc, gacc, scal, s_red);
+}
+
+// ----------------------------------------------------------------------------------------------- launchers ----
+static dim3 march_block(int N) { return dim3(N % 128 == 0 ? 128 : (N % 64 == 0 ? 64 : 32), 1, 1); }
+
+static int march_segment(int N, int tuned, int halo) {
+    // segment length: long enough that the 2*halo recomputed cells stay a small fraction, short enough that the grid
+    // holds several waves of blocks on 148 SMs
+    int S = tuned > 0 ? tuned : (N >= 128 ? 64 : 32);
+    if (S > N) S = N;
+    if (S < 2 * halo) S = 2 * halo;
+    return S;
+}
+
+template <int DIR>
+static int march_fwd_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const MPtr5& pout,
+                              float* cmax, const SweepConst& sc, int S, bool eps) {
+    if (g) {
+        if (eps) sweep_march_fwd_kernel<DIR, true, true><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+        else sweep_march_fwd_kernel<DIR, true, false><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+    } else {
+        if (eps) sweep_march_fwd_kernel<DIR, false, true><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+        else sweep_march_fwd_kernel<DIR, false, false><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+    }
+    return DH_OK;
+}
+
+template <int DIR>
+static int march_adj_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const Ptr5& pco,
+                              const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S, bool eps) {
+    if (g) {
+        if (eps) sweep_march_adj_kernel<DIR, true, true><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+        else sweep_march_adj_kernel<DIR, true, false><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+    } else {
+        if (eps) sweep_march_adj_kernel<DIR, false, true><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+        else sweep_march_adj_kernel<DIR, false, false><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+    }
+    return DH_OK;
+}
+
+int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
+                       const SweepConst& sc) {
+    const int N = c->N;
+    const int S = march_segment(N, c->tune_march_s_fwd, 3);
+    const dim3 block = march_block(N);
+    const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
+    const bool eps = c->opt.lim_eps > 1e-18;
+    if (d == 1) march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps);
+    else march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps);
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, const Ptr5& pco, const MPtr5& pci,
+                           float* gbar, double* scal, const SweepConst& sc) {
+    const int N = c->N;
+    const int S = march_segment(N, c->tune_march_s_adj, 4);
+    const dim3 block = march_block(N);
+    const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
+    const bool eps = c->opt.lim_eps > 1e-18;
+    if (d == 1) march_adj_dispatch<1>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    else march_adj_dispatch<2>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+}  // namespace dh
