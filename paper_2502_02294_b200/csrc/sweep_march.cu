@@ -95,13 +95,36 @@ struct FwdPipe {
     }
 };
 
+// Asynchronous staging ring.  Every thread copies the cells of ITS OWN pencil a few iterations ahead of their use with
+// 4-byte cp.async (a warp's 32 copies are one coalesced 128-byte row segment) into ring[stage][field][thread] and reads
+// them back with conflict-free LDS; since a thread only ever reads what it copied itself, cp.async.wait_group is the
+// only synchronisation -- no barrier.  The ring hides the HBM latency that 12-16 resident warps of a register-heavy
+// kernel cannot, and in the adjoint doubles as the window of already-visited cells (re-read instead of carried).
+__device__ __forceinline__ void cp_async4(float* smem_dst, const float* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int PENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
+
+constexpr int RING = 8;          // stages (power of two)
+constexpr int PF_FWD = 3;        // iterations of prefetch, forward
+constexpr int PF_ADJ = 2;
+#ifndef DH_ADJ_BLOCKS
+#define DH_ADJ_BLOCKS 3
+#endif
+constexpr int ADJ_BLOCKS = DH_ADJ_BLOCKS;        // adjoint: stages i-4 .. i are re-read, i+1 .. i+2 in flight, one spare
+
 // block = (BX lanes along x, BY pencils); grid = (N / BX, N / BY, segments along the sweep axis)
 template <int DIR, bool HAS_G, bool EPS>
 __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const float* __restrict__ gfield, MPtr5 outp,
                                                                  float* cmax, SweepConst sc, int S) {
-    constexpr int HALO = 3;
+    constexpr int HALO = 3, NF = HAS_G ? 6 : 5;
+    extern __shared__ float ring[];              // [RING][NF][nthr]
     __shared__ int s_max;
-    if (threadIdx.x == 0 && threadIdx.y == 0) s_max = 0;
+    const int nthr = blockDim.x * blockDim.y, tid = threadIdx.y * blockDim.x + threadIdx.x;
+    if (tid == 0) s_max = 0;
     __syncthreads();
     const int N = sc.N;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -110,28 +133,36 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
     const int len = min(S, N - p0);
     const int stride = DIR == 1 ? N : N * N;
     const int base = DIR == 1 ? o * N * N + x : o * N + x;
+    const int niter = len + 2 * HALO;
     AxisPos ld;
     ld.set(p0 - HALO, N, base, stride);
     int off_out = base + p0 * stride;
+    float* const my = ring + tid;
+    auto issue = [&](int it) {
+        float* dst = my + (it & (RING - 1)) * NF * nthr;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) cp_async4(dst + k * nthr, in.p[k] + ld.off);
+        if (HAS_G) cp_async4(dst + 5 * nthr, gfield + ld.off);
+        ld.next(N, base, stride);
+    };
+#pragma unroll
+    for (int it = 0; it < PF_FWD; ++it) {
+        if (it < niter) issue(it);
+        cp_async_commit();
+    }
     FwdPipe<HAS_G, EPS> pipe;
     pipe.init();
-    float un[5], gn = 0.f;
-#pragma unroll
-    for (int k = 0; k < 5; ++k) un[k] = __ldg(in.p[k] + ld.off);
-    if (HAS_G) gn = __ldg(gfield + ld.off);
     float cm = 0.f;
-    const int niter = len + 2 * HALO;
 #pragma unroll 2
     for (int i = 0; i < niter; ++i) {
-        float u0[5], g0 = gn;
+        if (i + PF_FWD < niter) issue(i + PF_FWD);
+        cp_async_commit();
+        cp_async_wait<PF_FWD>();
+        const float* src = my + (i & (RING - 1)) * NF * nthr;
+        float u0[5], g0 = 0.f;
 #pragma unroll
-        for (int k = 0; k < 5; ++k) u0[k] = un[k];
-        if (i + 1 < niter) {                        // prefetch the next cell
-            ld.next(N, base, stride);
-#pragma unroll
-            for (int k = 0; k < 5; ++k) un[k] = __ldg(in.p[k] + ld.off);
-            if (HAS_G) gn = __ldg(gfield + ld.off);
-        }
+        for (int k = 0; k < 5; ++k) u0[k] = src[k * nthr];
+        if (HAS_G) g0 = src[5 * nthr];
         float out[5], c0;
         pipe.push(u0, g0, sc, out, c0);
         cm = (c0 > cm || c0 != c0) ? c0 : cm;
@@ -152,28 +183,28 @@ struct AdjPipe {
     float us1[5], us2[5];                  // u*_{q-2}, u*_{q-3}
     float Gs[5], dGs[5], Hs[5], dHs[5];    // G*_{q-2}, dG_{q-3}, H*_{q-2}, dH_{q-3}
     // cotangents in flight
-    float ob1[5], ob2[5];                  // ob_{q-2}, ob_{q-3}
     float GB0[5], GB1[5];                  // partial G*_b of cells q-3 (interfaces q-4, q-3) and q-2 (interface q-3)
     float HB0[5], HB1[5];                  // partial H*_b of cells q-3 (interfaces q-5, q-4) and q-2 (interface q-4)
-    float uR[5], accR[5], usbR[5], DbR[5]; // u_{q-4}, ob + u*_b + source^T of cell q-4, u*_b_{q-4}, D_b_{q-5}
+    float accR[5], usbR[5], DbR[5];        // ob + u*_b + source^T of cell q-4, u*_b_{q-4}, D_b_{q-5}
 
     __device__ __forceinline__ void init() {
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             u1[k] = 1.f; G1[k] = 0.f; D2[k] = 0.f; us1[k] = 1.f; us2[k] = 1.f; Gs[k] = 0.f; dGs[k] = 0.f; Hs[k] = 0.f;
-            dHs[k] = 0.f; ob1[k] = 0.f; ob2[k] = 0.f; GB0[k] = 0.f; GB1[k] = 0.f; HB0[k] = 0.f; HB1[k] = 0.f;
-            uR[k] = 1.f; accR[k] = 0.f; usbR[k] = 0.f; DbR[k] = 0.f;
+            dHs[k] = 0.f; GB0[k] = 0.f; GB1[k] = 0.f; HB0[k] = 0.f; HB1[k] = 0.f;
+            accR[k] = 0.f; usbR[k] = 0.f; DbR[k] = 0.f;
         }
         g1 = 0.f;
     }
 
-    // Takes u_q, g_q, ob_{q-1} and the re-read u_{q-3}, g_{q-3}.  Returns ub = u_b of cell q-4, gb = g_b of cell q-3,
-    // and the scalar-cotangent terms of this iteration, split by the cell / interface they belong to so the caller
-    // can count each once: lamG (interface q-2), lamH (interface q-3), and for cell q-3: lamA, kapM, gamM; for cell
-    // q-4: gamR.
-    __device__ __forceinline__ void push(const float (&u0)[5], float g0, const float (&ob0)[5], const float (&uM)[5],
-                                         float gM, const SweepConst& sc, float (&ub)[5], float& gb, float& lamG,
-                                         float& lamH, float& lamA, float& kapM, float& gamM, float& gamR) {
+    // Takes u_q, g_q and, re-read from the ring, ob_{q-1}, ob_{q-2}, ob_{q-3}, u_{q-3}, g_{q-3}, u_{q-4}.  Returns
+    // ub = u_b of cell q-4, gb = g_b of cell q-3, and the scalar-cotangent terms of this iteration split by the cell /
+    // interface they belong to so the caller can count each once: lamG (interface q-2), lamH (interface q-3), and
+    // for cell q-3: lamA, kapM, gamM; for cell q-4: gamR.
+    __device__ __forceinline__ void push(const float (&u0)[5], float g0, const float (&ob0)[5], const float (&ob1)[5],
+                                         const float (&ob2)[5], const float (&uM)[5], float gM, const float (&uR)[5],
+                                         const SweepConst& sc, float (&ub)[5], float& gb, float& lamG, float& lamH,
+                                         float& lamA, float& kapM, float& gamM, float& gamR) {
         // ---- forward recompute: P(u_q), u*_{q-1}, P(u*_{q-1})
         float G0[5], H0[5], cdummy;
         prim_GH(u0, sc, G0, H0, cdummy);
@@ -261,10 +292,8 @@ struct AdjPipe {
         for (int k = 0; k < 5; ++k) {
             ub[k] += accR[k];
             accR[k] = acc[k];
-            uR[k] = uM[k];
             // rotate the rest
             us2[k] = us1[k]; us1[k] = us0[k];
-            ob2[k] = ob1[k]; ob1[k] = ob0[k];
             u1[k] = u0[k]; G1[k] = G0[k];
         }
         g1 = g0;
@@ -272,11 +301,14 @@ struct AdjPipe {
 };
 
 template <int DIR, bool HAS_G, bool EPS>
-__global__ void __launch_bounds__(128, 3) sweep_march_adj_kernel(Ptr5 in, const float* __restrict__ gfield, Ptr5 cot_out,
-                                                                 MPtr5 cot_in, float* __restrict__ gbar, double* scal,
-                                                                 SweepConst sc, int S) {
-    constexpr int HALO = 4;
+__global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 in, const float* __restrict__ gfield,
+                                                                          Ptr5 cot_out, MPtr5 cot_in,
+                                                                          float* __restrict__ gbar, double* scal,
+                                                                          SweepConst sc, int S) {
+    constexpr int HALO = 4, NF = HAS_G ? 11 : 10, OB = HAS_G ? 6 : 5;
+    extern __shared__ float ring[];              // [RING][NF][nthr]: u (5), g, ob (5) of one cell per stage
     __shared__ float s_red[96];
+    const int nthr = blockDim.x * blockDim.y, tid = threadIdx.y * blockDim.x + threadIdx.x;
     const int N = sc.N;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int o = blockIdx.y * blockDim.y + threadIdx.y;
@@ -284,47 +316,85 @@ __global__ void __launch_bounds__(128, 3) sweep_march_adj_kernel(Ptr5 in, const 
     const int len = min(S, N - p0);
     const int stride = DIR == 1 ? N : N * N;
     const int base = DIR == 1 ? o * N * N + x : o * N + x;
-    AxisPos ldq, ldo, ldm;                       // cells q (u, g), q-1 (ob), q-3 (re-read u, g; g_b store)
-    ldq.set(p0 - HALO, N, base, stride);
-    ldo.set(p0 - HALO - 1, N, base, stride);
-    ldm.set(p0 - HALO - 3, N, base, stride);
-    int off_r = base + p0 * stride;              // cell q-4 once it is owned
+    const int niter = len + 2 * HALO;
+    AxisPos ld;
+    ld.set(p0 - HALO, N, base, stride);
+    int off_m = base + (p0 - 1) * stride;         // cell q-3 (g_b store), valid from the first owned cell on
+    int off_r = base + (p0 - 1) * stride;         // cell q-4 (u_b store)
+    float* const my = ring + tid;
+    auto issue = [&](int it) {
+        float* dst = my + (it & (RING - 1)) * NF * nthr;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            cp_async4(dst + k * nthr, in.p[k] + ld.off);
+            cp_async4(dst + (OB + k) * nthr, cot_out.p[k] + ld.off);
+        }
+        if (HAS_G) cp_async4(dst + 5 * nthr, gfield + ld.off);
+        ld.next(N, base, stride);
+    };
+    // stages -4 .. -1 are read (as ob / re-read cells) before they were ever filled: give them finite values
+#pragma unroll
+    for (int st = RING - 4; st < RING; ++st)
+#pragma unroll
+        for (int k = 0; k < NF; ++k) my[(st * NF + k) * nthr] = k < 5 ? 1.f : 0.f;
+#pragma unroll
+    for (int it = 0; it < PF_ADJ; ++it) {
+        if (it < niter) issue(it);
+        cp_async_commit();
+    }
     AdjPipe<HAS_G, EPS> pipe;
     pipe.init();
     float lacc = 0.f, kacc = 0.f, gacc = 0.f;
-    const int niter = len + 2 * HALO;
 #pragma unroll 1
     for (int i = 0; i < niter; ++i) {
-        float u0[5], ob0[5], uM[5], g0 = 0.f, gM = 0.f;
+        if (i + PF_ADJ < niter) issue(i + PF_ADJ);
+        cp_async_commit();
+        cp_async_wait<PF_ADJ>();
+        const float* s0 = my + (i & (RING - 1)) * NF * nthr;
+        const float* s1 = my + ((i - 1) & (RING - 1)) * NF * nthr;
+        const float* s2 = my + ((i - 2) & (RING - 1)) * NF * nthr;
+        const float* s3 = my + ((i - 3) & (RING - 1)) * NF * nthr;
+        const float* s4 = my + ((i - 4) & (RING - 1)) * NF * nthr;
+        float u0[5], ob0[5], ob1[5], ob2[5], uM[5], uR[5], g0 = 0.f, gM = 0.f;
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-            u0[k] = __ldg(in.p[k] + ldq.off);
-            ob0[k] = __ldg(cot_out.p[k] + ldo.off);
-            uM[k] = __ldg(in.p[k] + ldm.off);
+            u0[k] = s0[k * nthr];
+            ob0[k] = s1[(OB + k) * nthr];
+            ob1[k] = s2[(OB + k) * nthr];
+            ob2[k] = s3[(OB + k) * nthr];
+            uM[k] = s3[k * nthr];
+            uR[k] = s4[k * nthr];
         }
-        if (HAS_G) { g0 = __ldg(gfield + ldq.off); gM = __ldg(gfield + ldm.off); }
+        if (HAS_G) { g0 = s0[5 * nthr]; gM = s3[5 * nthr]; }
         float ub[5], gb, lamG, lamH, lamA, kapM, gamM, gamR;
-        pipe.push(u0, g0, ob0, uM, gM, sc, ub, gb, lamG, lamH, lamA, kapM, gamM, gamR);
+        pipe.push(u0, g0, ob0, ob1, ob2, uM, gM, uR, sc, ub, gb, lamG, lamH, lamA, kapM, gamM, gamR);
         // interface q-2 = p0 + i - 6, cell / interface q-3 = p0 + i - 7, cell q-4 = p0 + i - 8
         if (i >= 6 && i < len + 6) lacc += lamG;
-        if (i >= 7 && i < len + 7) {
-            lacc += lamH + lamA; kacc += kapM; gacc += gamM;
-            if (HAS_G) gbar[ldm.off] = gb;
+        if (i >= 7) {
+            off_m += stride;
+            if (i < len + 7) {
+                lacc += lamH + lamA; kacc += kapM; gacc += gamM;
+                if (HAS_G) gbar[off_m] = gb;
+            }
         }
         if (i >= 8) {
+            off_r += stride;
             gacc += gamR;
 #pragma unroll
             for (int k = 0; k < 5; ++k) cot_in.p[k][off_r] = ub[k];
-            off_r += stride;
         }
-        ldq.next(N, base, stride);
-        ldo.next(N, base, stride);
-        ldm.next(N, base, stride);
     }
     block_sum3_to_global(lacc, kacc, gacc, scal, s_red);
 }
 
 // ----------------------------------------------------------------------------------------------- launchers ----
+#define MARCH_LAUNCH(kern, grid, block, sm, stream, ...)                                                        \
+    do {                                                                                                        \
+        if ((sm) > 48 * 1024)                                                                                   \
+            DH_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sm)));        \
+        kern<<<grid, block, sm, stream>>>(__VA_ARGS__);                                                         \
+    } while (0)
+
 static dim3 march_block(int N) { return dim3(N % 128 == 0 ? 128 : (N % 64 == 0 ? 64 : 32), 1, 1); }
 
 static int march_segment(int N, int tuned, int halo) {
@@ -340,11 +410,13 @@ template <int DIR>
 static int march_fwd_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const MPtr5& pout,
                               float* cmax, const SweepConst& sc, int S, bool eps) {
     if (g) {
-        if (eps) sweep_march_fwd_kernel<DIR, true, true><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
-        else sweep_march_fwd_kernel<DIR, true, false><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+        const size_t sm = (size_t)RING * 6 * block.x * block.y * sizeof(float);
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
     } else {
-        if (eps) sweep_march_fwd_kernel<DIR, false, true><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
-        else sweep_march_fwd_kernel<DIR, false, false><<<grid, block, 0, c->stream>>>(pin, g, pout, cmax, sc, S);
+        const size_t sm = (size_t)RING * 5 * block.x * block.y * sizeof(float);
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
     }
     return DH_OK;
 }
@@ -353,11 +425,13 @@ template <int DIR>
 static int march_adj_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const Ptr5& pco,
                               const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S, bool eps) {
     if (g) {
-        if (eps) sweep_march_adj_kernel<DIR, true, true><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
-        else sweep_march_adj_kernel<DIR, true, false><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+        const size_t sm = (size_t)RING * 11 * block.x * block.y * sizeof(float);
+        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
     } else {
-        if (eps) sweep_march_adj_kernel<DIR, false, true><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
-        else sweep_march_adj_kernel<DIR, false, false><<<grid, block, 0, c->stream>>>(pin, g, pco, pci, gbar, scal, sc, S);
+        const size_t sm = (size_t)RING * 10 * block.x * block.y * sizeof(float);
+        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
     }
     return DH_OK;
 }
