@@ -155,7 +155,10 @@ int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
 /* Launch-geometry knobs (performance only; results stay within the parity tolerances).  key (HOST string):
  *   "march_s_fwd", "march_s_adj": cells per thread segment of the marching y/z sweeps (0 = built-in choice);
- *   "yz_chain": 1 routes the y/z sweeps through the shared-memory chain kernels the x sweep uses.
+ *   "yz_chain": 1 routes the y/z sweeps through the shared-memory chain kernels the x sweep uses;
+ *   "tape": 0 makes dh_run_vjp recompute g' and the sweep inputs inside every step VJP instead of keeping them for
+ *           the steps of the segment being reversed (13 N^3 floats per step of a segment; default 1, falls back to
+ *           recomputation by itself when the device cannot hold them).
  * Unknown key: DH_ERR_INVALID. */
 int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of

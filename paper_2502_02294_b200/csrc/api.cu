@@ -91,54 +91,91 @@ static void snapshot_view(const dh_ctx* c, const Snapshot& s, dh_state* st) {
     st->a = s.a; st->dt_prev = s.dt_prev; st->step = s.step;
 }
 
+static void tape_view(const dh_ctx* c, StepTape& t) {
+    for (int d = 0; d < 3; ++d) t.gp[d] = t.buf + (size_t)d * c->n3;
+    for (int i = 0; i < 2; ++i)
+        for (int k = 0; k < 5; ++k) t.sw[i][k] = t.buf + (size_t)(3 + 5 * i + k) * c->n3;
+}
+
+// Tapes for the steps of one segment.  All or nothing: if the device cannot hold them the reverse pass falls back to
+// recomputing g' and the sweep inputs inside every step VJP (same results, more work).
+static bool ensure_tapes(dh_ctx* c, int in_seg) {
+    if (!c->tune_tape) return false;
+    if ((int)c->tapes.size() < in_seg) c->tapes.resize(in_seg);
+    const size_t bytes = (size_t)13 * c->n3 * sizeof(float);
+    for (int i = 0; i < in_seg; ++i) {
+        if (c->tapes[i].buf) continue;
+        if (dev_alloc(c, (void**)&c->tapes[i].buf, bytes) != DH_OK) {
+            for (auto& t : c->tapes) { dev_free(c, t.buf, bytes); t.buf = nullptr; }
+            set_error("");
+            return false;
+        }
+        tape_view(c, c->tapes[i]);
+    }
+    return true;
+}
+
 static void free_snaps(dh_ctx* c, std::vector<Snapshot>& v) {
     for (auto& s : v) dev_free(c, s.buf, state_floats(c) * sizeof(float));
     v.clear();
 }
 
 // S1 + S2: delta_tot and g' from the state's gas density and particle positions.
-static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A) {
+static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A, float* const gp[3]) {
     DH_TRY(launch_deposit(c, gas[0], part[0], part[1], part[2], c->delta));
-    DH_TRY(poisson_forward(c, c->delta, A, c->gp));
+    DH_TRY(poisson_forward(c, c->delta, A, gp));
     return DH_OK;
 }
 
-// The forward step on explicit arrays.  If sweep_inputs != nullptr the inputs of sweeps 2 and 3 are kept there and the
-// particle update is skipped when `skip_particles` (the reverse pass only needs g' and the sweep inputs).
-static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], const StepScalars& s, int64_t step,
-                       float* cmax3, bool skip_particles, float* (*sweep_inputs)[5], bool last_sweep_needed) {
+// The forward step from (gas, part) to (gas_out, part_out); out may alias in (in-place update: the sweeps go
+// gas -> A -> B -> gas_out, every field read and written once per sweep, no copy).  With a tape, g' and the two
+// intermediate gas states A, B are written into it (and survive the step); otherwise they live in the context's
+// scratch.  part_out == nullptr skips the particle update, last_sweep == false stops after sweep 2 (the reverse pass
+// needs nothing more of a segment's last step).
+static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], float* const gas_out[5],
+                       float* const part_out[6], const StepScalars& s, int64_t step, float* cmax3, StepTape* tape,
+                       bool last_sweep) {
     const bool grav = c->opt.gravity_on != 0;
-    if (grav) DH_TRY(compute_gravity(c, gas, part, (float)s.A));
-    if (c->np > 0 && !skip_particles)
-        DH_TRY(launch_kick_drift(c, grav ? c->gp : nullptr, part, (float)s.K, (float)(s.dtau / c->dx)));
+    float* const* gp = tape ? tape->gp : c->gp;
+    if (grav) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp));
+    if (c->np > 0 && part_out)
+        DH_TRY(launch_kick_drift(c, grav ? gp : nullptr, part, part_out, (float)s.K, (float)(s.dtau / c->dx)));
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
         const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
-        // gas -> tmp -> tmp2 -> gas: every sweep reads and writes each field once, no copy back; the reverse pass keeps
-        // the two intermediate states (inputs of sweeps 2 and 3) in its own buffers instead
         float* cur[5]; float* nxt[5];
         for (int k = 0; k < 5; ++k) cur[k] = gas[k];
         for (int sidx = 0; sidx < 3; ++sidx) {
-            if (sidx == 2 && !last_sweep_needed) break;
+            if (sidx == 2 && !last_sweep) break;
             const int d = order[sidx];
             for (int k = 0; k < 5; ++k)
-                nxt[k] = sidx == 2 ? gas[k] : (sweep_inputs ? sweep_inputs[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
-            DH_TRY(launch_sweep(c, d, cur, grav ? c->gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr));
+                nxt[k] = sidx == 2 ? gas_out[k] : (tape ? tape->sw[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
+            DH_TRY(launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr));
             for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
         }
+    } else if (gas_out[0] != gas[0]) {
+        for (int k = 0; k < 5; ++k)
+            DH_CUDA(cudaMemcpyAsync(gas_out[k], gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     }
     return DH_OK;
 }
 
+// The step VJP.  tape == nullptr: g' and the inputs of sweeps 2 and 3 are recomputed from the step's input state
+// into the context's scratch first; otherwise they are taken from the tape the reverse pass recorded.
 static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_in[6], const StepScalars& s, int64_t step,
                            float* const cot_gas_out[5], float* const cot_part_out[6], float* const cot_gas_in[5],
-                           float* const cot_part_in[6]) {
+                           float* const cot_part_in[6], StepTape* tape) {
     DH_TRY(ensure_adjoint_scratch(c));
     const bool grav = c->opt.gravity_on != 0;
     const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
-    // ---- recompute: g' and the inputs of sweeps 2 and 3 (the third sweep's output is not needed)
-    float* (*swin)[5] = c->sw_in;
-    DH_TRY(step_arrays(c, gas_in, part_in, s, step, nullptr, true, c->opt.hydro_on ? swin : nullptr, false));
+    StepTape local;
+    if (!tape) {
+        for (int d = 0; d < 3; ++d) local.gp[d] = c->gp[d];
+        for (int i = 0; i < 2; ++i) for (int k = 0; k < 5; ++k) local.sw[i][k] = c->sw_in[i][k];
+        DH_TRY(step_arrays(c, gas_in, part_in, gas_in, nullptr, s, step, nullptr, &local, false));
+        tape = &local;
+    }
+    float* const* gp = tape->gp;
     // ---- S4 reversed
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
@@ -146,12 +183,12 @@ static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_
         for (int k = 0; k < 5; ++k) cur[k] = cot_gas_out[k];
         for (int sidx = 2; sidx >= 0; --sidx) {
             const int d = order[sidx];
-            float* const* src = (sidx == 0) ? gas_in : swin[sidx - 1];
+            float* const* src = (sidx == 0) ? gas_in : tape->sw[sidx - 1];
             // the last adjoint sweep writes the caller's cot_gas_in; the others alternate between the two scratch sets
             if (sidx == 0) for (int k = 0; k < 5; ++k) nxt[k] = cot_gas_in[k];
             else if (sidx == 2) for (int k = 0; k < 5; ++k) nxt[k] = c->cot_tmp[k];
             else for (int k = 0; k < 5; ++k) nxt[k] = c->gas_tmp[k];
-            DH_TRY(launch_sweep_vjp(c, d, src, grav ? c->gp[d] : nullptr, lam, kap, cur, nxt, grav ? c->gpb[d] : nullptr,
+            DH_TRY(launch_sweep_vjp(c, d, src, grav ? gp[d] : nullptr, lam, kap, cur, nxt, grav ? c->gpb[d] : nullptr,
                                     c->scal_dev));
             for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
         }
@@ -163,12 +200,12 @@ static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_
     }
     // ---- S3 reversed (vector deposit adds to the g'_bar the sweeps wrote)
     if (c->np > 0) {
-        DH_TRY(launch_kick_drift_vjp(c, grav ? c->gp : nullptr, part_in, cot_part_out, cot_part_in, c->gpb, (float)s.K,
-                                     (float)(s.dtau / c->dx), c->scal_dev));
+        DH_TRY(launch_kick_drift_vjp(c, grav ? const_cast<float* const*>(gp) : nullptr, part_in, cot_part_out, cot_part_in,
+                                     c->gpb, (float)s.K, (float)(s.dtau / c->dx), c->scal_dev));
     }
     // ---- S2, S1 reversed
     if (grav) {
-        if (c->opt.want_dA) DH_TRY(launch_dot3(c, c->gpb, c->gp, 1.0 / s.A, c->scal_dev + 5));
+        if (c->opt.want_dA) DH_TRY(launch_dot3(c, c->gpb, const_cast<float* const*>(gp), 1.0 / s.A, c->scal_dev + 5));
         DH_TRY(poisson_adjoint(c, c->gpb, (float)s.A, c->delta));
         DH_TRY(launch_deposit_vjp(c, c->delta, part_in, cot_gas_in[0], cot_part_in));
     }
@@ -302,6 +339,7 @@ int dh_free(dh_ctx* c) {
     cudaFree(c->hv_state); cudaFree(c->hv_cot);
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
+    for (auto& t : c->tapes) cudaFree(t.buf);
     for (auto e : c->prof_ev) cudaEventDestroy(e);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     cudaGetLastError();
@@ -348,6 +386,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     if (!strcmp(key, "march_s_fwd")) c->tune_march_s_fwd = value;
     else if (!strcmp(key, "march_s_adj")) c->tune_march_s_adj = value;
     else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
+    else if (!strcmp(key, "tape")) c->tune_tape = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -395,7 +434,7 @@ int dh_step(dh_ctx* c, dh_state* st, double dt, double a, float* cfl_cmax_out) {
     const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
     float* cm = cfl_cmax_out ? cfl_cmax_out : c->cmax_step;
     DH_CUDA(cudaMemsetAsync(cm, 0, 3 * sizeof(float), c->stream));
-    DH_TRY(step_arrays(c, st->gas, st->part, s, st->step, cm, false, nullptr, true));
+    DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, cm, nullptr, true));
     st->a = c->cosmo.static_mode ? 1.0 : a;
     st->dt_prev = dt;
     st->step += 1;
@@ -408,7 +447,8 @@ int dh_step_vjp(dh_ctx* c, const dh_state* st, double dt, double a, const dh_cot
     DH_TRY(check_state(c, cot_out->gas, cot_out->part));
     DH_TRY(check_state(c, cot_in->gas, cot_in->part));
     const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
-    DH_TRY(step_vjp_arrays(c, st->gas, st->part, s, st->step, cot_out->gas, cot_out->part, cot_in->gas, cot_in->part));
+    DH_TRY(step_vjp_arrays(c, st->gas, st->part, s, st->step, cot_out->gas, cot_out->part, cot_in->gas, cot_in->part,
+                           nullptr));
     return harvest_scalars(c, dp);
 }
 
@@ -432,7 +472,7 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     for (int k = 0; k < n_steps; ++k) {
         if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
-        DH_TRY(step_arrays(c, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, false, nullptr, true));
+        DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true));
         st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
         st->dt_prev = dt_sched[k];
         st->step += 1;
@@ -471,6 +511,7 @@ int dh_reserve(dh_ctx* c, int n_steps, int stride) {
     for (int i = 1; i < in_seg; ++i)
         if (!c->seg[i].buf) DH_TRY(dev_alloc(c, (void**)&c->seg[i].buf, bytes));
     DH_TRY(ensure_adjoint_scratch(c));
+    ensure_tapes(c, in_seg);
     c->run_valid = false;
     return DH_OK;
 }
@@ -498,22 +539,32 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
         if (cot_initial->part[k] != cot_final->part[k])
             DH_CUDA(cudaMemcpyAsync(cot_initial->part[k], cot_final->part[k], c->np * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     if ((int)c->seg.size() < stride) c->seg.resize(stride);
+    const int in_seg = stride < n ? stride : n;
+    const bool taped = ensure_tapes(c, in_seg);
     for (int sgi = nseg - 1; sgi >= 0; --sgi) {
         const int k0 = sgi * stride, k1 = (k0 + stride < n) ? k0 + stride : n;
-        // ---- re-run the segment from its snapshot, keeping every step's input (seg[0] aliases the snapshot itself)
-        dh_state cur;
-        snapshot_view(c, c->snaps[sgi], &cur);
-        for (int k = k0; k < k1 - 1; ++k) {
-            Snapshot& nx = c->seg[k - k0 + 1];
-            DH_TRY(snapshot_store(c, nx, &cur));          // copy, then advance the copy in place
-            dh_state adv;
-            snapshot_view(c, nx, &adv);
-            const StepScalars s = step_scalars(c->cosmo, adv.a, c->run_a[k], c->run_dt[k], adv.dt_prev);
-            DH_TRY(step_arrays(c, adv.gas, adv.part, s, adv.step, nullptr, false, nullptr, true));
-            nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
-            nx.dt_prev = c->run_dt[k];
-            nx.step = adv.step + 1;
-            snapshot_view(c, nx, &cur);
+        // ---- re-run the segment from its snapshot: step k goes from seg[k - k0] (seg[0] is the snapshot itself) to
+        // seg[k - k0 + 1] out of place, so every step's input survives; with tapes each step also leaves its g' and
+        // sweep inputs behind, and the segment's last step runs only that far
+        for (int k = k0; k < k1; ++k) {
+            const bool last = (k == k1 - 1);
+            if (last && !taped) break;
+            dh_state in;
+            snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
+            const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
+            StepTape* tape = taped ? &c->tapes[k - k0] : nullptr;
+            if (last) {
+                DH_TRY(step_arrays(c, in.gas, in.part, in.gas, nullptr, s, in.step, nullptr, tape, false));
+            } else {
+                Snapshot& nx = c->seg[k - k0 + 1];
+                if (!nx.buf) DH_TRY(dev_alloc(c, (void**)&nx.buf, state_floats(c) * sizeof(float)));
+                dh_state out;
+                snapshot_view(c, nx, &out);
+                DH_TRY(step_arrays(c, in.gas, in.part, out.gas, out.part, s, in.step, nullptr, tape, true));
+                nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
+                nx.dt_prev = c->run_dt[k];
+                nx.step = in.step + 1;
+            }
         }
         // ---- step VJPs, last step of the segment first
         for (int k = k1 - 1; k >= k0; --k) {
@@ -521,7 +572,7 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
             DH_TRY(step_vjp_arrays(c, in.gas, in.part, s, in.step, cot_initial->gas, cot_initial->part, cot_initial->gas,
-                                   cot_initial->part));
+                                   cot_initial->part, taped ? &c->tapes[k - k0] : nullptr));
         }
     }
     return harvest_scalars(c, dp);
@@ -603,7 +654,7 @@ int dh_poisson_vjp(dh_ctx* c, float* const g_bar[3], double A, float* delta_bar_
 
 int dh_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], double K, double dtau_over_dx) {
     if (!c || !part) { set_error("dh_kick_drift: bad argument"); return DH_ERR_INVALID; }
-    return launch_kick_drift(c, g, part, (float)K, (float)dtau_over_dx);
+    return launch_kick_drift(c, g, part, part, (float)K, (float)dtau_over_dx);
 }
 
 }  // extern "C"

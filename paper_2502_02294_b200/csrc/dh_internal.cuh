@@ -55,6 +55,14 @@ struct Snapshot {
     int64_t step = 0;
 };
 
+// What the VJP of one step needs besides the step's input state: g' of the start-of-step state and the inputs of
+// sweeps 2 and 3.  Kept per step of a segment by the reverse pass when memory allows (13 N^3 floats), else recomputed.
+struct StepTape {
+    float* buf = nullptr;   // 13 N^3 floats: g'_x, g'_y, g'_z, sweep-2 input (5), sweep-3 input (5)
+    float* gp[3] = {nullptr, nullptr, nullptr};
+    float* sw[2][5] = {};
+};
+
 }  // namespace dh
 
 struct dh_ctx {
@@ -101,6 +109,8 @@ struct dh_ctx {
     // checkpoints of the last dh_run
     std::vector<dh::Snapshot> snaps;     // segment snapshots
     std::vector<dh::Snapshot> seg;       // per-step inputs inside one segment (reverse pass)
+    std::vector<dh::StepTape> tapes;     // per-step intermediates inside one segment (reverse pass)
+    int tune_tape = 1;                   // 0: always recompute g' and the sweep inputs in the step VJP
     std::vector<double> run_a, run_dt;
     int run_n = 0, run_stride = 0;
     double run_a0 = 0, run_dtprev0 = 0;
@@ -153,7 +163,8 @@ int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float
 int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta);
 int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]);
 int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat);
-int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float K, float dtau_dx);
+int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float* const part_out[6], float K,
+                      float dtau_dx);
 int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6], float* const cot_out[6],
                           float* const cot_in[6], float* const gbar[3], float K, float dtau_dx, double* scal_bar);
 int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6], float* rho_bar_gas,

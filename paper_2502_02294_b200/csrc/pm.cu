@@ -194,11 +194,12 @@ __device__ __forceinline__ float wrap_pos(float x, float fN) {
     return x >= fN ? x - fN : x;
 }
 
+// in -> out (the same arrays when the update is in place; one thread reads and writes only its own particle)
 __global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
-                                                         const float* __restrict__ gz, float* __restrict__ px,
-                                                         float* __restrict__ py, float* __restrict__ pz,
-                                                         float* __restrict__ wx_, float* __restrict__ wy_,
-                                                         float* __restrict__ wz_, int64_t np, int N, float K,
+                                                         const float* __restrict__ gz, const float* px, const float* py,
+                                                         const float* pz, const float* wx_, const float* wy_,
+                                                         const float* wz_, float* ox, float* oy, float* oz, float* owx,
+                                                         float* owy, float* owz, int64_t np, int N, float K,
                                                          float dtau_dx, int gravity) {
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
@@ -212,10 +213,10 @@ __global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict
         uz = fmaf(K, gather8(gz, c, N, wx, wy, wz), uz);
     }
     const float fN = (float)N;
-    px[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN);
-    py[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN);
-    pz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN);
-    wx_[p] = ux; wy_[p] = uy; wz_[p] = uz;
+    ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN);
+    oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN);
+    oz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN);
+    owx[p] = ux; owy[p] = uy; owz[p] = uz;
 }
 
 __device__ __forceinline__ void block_sum2_to_global(float a, float b, double* outa, double* outb, float* sm /*64*/) {
@@ -469,13 +470,15 @@ int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar)
     return DH_OK;
 }
 
-int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float K, float dtau_dx) {
+int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float* const part_out[6], float K,
+                      float dtau_dx) {
     if (c->np <= 0) return DH_OK;
     const int grav = c->opt.gravity_on && g && g[0];
     Prof prof(c, PROF_KICK_DRIFT);
     kick_drift_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
         grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
-        part[5], c->np, c->N, K, dtau_dx, grav);
+        part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], c->np, c->N, K, dtau_dx,
+        grav);
     c->launches++;
     DH_CUDA(cudaGetLastError());
     return DH_OK;

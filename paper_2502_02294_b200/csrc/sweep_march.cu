@@ -109,6 +109,7 @@ template <int PENDING>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
 
 constexpr int RING = 8;          // stages (power of two)
+constexpr int NTHR = 128;        // threads per block, fixed: ring offsets are immediates
 constexpr int PF_FWD = 3;        // iterations of prefetch, forward
 constexpr int PF_ADJ = 2;
 #ifndef DH_ADJ_BLOCKS
@@ -123,7 +124,8 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
     constexpr int HALO = 3, NF = HAS_G ? 6 : 5;
     extern __shared__ float ring[];              // [RING][NF][nthr]
     __shared__ int s_max;
-    const int nthr = blockDim.x * blockDim.y, tid = threadIdx.y * blockDim.x + threadIdx.x;
+    constexpr int nthr = NTHR;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
     if (tid == 0) s_max = 0;
     __syncthreads();
     const int N = sc.N;
@@ -308,7 +310,8 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
     constexpr int HALO = 4, NF = HAS_G ? 11 : 10, OB = HAS_G ? 6 : 5;
     extern __shared__ float ring[];              // [RING][NF][nthr]: u (5), g, ob (5) of one cell per stage
     __shared__ float s_red[96];
-    const int nthr = blockDim.x * blockDim.y, tid = threadIdx.y * blockDim.x + threadIdx.x;
+    constexpr int nthr = NTHR;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
     const int N = sc.N;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int o = blockIdx.y * blockDim.y + threadIdx.y;
@@ -395,12 +398,16 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
         kern<<<grid, block, sm, stream>>>(__VA_ARGS__);                                                         \
     } while (0)
 
-static dim3 march_block(int N) { return dim3(N % 128 == 0 ? 128 : (N % 64 == 0 ? 64 : 32), 1, 1); }
+// NTHR threads: as many lanes along x as divide N, the rest along the pencil index (N is a multiple of 32)
+static dim3 march_block(int N) {
+    const int bx = N % 128 == 0 ? 128 : (N % 64 == 0 ? 64 : 32);
+    return dim3(bx, NTHR / bx, 1);
+}
 
 static int march_segment(int N, int tuned, int halo) {
     // segment length: long enough that the 2*halo recomputed cells stay a small fraction, short enough that the grid
     // holds several waves of blocks on 148 SMs
-    int S = tuned > 0 ? tuned : (N >= 128 ? 64 : 32);
+    int S = tuned > 0 ? tuned : (N >= 256 ? 128 : (N >= 128 ? 64 : 32));
     if (S > N) S = N;
     if (S < 2 * halo) S = 2 * halo;
     return S;
