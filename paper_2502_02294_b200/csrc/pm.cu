@@ -64,68 +64,44 @@ __global__ void source_init_kernel(const float4* __restrict__ rho, float4* __res
     }
 }
 
-// Particles are stored in lattice order (particle p started at lattice site p) and move only a few cells over a run,
-// so a block of consecutive particles touches a compact brick of the mesh.  Each block accumulates its particles
-// into a shared-memory brick [BZ][BY][BX] anchored at the brick's first lattice site (red.shared), flushes the brick
-// with one red.global per non-zero cell, and sends the rare particle that left the brick straight to global memory.
-// Block = one PX x PY x PZ brick of lattice sites, 256 threads (see launch_deposit for the geometry).
-template <int PX, int PY, int PZ, int M>
-__global__ void __launch_bounds__(256)
-deposit_brick_kernel(const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z, int nps,
-                     int N, float mp, float cell_per_part, float* __restrict__ delta) {
-    // brick of lattice sites [PZ][PY][PX]; mesh tile with margin M cells each side (in mesh cells)
-    constexpr int TX = PX + 2 * M, TY = PY + 2 * M, TZ = PZ + 2 * M;
-    __shared__ float tile[TZ * TY * TX];
-    const int nthr = blockDim.x;
-    for (int i = threadIdx.x; i < TZ * TY * TX; i += nthr) tile[i] = 0.f;
-    __syncthreads();
-    const int nbx = (nps + PX - 1) / PX, nby = (nps + PY - 1) / PY;
-    const int bx = blockIdx.x % nbx, by = (blockIdx.x / nbx) % nby, bz = blockIdx.x / (nbx * nby);
-    // mesh cell of the brick's first lattice site (lattice site q sits at (q + 1/2) * cell_per_part)
-    const int ox = (int)floorf((bx * PX + 0.5f) * cell_per_part - 0.5f) - M;
-    const int oy = (int)floorf((by * PY + 0.5f) * cell_per_part - 0.5f) - M;
-    const int oz = (int)floorf((bz * PZ + 0.5f) * cell_per_part - 0.5f) - M;
-    for (int l = threadIdx.x; l < PX * PY * PZ; l += nthr) {
-        const int lx = l % PX, ly = (l / PX) % PY, lz = l / (PX * PY);
-        const int qx = bx * PX + lx, qy = by * PY + ly, qz = bz * PZ + lz;
-        if (qx >= nps || qy >= nps || qz >= nps) continue;
-        const int64_t p = ((int64_t)qz * nps + qy) * nps + qx;
-        const Cic c = cic_of(__ldg(x + p), __ldg(y + p), __ldg(z + p), N);
-        // tile-relative coordinates of i0 (minimum image with respect to the tile origin)
-        int rx = c.i0[0] - ox, ry = c.i0[1] - oy, rz = c.i0[2] - oz;
-        rx -= N * (int)floorf((float)rx / (float)N);
-        ry -= N * (int)floorf((float)ry / (float)N);
-        rz -= N * (int)floorf((float)rz / (float)N);
-        const bool inside = rx < TX - 1 && ry < TY - 1 && rz < TZ - 1;
-        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {mp * (1.f - c.f[2]), mp * c.f[2]};
+// Particles are stored in lattice order (particle p started at lattice site p) and neighbouring particles move
+// together, so the 32 lanes of a warp (32 consecutive lattice sites along x) deposit into a compact, mostly
+// consecutive run of cells: lane l's upper-x cell is usually lane l+1's lower-x cell.  The kernel uses that in
+// registers: every lane hands the four upper-x contributions to the next lane when the cells match (one shuffle
+// each), so a warp issues 4 coalesced RED.ADD.F32 on consecutive addresses instead of 8, and only the lanes whose
+// neighbour does not match (warp end, a particle that crossed its neighbour, a row change) issue the other 4.  The
+// reductions go straight to the mesh in L2: on B200 coalesced fp32 RED runs at > 1.4e12 adds/s, faster than any
+// shared-memory tile (fp32 shared atomics are compare-and-swap loops on sm_100), and no assumption is made about how
+// far particles have moved.
+__global__ void __launch_bounds__(256) deposit_kernel(const float* __restrict__ x, const float* __restrict__ y,
+                                                      const float* __restrict__ z, int64_t np, int N, float mp,
+                                                      float* __restrict__ delta) {
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = p < np;
+    const int lane = threadIdx.x & 31;
+    Cic c;
+    if (live) c = cic_of(__ldg(x + p), __ldg(y + p), __ldg(z + p), N);
+    else { c.i0[0] = c.i0[1] = c.i0[2] = -7; c.i1[0] = c.i1[1] = c.i1[2] = -7; c.f[0] = c.f[1] = c.f[2] = 0.f; }
+    const int row = c.i0[2] * N + c.i0[1];                 // (i0z, i0y): identifies the 2x2 group of rows touched
+    const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
+    const int i0x_next = __shfl_down_sync(0xffffffffu, c.i0[0], 1);
+    const bool pass = live && lane < 31 && row_next == row && i0x_next == c.i1[0];
+    const float wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {mp * (1.f - c.f[2]), mp * c.f[2]};
+    const float wlo = 1.f - c.f[0], whi = c.f[0];
 #pragma unroll
-        for (int cz = 0; cz < 2; ++cz)
+    for (int cz = 0; cz < 2; ++cz)
 #pragma unroll
-            for (int cy = 0; cy < 2; ++cy)
-#pragma unroll
-                for (int cx = 0; cx < 2; ++cx) {
-                    const float w = wz[cz] * wy[cy] * wx[cx];
-                    if (inside) {
-                        atomicAdd(&tile[((rz + cz) * TY + (ry + cy)) * TX + (rx + cx)], w);
-                    } else {
-                        const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
-                                             (cx ? c.i1[0] : c.i0[0]);
-                        atomicAdd(delta + cell, w);
-                    }
-                }
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < TZ * TY * TX; i += nthr) {
-        const float v = tile[i];
-        if (v != 0.f) {
-            int tx = i % TX, ty = (i / TX) % TY, tz = i / (TX * TY);
-            int gx = ox + tx, gy = oy + ty, gz = oz + tz;
-            gx -= N * (int)floorf((float)gx / (float)N);
-            gy -= N * (int)floorf((float)gy / (float)N);
-            gz -= N * (int)floorf((float)gz / (float)N);
-            atomicAdd(delta + ((int64_t)gz * N + gy) * N + gx, v);
+        for (int cy = 0; cy < 2; ++cy) {
+            const float wzy = wz[cz] * wy[cy];
+            const float up = wzy * whi;
+            const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
+            const float lo = fmaf(wzy, wlo, lane > 0 ? recv : 0.f);
+            if (live) {
+                const int64_t rowoff = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N;
+                atomicAdd(delta + rowoff + c.i0[0], lo);
+                if (!pass) atomicAdd(delta + rowoff + c.i1[0], up);
+            }
         }
-    }
 }
 
 // ----------------------------------------------------------------------------------------- Green's function ----
@@ -242,52 +218,77 @@ __device__ __forceinline__ void block_sum2_to_global(float a, float b, double* o
 // Adjoint of kick + drift + gather.  Forward: w' = w + K g_p(x); x' = wrap(x + w' dtau/dx).
 //   wt_b = w'_b + (dtau/dx) x'_b;  w_b = wt_b;  x_b = x'_b + K sum_d wt_b,d d g_p,d / dx;
 //   g'_b(cell) += W K wt_b (vector deposit);  K_b += wt_b . g_p;  (dtau/dx)_b += x'_b . w'
+// The vector deposit aggregates along x inside the warp exactly like deposit_kernel: 12 coalesced RED per warp
+// instead of 24, the rest only from lanes whose neighbour does not continue the run of cells.
 __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
     const float* __restrict__ gx, const float* __restrict__ gy, const float* __restrict__ gz,
     const float* __restrict__ px, const float* __restrict__ py, const float* __restrict__ pz,
     const float* __restrict__ wx_, const float* __restrict__ wy_, const float* __restrict__ wz_,
-    const float* __restrict__ xbo, const float* __restrict__ ybo, const float* __restrict__ zbo,
-    const float* __restrict__ wxbo, const float* __restrict__ wybo, const float* __restrict__ wzbo,
-    float* __restrict__ xbi, float* __restrict__ ybi, float* __restrict__ zbi,
-    float* __restrict__ wxbi, float* __restrict__ wybi, float* __restrict__ wzbi,
+    const float* xbo, const float* ybo, const float* zbo, const float* wxbo, const float* wybo, const float* wzbo,
+    float* xbi, float* ybi, float* zbi, float* wxbi, float* wybi, float* wzbi,
     float* __restrict__ gbx, float* __restrict__ gby, float* __restrict__ gbz,
     int64_t np, int N, float K, float dtau_dx, int gravity, double* K_b, double* dtdx_b) {
     __shared__ float sm[64];
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = p < np;
+    const int lane = threadIdx.x & 31;
     float kacc = 0.f, dacc = 0.f;
-    if (p < np) {
-        const float x = px[p], y = py[p], z = pz[p];
-        const float xb[3] = {xbo[p], ybo[p], zbo[p]};
-        float wt[3] = {fmaf(dtau_dx, xb[0], wxbo[p]), fmaf(dtau_dx, xb[1], wybo[p]), fmaf(dtau_dx, xb[2], wzbo[p])};
-        float gp[3] = {0.f, 0.f, 0.f};
-        float xo[3] = {xb[0], xb[1], xb[2]};
-        if (gravity) {
-            const Cic c = cic_of(x, y, z, N);
-            const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
-            const float dm[2] = {-1.f, 1.f};
-            const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
+    float x = 1.f, y = 1.f, z = 1.f, xb[3] = {0.f, 0.f, 0.f}, wb[3] = {0.f, 0.f, 0.f}, w0[3] = {0.f, 0.f, 0.f};
+    if (live) {
+        x = px[p]; y = py[p]; z = pz[p];
+        xb[0] = xbo[p]; xb[1] = ybo[p]; xb[2] = zbo[p];
+        wb[0] = wxbo[p]; wb[1] = wybo[p]; wb[2] = wzbo[p];
+        w0[0] = wx_[p]; w0[1] = wy_[p]; w0[2] = wz_[p];
+    }
+    const float wt[3] = {fmaf(dtau_dx, xb[0], wb[0]), fmaf(dtau_dx, xb[1], wb[1]), fmaf(dtau_dx, xb[2], wb[2])};
+    float gp[3] = {0.f, 0.f, 0.f};
+    float xo[3] = {xb[0], xb[1], xb[2]};
+    if (gravity) {                                   // uniform across the grid
+        Cic c = cic_of(x, y, z, N);
+        const int row = live ? c.i0[2] * N + c.i0[1] : -7;
+        const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
+        const int i0x_next = __shfl_down_sync(0xffffffffu, c.i0[0], 1);
+        const bool pass = live && lane < 31 && row_next == row && i0x_next == c.i1[0];
+        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
+        const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
 #pragma unroll
-            for (int cz = 0; cz < 2; ++cz)
+        for (int cz = 0; cz < 2; ++cz)
 #pragma unroll
-                for (int cy = 0; cy < 2; ++cy)
+            for (int cy = 0; cy < 2; ++cy) {
+                const int64_t rowoff = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N;
+                const float wzy = wz[cz] * wy[cy];
+                const float dzy = (cz ? 1.f : -1.f) * wy[cy], dyz = (cy ? 1.f : -1.f) * wz[cz];
+                float s_lo = 0.f, s_hi = 0.f;        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
+                if (live) {
+                    const int64_t clo = rowoff + c.i0[0], chi = rowoff + c.i1[0];
+                    const float a0 = __ldg(gx + clo), a1 = __ldg(gy + clo), a2 = __ldg(gz + clo);
+                    const float b0 = __ldg(gx + chi), b1 = __ldg(gy + chi), b2 = __ldg(gz + chi);
+                    const float wl = wzy * wx[0], wh = wzy * wx[1];
+                    gp[0] = fmaf(wl, a0, fmaf(wh, b0, gp[0]));
+                    gp[1] = fmaf(wl, a1, fmaf(wh, b1, gp[1]));
+                    gp[2] = fmaf(wl, a2, fmaf(wh, b2, gp[2]));
+                    s_lo = kw[0] * a0 + kw[1] * a1 + kw[2] * a2;
+                    s_hi = kw[0] * b0 + kw[1] * b1 + kw[2] * b2;
+                }
+                xo[0] = fmaf(wzy, s_hi - s_lo, xo[0]);
+                xo[1] = fmaf(dyz, fmaf(wx[0], s_lo, wx[1] * s_hi), xo[1]);
+                xo[2] = fmaf(dzy, fmaf(wx[0], s_lo, wx[1] * s_hi), xo[2]);
+                // vector deposit of K wt with warp aggregation along x
 #pragma unroll
-                    for (int cx = 0; cx < 2; ++cx) {
-                        const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
-                                             (cx ? c.i1[0] : c.i0[0]);
-                        const float g0 = __ldg(gx + cell), g1 = __ldg(gy + cell), g2 = __ldg(gz + cell);
-                        const float w = wz[cz] * wy[cy] * wx[cx];
-                        gp[0] = fmaf(w, g0, gp[0]); gp[1] = fmaf(w, g1, gp[1]); gp[2] = fmaf(w, g2, gp[2]);
-                        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
-                        const float s = kw[0] * g0 + kw[1] * g1 + kw[2] * g2;
-                        xo[0] = fmaf(dm[cx] * wy[cy] * wz[cz], s, xo[0]);
-                        xo[1] = fmaf(wx[cx] * dm[cy] * wz[cz], s, xo[1]);
-                        xo[2] = fmaf(wx[cx] * wy[cy] * dm[cz], s, xo[2]);
-                        atomicAdd(gbx + cell, w * kw[0]);
-                        atomicAdd(gby + cell, w * kw[1]);
-                        atomicAdd(gbz + cell, w * kw[2]);
+                for (int d = 0; d < 3; ++d) {
+                    const float up = wzy * wx[1] * kw[d];
+                    const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
+                    const float lo = fmaf(wzy * wx[0], kw[d], lane > 0 ? recv : 0.f);
+                    float* gb = d == 0 ? gbx : (d == 1 ? gby : gbz);
+                    if (live) {
+                        atomicAdd(gb + rowoff + c.i0[0], lo);
+                        if (!pass) atomicAdd(gb + rowoff + c.i1[0], up);
                     }
-        }
-        const float wn[3] = {fmaf(K, gp[0], wx_[p]), fmaf(K, gp[1], wy_[p]), fmaf(K, gp[2], wz_[p])};
+                }
+            }
+    }
+    if (live) {
+        const float wn[3] = {fmaf(K, gp[0], w0[0]), fmaf(K, gp[1], w0[1]), fmaf(K, gp[2], w0[2])};
         kacc = wt[0] * gp[0] + wt[1] * gp[1] + wt[2] * gp[2];
         dacc = xb[0] * wn[0] + xb[1] * wn[1] + xb[2] * wn[2];
         xbi[p] = xo[0]; ybi[p] = xo[1]; zbi[p] = xo[2];
@@ -406,11 +407,7 @@ int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float*
     DH_CUDA(cudaGetLastError());
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT);
-        constexpr int PX = 32, PY = 8, PZ = 8, M = 2;   // 2048 particles per block, 36x12x12 mesh brick (20 KB)
-        const int nps = c->nps;
-        const int nbx = (nps + PX - 1) / PX, nby = (nps + PY - 1) / PY, nbz = (nps + PZ - 1) / PZ;
-        deposit_brick_kernel<PX, PY, PZ, M><<<(unsigned)((int64_t)nbx * nby * nbz), 256, 0, c->stream>>>(
-            x, y, z, nps, c->N, (float)c->m_p, (float)c->N / (float)nps, delta);
+        deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, c->np, c->N, (float)c->m_p, delta);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }
