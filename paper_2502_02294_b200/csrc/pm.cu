@@ -37,6 +37,34 @@ __device__ __forceinline__ Cic cic_of(float x, float y, float z, int N) {
     return c;
 }
 
+// The 8 cells of a particle's cloud as 32-bit linear indices (N^3 <= 2^30): lo[j] / hi[j] = lower- / upper-x cell of
+// row j = 2 cz + cy, and the row weights wzy[j] = wz[cz] wy[cy].  All index arithmetic of the particle kernels is
+// 32-bit: these kernels are bound by instruction issue, not by bytes, and 64-bit address chains were half of it.
+struct Cic8 {
+    int lo[4], hi[4];
+    float wzy[4], wx0, wx1;
+    int i0x, i1x, row;     // row = i0z N + i0y identifies the 2x2 group of rows
+    float fy, fz;
+};
+
+__device__ __forceinline__ Cic8 cic8_of(float x, float y, float z, int N) {
+    Cic8 q;
+    int i0y, i1y, i0z, i1z;
+    float fx;
+    cic_axis(x, N, q.i0x, q.i1x, fx);
+    cic_axis(y, N, i0y, i1y, q.fy);
+    cic_axis(z, N, i0z, i1z, q.fz);
+    const int z0 = i0z * N, z1 = i1z * N;
+    q.row = z0 + i0y;
+    const int r[4] = {(z0 + i0y) * N, (z0 + i1y) * N, (z1 + i0y) * N, (z1 + i1y) * N};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { q.lo[j] = r[j] + q.i0x; q.hi[j] = r[j] + q.i1x; }
+    q.wx0 = 1.f - fx; q.wx1 = fx;
+    const float wy0 = 1.f - q.fy, wz0 = 1.f - q.fz;
+    q.wzy[0] = wz0 * wy0; q.wzy[1] = wz0 * q.fy; q.wzy[2] = q.fz * wy0; q.wzy[3] = q.fz * q.fy;
+    return q;
+}
+
 __global__ void cell_index_kernel(const float* __restrict__ x, int64_t n, int N, int32_t* i0, int32_t* i1) {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
@@ -74,34 +102,27 @@ __global__ void source_init_kernel(const float4* __restrict__ rho, float4* __res
 // shared-memory tile (fp32 shared atomics are compare-and-swap loops on sm_100), and no assumption is made about how
 // far particles have moved.
 __global__ void __launch_bounds__(256) deposit_kernel(const float* __restrict__ x, const float* __restrict__ y,
-                                                      const float* __restrict__ z, int64_t np, int N, float mp,
+                                                      const float* __restrict__ z, int np, int N, float mp,
                                                       float* __restrict__ delta) {
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = p < np;
     const int lane = threadIdx.x & 31;
-    Cic c;
-    if (live) c = cic_of(__ldg(x + p), __ldg(y + p), __ldg(z + p), N);
-    else { c.i0[0] = c.i0[1] = c.i0[2] = -7; c.i1[0] = c.i1[1] = c.i1[2] = -7; c.f[0] = c.f[1] = c.f[2] = 0.f; }
-    const int row = c.i0[2] * N + c.i0[1];                 // (i0z, i0y): identifies the 2x2 group of rows touched
+    Cic8 q = cic8_of(live ? __ldg(x + p) : 1.f, live ? __ldg(y + p) : 1.f, live ? __ldg(z + p) : 1.f, N);
+    const int row = live ? q.row : -7;
     const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
-    const int i0x_next = __shfl_down_sync(0xffffffffu, c.i0[0], 1);
-    const bool pass = live && lane < 31 && row_next == row && i0x_next == c.i1[0];
-    const float wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {mp * (1.f - c.f[2]), mp * c.f[2]};
-    const float wlo = 1.f - c.f[0], whi = c.f[0];
+    const int i0x_next = __shfl_down_sync(0xffffffffu, q.i0x, 1);
+    const bool pass = live && lane < 31 && row_next == row && i0x_next == q.i1x;
+    const float wlo = mp * q.wx0, whi = mp * q.wx1;
 #pragma unroll
-    for (int cz = 0; cz < 2; ++cz)
-#pragma unroll
-        for (int cy = 0; cy < 2; ++cy) {
-            const float wzy = wz[cz] * wy[cy];
-            const float up = wzy * whi;
-            const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
-            const float lo = fmaf(wzy, wlo, lane > 0 ? recv : 0.f);
-            if (live) {
-                const int64_t rowoff = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N;
-                atomicAdd(delta + rowoff + c.i0[0], lo);
-                if (!pass) atomicAdd(delta + rowoff + c.i1[0], up);
-            }
+    for (int j = 0; j < 4; ++j) {
+        const float up = q.wzy[j] * whi;
+        const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
+        const float lo = fmaf(q.wzy[j], wlo, lane > 0 ? recv : 0.f);
+        if (live) {
+            atomicAdd(delta + q.lo[j], lo);
+            if (!pass) atomicAdd(delta + q.hi[j], up);
         }
+    }
 }
 
 // ----------------------------------------------------------------------------------------- Green's function ----
@@ -147,26 +168,22 @@ __global__ void __launch_bounds__(256) green_adj_kernel(const float2* __restrict
 }
 
 // ------------------------------------------------------------------------------------------- gather helpers ----
-__device__ __forceinline__ float gather8(const float* __restrict__ m, const Cic& c, int N, const float (&wx)[2],
-                                         const float (&wy)[2], const float (&wz)[2]) {
+__device__ __forceinline__ float gather8(const float* __restrict__ m, const Cic8& q) {
     float acc = 0.f;
 #pragma unroll
-    for (int cz = 0; cz < 2; ++cz) {
-        const int64_t bz = (int64_t)(cz ? c.i1[2] : c.i0[2]) * N;
-#pragma unroll
-        for (int cy = 0; cy < 2; ++cy) {
-            const int64_t row = (bz + (cy ? c.i1[1] : c.i0[1])) * N;
-            const float wzy = wz[cz] * wy[cy];
-            acc = fmaf(wzy * wx[0], __ldg(m + row + c.i0[0]), acc);
-            acc = fmaf(wzy * wx[1], __ldg(m + row + c.i1[0]), acc);
-        }
+    for (int j = 0; j < 4; ++j) {
+        const float row = fmaf(q.wx0, __ldg(m + q.lo[j]), q.wx1 * __ldg(m + q.hi[j]));
+        acc = fmaf(q.wzy[j], row, acc);
     }
     return acc;
 }
 
 // ---------------------------------------------------------------------------------------------- kick + drift ----
-__device__ __forceinline__ float wrap_pos(float x, float fN) {
-    x -= fN * floorf(x / fN);
+// x mod N into [0, N) without a division: the reciprocal form can be one period off next to a multiple of N, which the
+// two corrections absorb (any finite x).
+__device__ __forceinline__ float wrap_pos(float x, float fN, float invN) {
+    x = fmaf(-fN, floorf(x * invN), x);
+    x = x < 0.f ? x + fN : x;
     return x >= fN ? x - fN : x;
 }
 
@@ -175,23 +192,21 @@ __global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict
                                                          const float* __restrict__ gz, const float* px, const float* py,
                                                          const float* pz, const float* wx_, const float* wy_,
                                                          const float* wz_, float* ox, float* oy, float* oz, float* owx,
-                                                         float* owy, float* owz, int64_t np, int N, float K,
-                                                         float dtau_dx, int gravity) {
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+                                                         float* owy, float* owz, int np, int N, float K,
+                                                         float dtau_dx, float fN, float invN, int gravity) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    float x = px[p], y = py[p], z = pz[p];
+    const float x = px[p], y = py[p], z = pz[p];
     float ux = wx_[p], uy = wy_[p], uz = wz_[p];
     if (gravity) {
-        const Cic c = cic_of(x, y, z, N);
-        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
-        ux = fmaf(K, gather8(gx, c, N, wx, wy, wz), ux);
-        uy = fmaf(K, gather8(gy, c, N, wx, wy, wz), uy);
-        uz = fmaf(K, gather8(gz, c, N, wx, wy, wz), uz);
+        const Cic8 q = cic8_of(x, y, z, N);
+        ux = fmaf(K, gather8(gx, q), ux);
+        uy = fmaf(K, gather8(gy, q), uy);
+        uz = fmaf(K, gather8(gz, q), uz);
     }
-    const float fN = (float)N;
-    ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN);
-    oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN);
-    oz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN);
+    ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN, invN);
+    oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN, invN);
+    oz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN, invN);
     owx[p] = ux; owy[p] = uy; owz[p] = uz;
 }
 
@@ -227,9 +242,9 @@ __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
     const float* xbo, const float* ybo, const float* zbo, const float* wxbo, const float* wybo, const float* wzbo,
     float* xbi, float* ybi, float* zbi, float* wxbi, float* wybi, float* wzbi,
     float* __restrict__ gbx, float* __restrict__ gby, float* __restrict__ gbz,
-    int64_t np, int N, float K, float dtau_dx, int gravity, double* K_b, double* dtdx_b) {
+    int np, int N, float K, float dtau_dx, int gravity, double* K_b, double* dtdx_b) {
     __shared__ float sm[64];
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = p < np;
     const int lane = threadIdx.x & 31;
     float kacc = 0.f, dacc = 0.f;
@@ -244,48 +259,46 @@ __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
     float gp[3] = {0.f, 0.f, 0.f};
     float xo[3] = {xb[0], xb[1], xb[2]};
     if (gravity) {                                   // uniform across the grid
-        Cic c = cic_of(x, y, z, N);
-        const int row = live ? c.i0[2] * N + c.i0[1] : -7;
+        const Cic8 q = cic8_of(x, y, z, N);
+        const int row = live ? q.row : -7;
         const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
-        const int i0x_next = __shfl_down_sync(0xffffffffu, c.i0[0], 1);
-        const bool pass = live && lane < 31 && row_next == row && i0x_next == c.i1[0];
-        const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
+        const int i0x_next = __shfl_down_sync(0xffffffffu, q.i0x, 1);
+        const bool pass = live && lane < 31 && row_next == row && i0x_next == q.i1x;
         const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
+        const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
 #pragma unroll
-        for (int cz = 0; cz < 2; ++cz)
+        for (int j = 0; j < 4; ++j) {
+            const int cz = j >> 1, cy = j & 1;
+            const float wzy = q.wzy[j];
+            const float dzy = (cz ? 1.f : -1.f) * wy[cy], dyz = (cy ? 1.f : -1.f) * wz[cz];
+            float s_lo = 0.f, s_hi = 0.f;        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
+            if (live) {
+                const float a0 = __ldg(gx + q.lo[j]), a1 = __ldg(gy + q.lo[j]), a2 = __ldg(gz + q.lo[j]);
+                const float b0 = __ldg(gx + q.hi[j]), b1 = __ldg(gy + q.hi[j]), b2 = __ldg(gz + q.hi[j]);
+                const float wl = wzy * q.wx0, wh = wzy * q.wx1;
+                gp[0] = fmaf(wl, a0, fmaf(wh, b0, gp[0]));
+                gp[1] = fmaf(wl, a1, fmaf(wh, b1, gp[1]));
+                gp[2] = fmaf(wl, a2, fmaf(wh, b2, gp[2]));
+                s_lo = kw[0] * a0 + kw[1] * a1 + kw[2] * a2;
+                s_hi = kw[0] * b0 + kw[1] * b1 + kw[2] * b2;
+            }
+            const float s_x = fmaf(q.wx0, s_lo, q.wx1 * s_hi);
+            xo[0] = fmaf(wzy, s_hi - s_lo, xo[0]);
+            xo[1] = fmaf(dyz, s_x, xo[1]);
+            xo[2] = fmaf(dzy, s_x, xo[2]);
+            // vector deposit of K wt with warp aggregation along x
 #pragma unroll
-            for (int cy = 0; cy < 2; ++cy) {
-                const int64_t rowoff = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N;
-                const float wzy = wz[cz] * wy[cy];
-                const float dzy = (cz ? 1.f : -1.f) * wy[cy], dyz = (cy ? 1.f : -1.f) * wz[cz];
-                float s_lo = 0.f, s_hi = 0.f;        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
+            for (int d = 0; d < 3; ++d) {
+                const float up = wzy * q.wx1 * kw[d];
+                const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
+                const float lo = fmaf(wzy * q.wx0, kw[d], lane > 0 ? recv : 0.f);
+                float* gb = d == 0 ? gbx : (d == 1 ? gby : gbz);
                 if (live) {
-                    const int64_t clo = rowoff + c.i0[0], chi = rowoff + c.i1[0];
-                    const float a0 = __ldg(gx + clo), a1 = __ldg(gy + clo), a2 = __ldg(gz + clo);
-                    const float b0 = __ldg(gx + chi), b1 = __ldg(gy + chi), b2 = __ldg(gz + chi);
-                    const float wl = wzy * wx[0], wh = wzy * wx[1];
-                    gp[0] = fmaf(wl, a0, fmaf(wh, b0, gp[0]));
-                    gp[1] = fmaf(wl, a1, fmaf(wh, b1, gp[1]));
-                    gp[2] = fmaf(wl, a2, fmaf(wh, b2, gp[2]));
-                    s_lo = kw[0] * a0 + kw[1] * a1 + kw[2] * a2;
-                    s_hi = kw[0] * b0 + kw[1] * b1 + kw[2] * b2;
-                }
-                xo[0] = fmaf(wzy, s_hi - s_lo, xo[0]);
-                xo[1] = fmaf(dyz, fmaf(wx[0], s_lo, wx[1] * s_hi), xo[1]);
-                xo[2] = fmaf(dzy, fmaf(wx[0], s_lo, wx[1] * s_hi), xo[2]);
-                // vector deposit of K wt with warp aggregation along x
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    const float up = wzy * wx[1] * kw[d];
-                    const float recv = __shfl_up_sync(0xffffffffu, pass ? up : 0.f, 1);
-                    const float lo = fmaf(wzy * wx[0], kw[d], lane > 0 ? recv : 0.f);
-                    float* gb = d == 0 ? gbx : (d == 1 ? gby : gbz);
-                    if (live) {
-                        atomicAdd(gb + rowoff + c.i0[0], lo);
-                        if (!pass) atomicAdd(gb + rowoff + c.i1[0], up);
-                    }
+                    atomicAdd(gb + q.lo[j], lo);
+                    if (!pass) atomicAdd(gb + q.hi[j], up);
                 }
             }
+        }
     }
     if (live) {
         const float wn[3] = {fmaf(K, gp[0], w0[0]), fmaf(K, gp[1], w0[1]), fmaf(K, gp[2], w0[2])};
@@ -301,26 +314,21 @@ __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
 __global__ void __launch_bounds__(256) deposit_adj_kernel(const float* __restrict__ db, const float* __restrict__ px,
                                                           const float* __restrict__ py, const float* __restrict__ pz,
                                                           float* __restrict__ xb, float* __restrict__ yb,
-                                                          float* __restrict__ zb, int64_t np, int N, float mp) {
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+                                                          float* __restrict__ zb, int np, int N, float mp) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
-    const Cic c = cic_of(px[p], py[p], pz[p], N);
-    const float wx[2] = {1.f - c.f[0], c.f[0]}, wy[2] = {1.f - c.f[1], c.f[1]}, wz[2] = {1.f - c.f[2], c.f[2]};
-    const float dm[2] = {-1.f, 1.f};
+    const Cic8 q = cic8_of(px[p], py[p], pz[p], N);
+    const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
     float a0 = 0.f, a1 = 0.f, a2 = 0.f;
 #pragma unroll
-    for (int cz = 0; cz < 2; ++cz)
-#pragma unroll
-        for (int cy = 0; cy < 2; ++cy)
-#pragma unroll
-            for (int cx = 0; cx < 2; ++cx) {
-                const int64_t cell = ((int64_t)(cz ? c.i1[2] : c.i0[2]) * N + (cy ? c.i1[1] : c.i0[1])) * N +
-                                     (cx ? c.i1[0] : c.i0[0]);
-                const float v = __ldg(db + cell);
-                a0 = fmaf(dm[cx] * wy[cy] * wz[cz], v, a0);
-                a1 = fmaf(wx[cx] * dm[cy] * wz[cz], v, a1);
-                a2 = fmaf(wx[cx] * wy[cy] * dm[cz], v, a2);
-            }
+    for (int j = 0; j < 4; ++j) {
+        const int cz = j >> 1, cy = j & 1;
+        const float vlo = __ldg(db + q.lo[j]), vhi = __ldg(db + q.hi[j]);
+        const float vx = fmaf(q.wx0, vlo, q.wx1 * vhi);
+        a0 = fmaf(q.wzy[j], vhi - vlo, a0);
+        a1 = fmaf((cy ? 1.f : -1.f) * wz[cz], vx, a1);
+        a2 = fmaf((cz ? 1.f : -1.f) * wy[cy], vx, a2);
+    }
     xb[p] = fmaf(mp, a0, xb[p]);
     yb[p] = fmaf(mp, a1, yb[p]);
     zb[p] = fmaf(mp, a2, zb[p]);
@@ -407,7 +415,7 @@ int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float*
     DH_CUDA(cudaGetLastError());
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT);
-        deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, c->np, c->N, (float)c->m_p, delta);
+        deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, (int)c->np, c->N, (float)c->m_p, delta);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }
@@ -474,8 +482,8 @@ int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float*
     Prof prof(c, PROF_KICK_DRIFT);
     kick_drift_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
         grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
-        part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], c->np, c->N, K, dtau_dx,
-        grav);
+        part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
+        dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
     c->launches++;
     DH_CUDA(cudaGetLastError());
     return DH_OK;
@@ -490,7 +498,7 @@ int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6],
         grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part_in[0], part_in[1], part_in[2],
         part_in[3], part_in[4], part_in[5], cot_out[0], cot_out[1], cot_out[2], cot_out[3], cot_out[4], cot_out[5],
         cot_in[0], cot_in[1], cot_in[2], cot_in[3], cot_in[4], cot_in[5], grav ? gbar[0] : nullptr,
-        grav ? gbar[1] : nullptr, grav ? gbar[2] : nullptr, c->np, c->N, K, dtau_dx, grav, scal_bar + 3, scal_bar + 4);
+        grav ? gbar[1] : nullptr, grav ? gbar[2] : nullptr, (int)c->np, c->N, K, dtau_dx, grav, scal_bar + 3, scal_bar + 4);
     c->launches++;
     DH_CUDA(cudaGetLastError());
     return DH_OK;
@@ -509,7 +517,7 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT_ADJ);
         deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
-            delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], c->np, c->N, (float)c->m_p);
+            delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }

@@ -338,7 +338,9 @@ def test_run_host_variant_matches_device_variant(api, torch_, W):
     hg = torch_.from_numpy(gas.copy()).pin_memory(); hp = torch_.from_numpy(part.copy()).pin_memory()
     a, dtp, st = ctx.dh_run_host(hg, hp, cfg.a0, 0.0, 0, a_s[1:], dt_s, 2)
     assert st == 4 and abs(a - cfg.a1) < 1e-15
-    assert PT.max_rel(hg.numpy(), sg.gas.cpu().numpy()) < 1e-6          # atomics order may differ in the last bit
+    # two GPU runs of the same code: the deposit's fp32 RED order differs, i.e. last-bit differences in delta_tot per
+    # step (4 steps here); this is a run-to-run consistency bound, not an oracle tolerance
+    assert PT.max_rel(hg.numpy(), sg.gas.cpu().numpy()) < 5e-6
     cg = np.zeros_like(gas); cg[0] = 1.0
     hcg = torch_.from_numpy(cg).pin_memory(); hcp = torch_.zeros(part.shape).pin_memory()
     dp = ctx.dh_run_vjp_host(hcg, hcp)
