@@ -158,7 +158,9 @@ int dh_sync(dh_ctx* ctx);
  *   "yz_chain": 1 routes the y/z sweeps through the shared-memory chain kernels the x sweep uses;
  *   "tape": 0 makes dh_run_vjp recompute g' and the sweep inputs inside every step VJP instead of keeping them for
  *           the steps of the segment being reversed (13 N^3 floats per step of a segment; default 1, falls back to
- *           recomputation by itself when the device cannot hold them).
+ *           recomputation by itself when the device cannot hold them);
+ *   "gstore": 0 makes a checkpointed dh_run NOT keep every step's g' (3 N^3 floats per step of the run) for
+ *           dh_run_vjp, which then repeats deposit + Poisson solve in the segment re-run (default 1, same fallback).
  * Unknown key: DH_ERR_INVALID. */
 int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of

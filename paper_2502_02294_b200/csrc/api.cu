@@ -115,6 +115,27 @@ static bool ensure_tapes(dh_ctx* c, int in_seg) {
     return true;
 }
 
+// Per-step store of g' for a checkpointed run (3 N^3 floats per step): the forward pass writes each step's g' there
+// instead of into scratch, so neither the segment re-run nor the step VJP repeats the deposit and the Poisson solve.
+// All or nothing, like the tapes: when the device cannot hold n_steps of them the reverse pass recomputes g'.
+static bool ensure_gstore(dh_ctx* c, int n_steps) {
+    if (!c->tune_gstore || !c->opt.gravity_on) return false;
+    const size_t bytes = (size_t)3 * c->n3 * sizeof(float);
+    if ((int)c->gstore.size() < n_steps) c->gstore.resize(n_steps);
+    for (int i = 0; i < n_steps; ++i) {
+        GravStore& g = c->gstore[i];
+        if (g.buf) continue;
+        if (dev_alloc(c, (void**)&g.buf, bytes) != DH_OK) {
+            for (auto& t : c->gstore) { dev_free(c, t.buf, bytes); t.buf = nullptr; }
+            c->gstore.clear();
+            set_error("");
+            return false;
+        }
+        for (int d = 0; d < 3; ++d) g.gp[d] = g.buf + (size_t)d * c->n3;
+    }
+    return true;
+}
+
 static void free_snaps(dh_ctx* c, std::vector<Snapshot>& v) {
     for (auto& s : v) dev_free(c, s.buf, state_floats(c) * sizeof(float));
     v.clear();
@@ -130,14 +151,15 @@ static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6],
 // The forward step from (gas, part) to (gas_out, part_out); out may alias in (in-place update: the sweeps go
 // gas -> A -> B -> gas_out, every field read and written once per sweep, no copy).  With a tape, g' and the two
 // intermediate gas states A, B are written into it (and survive the step); otherwise they live in the context's
-// scratch.  part_out == nullptr skips the particle update, last_sweep == false stops after sweep 2 (the reverse pass
+// scratch.  gp_keep: where g' of this step goes (the run's per-step g' store); gp_ready: it already holds g' of this
+// step, so deposit and Poisson solve are skipped.  part_out == nullptr skips the particle update, last_sweep == false stops after sweep 2 (the reverse pass
 // needs nothing more of a segment's last step).
 static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], float* const gas_out[5],
                        float* const part_out[6], const StepScalars& s, int64_t step, float* cmax3, StepTape* tape,
-                       bool last_sweep) {
+                       bool last_sweep, float* const* gp_keep = nullptr, bool gp_ready = false) {
     const bool grav = c->opt.gravity_on != 0;
-    float* const* gp = tape ? tape->gp : c->gp;
-    if (grav) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp));
+    float* const* gp = gp_keep ? gp_keep : (tape ? tape->gp : c->gp);
+    if (grav && !gp_ready) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp));
     if (c->np > 0 && part_out)
         DH_TRY(launch_kick_drift(c, grav ? gp : nullptr, part, part_out, (float)s.K, (float)(s.dtau / c->dx)));
     if (c->opt.hydro_on) {
@@ -164,7 +186,7 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
 // into the context's scratch first; otherwise they are taken from the tape the reverse pass recorded.
 static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_in[6], const StepScalars& s, int64_t step,
                            float* const cot_gas_out[5], float* const cot_part_out[6], float* const cot_gas_in[5],
-                           float* const cot_part_in[6], StepTape* tape) {
+                           float* const cot_part_in[6], StepTape* tape, float* const* gp_kept = nullptr) {
     DH_TRY(ensure_adjoint_scratch(c));
     const bool grav = c->opt.gravity_on != 0;
     const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
@@ -172,10 +194,10 @@ static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_
     if (!tape) {
         for (int d = 0; d < 3; ++d) local.gp[d] = c->gp[d];
         for (int i = 0; i < 2; ++i) for (int k = 0; k < 5; ++k) local.sw[i][k] = c->sw_in[i][k];
-        DH_TRY(step_arrays(c, gas_in, part_in, gas_in, nullptr, s, step, nullptr, &local, false));
+        DH_TRY(step_arrays(c, gas_in, part_in, gas_in, nullptr, s, step, nullptr, &local, false, gp_kept, gp_kept != nullptr));
         tape = &local;
     }
-    float* const* gp = tape->gp;
+    float* const* gp = gp_kept ? gp_kept : tape->gp;
     // ---- S4 reversed
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
@@ -340,6 +362,7 @@ int dh_free(dh_ctx* c) {
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
     for (auto& t : c->tapes) cudaFree(t.buf);
+    for (auto& t : c->gstore) cudaFree(t.buf);
     for (auto e : c->prof_ev) cudaEventDestroy(e);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     cudaGetLastError();
@@ -387,6 +410,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "march_s_adj")) c->tune_march_s_adj = value;
     else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
     else if (!strcmp(key, "tape")) c->tune_tape = value;
+    else if (!strcmp(key, "gstore")) c->tune_gstore = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -469,10 +493,12 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     c->run_a.assign(a_sched, a_sched + n_steps);
     c->run_dt.assign(dt_sched, dt_sched + n_steps);
     c->run_n = n_steps; c->run_stride = stride;
+    c->run_gstore = stride > 0 && ensure_gstore(c, n_steps);
     for (int k = 0; k < n_steps; ++k) {
         if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
-        DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true));
+        DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
+                           c->run_gstore ? c->gstore[k].gp : nullptr, false));
         st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
         st->dt_prev = dt_sched[k];
         st->step += 1;
@@ -512,6 +538,7 @@ int dh_reserve(dh_ctx* c, int n_steps, int stride) {
         if (!c->seg[i].buf) DH_TRY(dev_alloc(c, (void**)&c->seg[i].buf, bytes));
     DH_TRY(ensure_adjoint_scratch(c));
     ensure_tapes(c, in_seg);
+    ensure_gstore(c, n_steps);
     c->run_valid = false;
     return DH_OK;
 }
@@ -553,14 +580,15 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
             StepTape* tape = taped ? &c->tapes[k - k0] : nullptr;
+            float* const* gk = c->run_gstore ? c->gstore[k].gp : nullptr;
             if (last) {
-                DH_TRY(step_arrays(c, in.gas, in.part, in.gas, nullptr, s, in.step, nullptr, tape, false));
+                DH_TRY(step_arrays(c, in.gas, in.part, in.gas, nullptr, s, in.step, nullptr, tape, false, gk, gk != nullptr));
             } else {
                 Snapshot& nx = c->seg[k - k0 + 1];
                 if (!nx.buf) DH_TRY(dev_alloc(c, (void**)&nx.buf, state_floats(c) * sizeof(float)));
                 dh_state out;
                 snapshot_view(c, nx, &out);
-                DH_TRY(step_arrays(c, in.gas, in.part, out.gas, out.part, s, in.step, nullptr, tape, true));
+                DH_TRY(step_arrays(c, in.gas, in.part, out.gas, out.part, s, in.step, nullptr, tape, true, gk, gk != nullptr));
                 nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
                 nx.dt_prev = c->run_dt[k];
                 nx.step = in.step + 1;
@@ -572,7 +600,8 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
             DH_TRY(step_vjp_arrays(c, in.gas, in.part, s, in.step, cot_initial->gas, cot_initial->part, cot_initial->gas,
-                                   cot_initial->part, taped ? &c->tapes[k - k0] : nullptr));
+                                   cot_initial->part, taped ? &c->tapes[k - k0] : nullptr,
+                                   c->run_gstore ? c->gstore[k].gp : nullptr));
         }
     }
     return harvest_scalars(c, dp);

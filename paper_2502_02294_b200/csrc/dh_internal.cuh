@@ -63,6 +63,12 @@ struct StepTape {
     float* sw[2][5] = {};
 };
 
+// g' of one step of a checkpointed run, kept from the forward pass for the reverse pass.
+struct GravStore {
+    float* buf = nullptr;   // 3 N^3 floats
+    float* gp[3] = {nullptr, nullptr, nullptr};
+};
+
 }  // namespace dh
 
 struct dh_ctx {
@@ -111,6 +117,9 @@ struct dh_ctx {
     std::vector<dh::Snapshot> seg;       // per-step inputs inside one segment (reverse pass)
     std::vector<dh::StepTape> tapes;     // per-step intermediates inside one segment (reverse pass)
     int tune_tape = 1;                   // 0: always recompute g' and the sweep inputs in the step VJP
+    std::vector<dh::GravStore> gstore;   // per-step g' of the last checkpointed dh_run
+    int tune_gstore = 1;                 // 0: never keep g' from the forward pass
+    bool run_gstore = false;             // the last dh_run filled gstore[0 .. run_n)
     std::vector<double> run_a, run_dt;
     int run_n = 0, run_stride = 0;
     double run_a0 = 0, run_dtprev0 = 0;

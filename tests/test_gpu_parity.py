@@ -328,6 +328,32 @@ def test_config0_gradient_of_final_density_norm(api, torch_, O, W):
     ctx.close()
 
 
+def test_reverse_pass_storage_policies_agree(api, torch_, W):
+    """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
+    ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
+    policies differ by the order of the deposit's fp32 atomics in the recomputed g' (last-bit), nothing more."""
+    cfg = W.scaled_config(0, 32, n_steps=7, a1=0.03)
+    delta, gas, part = W.coupled_ic(cfg)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    out = []
+    for tape, gstore in ((1, 1), (0, 1), (1, 0), (0, 0)):
+        ctx = api.context_for(cfg)
+        ctx.dh_tune("tape", tape); ctx.dh_tune("gstore", gstore)
+        sg = api.State(gas, part, cfg.a0)
+        ctx.dh_run(sg, a_s[1:], dt_s, 3)
+        cg = torch_.zeros_like(sg.gas); cg[0] = sg.gas[0]
+        ct = api.Cot(cg, torch_.zeros_like(sg.part))
+        dp = ctx.dh_run_vjp(ct, ct)
+        out.append((ct.gas.cpu().numpy(), ct.part.cpu().numpy(), dp.dgamma, ctx.dh_launch_count()))
+        ctx.close()
+    g0, p0, dg0, n0 = out[0]
+    for g, p_, dg, n in out[1:]:
+        # same bound as "gradient independent of checkpoint_stride" (DESIGN.md reading R28)
+        assert PT.rel_l2(g, g0) < TOL_GRAD and PT.rel_l2(p_, p0) < TOL_GRAD and abs(dg / dg0 - 1) < 1e-4
+    # keeping g' removes deposit + Poisson from the segment re-run: fewer launches than recomputing it
+    assert out[0][3] < out[2][3] and out[1][3] < out[3][3]
+
+
 def test_run_host_variant_matches_device_variant(api, torch_, W):
     cfg = W.scaled_config(0, 32, n_steps=4, a1=0.02)
     delta, gas, part = W.coupled_ic(cfg)
