@@ -168,13 +168,18 @@ __global__ void __launch_bounds__(256) green_adj_kernel(const float2* __restrict
 }
 
 // ------------------------------------------------------------------------------------------- gather helpers ----
-__device__ __forceinline__ float gather8(const float* __restrict__ m, const Cic8& q) {
+// The 8 cloud values of every mesh a kernel gathers from are loaded in one batch (all loads issued before the first
+// use) and reduced afterwards: one memory round trip per kernel phase instead of one per cloud row.  ptxas only keeps
+// the batch together when the kernel's launch bounds allow it more than 32 registers (minimum blocks per SM given).
+struct Gath8 { float lo[4], hi[4]; };
+__device__ __forceinline__ void gather_issue(const float* __restrict__ m, const Cic8& q, Gath8& v) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { v.lo[j] = __ldg(m + q.lo[j]); v.hi[j] = __ldg(m + q.hi[j]); }
+}
+__device__ __forceinline__ float gather_reduce(const Gath8& v, const Cic8& q) {
     float acc = 0.f;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const float row = fmaf(q.wx0, __ldg(m + q.lo[j]), q.wx1 * __ldg(m + q.hi[j]));
-        acc = fmaf(q.wzy[j], row, acc);
-    }
+    for (int j = 0; j < 4; ++j) acc = fmaf(q.wzy[j], fmaf(q.wx0, v.lo[j], q.wx1 * v.hi[j]), acc);
     return acc;
 }
 
@@ -188,7 +193,7 @@ __device__ __forceinline__ float wrap_pos(float x, float fN, float invN) {
 }
 
 // in -> out (the same arrays when the update is in place; one thread reads and writes only its own particle)
-__global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
+__global__ void __launch_bounds__(256, 3) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
                                                          const float* __restrict__ gz, const float* px, const float* py,
                                                          const float* pz, const float* wx_, const float* wy_,
                                                          const float* wz_, float* ox, float* oy, float* oz, float* owx,
@@ -200,9 +205,11 @@ __global__ void __launch_bounds__(256) kick_drift_kernel(const float* __restrict
     float ux = wx_[p], uy = wy_[p], uz = wz_[p];
     if (gravity) {
         const Cic8 q = cic8_of(x, y, z, N);
-        ux = fmaf(K, gather8(gx, q), ux);
-        uy = fmaf(K, gather8(gy, q), uy);
-        uz = fmaf(K, gather8(gz, q), uz);
+        Gath8 a, b, c;
+        gather_issue(gx, q, a); gather_issue(gy, q, b); gather_issue(gz, q, c);
+        ux = fmaf(K, gather_reduce(a, q), ux);
+        uy = fmaf(K, gather_reduce(b, q), uy);
+        uz = fmaf(K, gather_reduce(c, q), uz);
     }
     ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN, invN);
     oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN, invN);
@@ -266,6 +273,8 @@ __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
         const bool pass = live && lane < 31 && row_next == row && i0x_next == q.i1x;
         const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
         const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
+        Gath8 vx, vy, vz;
+        if (live) { gather_issue(gx, q, vx); gather_issue(gy, q, vy); gather_issue(gz, q, vz); }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int cz = j >> 1, cy = j & 1;
@@ -273,8 +282,8 @@ __global__ void __launch_bounds__(256) kick_drift_adj_kernel(
             const float dzy = (cz ? 1.f : -1.f) * wy[cy], dyz = (cy ? 1.f : -1.f) * wz[cz];
             float s_lo = 0.f, s_hi = 0.f;        // sum_d K wt_d g_d(cell): what the weight derivatives multiply
             if (live) {
-                const float a0 = __ldg(gx + q.lo[j]), a1 = __ldg(gy + q.lo[j]), a2 = __ldg(gz + q.lo[j]);
-                const float b0 = __ldg(gx + q.hi[j]), b1 = __ldg(gy + q.hi[j]), b2 = __ldg(gz + q.hi[j]);
+                const float a0 = vx.lo[j], a1 = vy.lo[j], a2 = vz.lo[j];
+                const float b0 = vx.hi[j], b1 = vy.hi[j], b2 = vz.hi[j];
                 const float wl = wzy * q.wx0, wh = wzy * q.wx1;
                 gp[0] = fmaf(wl, a0, fmaf(wh, b0, gp[0]));
                 gp[1] = fmaf(wl, a1, fmaf(wh, b1, gp[1]));
@@ -320,18 +329,21 @@ __global__ void __launch_bounds__(256) deposit_adj_kernel(const float* __restric
     const Cic8 q = cic8_of(px[p], py[p], pz[p], N);
     const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
     float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+    Gath8 v;
+    gather_issue(db, q, v);
+    const float xb0 = xb[p], yb0 = yb[p], zb0 = zb[p];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int cz = j >> 1, cy = j & 1;
-        const float vlo = __ldg(db + q.lo[j]), vhi = __ldg(db + q.hi[j]);
+        const float vlo = v.lo[j], vhi = v.hi[j];
         const float vx = fmaf(q.wx0, vlo, q.wx1 * vhi);
         a0 = fmaf(q.wzy[j], vhi - vlo, a0);
         a1 = fmaf((cy ? 1.f : -1.f) * wz[cz], vx, a1);
         a2 = fmaf((cz ? 1.f : -1.f) * wy[cy], vx, a2);
     }
-    xb[p] = fmaf(mp, a0, xb[p]);
-    yb[p] = fmaf(mp, a1, yb[p]);
-    zb[p] = fmaf(mp, a2, zb[p]);
+    xb[p] = fmaf(mp, a0, xb0);
+    yb[p] = fmaf(mp, a1, yb0);
+    zb[p] = fmaf(mp, a2, zb0);
 }
 
 // y += a * x  (float4)
