@@ -45,6 +45,9 @@ BYTES_PER_CELL = {
     "source_init": 8, "deposit": 16, "fft_r2c": 8, "green": 16, "fft_c2r": 8, "kick_drift": 60,
     "sweep_x": 44, "sweep_y": 44, "sweep_z": 44, "sweep_x_adj": 68, "sweep_y_adj": 68, "sweep_z_adj": 68,
     "kick_drift_adj": 108, "green_adj": 16, "deposit_adj": 40, "axpy": 12, "dot3": 24, "fill": 4, "copy": 88,
+    # own FFT passes (csrc/fft.cu): x pass 4 + 4 per component, y pass 4 + 4 per component (half spectrum = 4 B/cell);
+    # "green" / "green_adj" are then the fused z pass: 4 in + 12 out / 12 in + 4 out
+    "fft_x1": 8, "fft_x3": 24, "fft_y1": 8, "fft_y3": 24,
 }
 BYTES_PER_CELL_NOG = {"sweep_x": 40, "sweep_y": 40, "sweep_z": 40, "sweep_x_adj": 60, "sweep_y_adj": 60,
                       "sweep_z_adj": 60, "copy": 40}

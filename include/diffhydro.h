@@ -161,6 +161,8 @@ int dh_sync(dh_ctx* ctx);
  *           recomputation by itself when the device cannot hold them);
  *   "gstore": 0 makes a checkpointed dh_run NOT keep every step's g' (3 N^3 floats per step of the run) for
  *           dh_run_vjp, which then repeats deposit + Poisson solve in the segment re-run (default 1, same fallback).
+ *   "own_fft": 0 routes the Poisson solve through cuFFT (1 R2C + multiply kernel + 3 C2R) instead of the library's own
+ *           FFT passes fused with the Green multiply (default 1 when grid_n is a power of two).
  * Unknown key: DH_ERR_INVALID. */
 int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of

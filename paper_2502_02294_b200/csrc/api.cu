@@ -333,6 +333,10 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
         if (cufftSetStream(c->plan_r2c, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_c2r, c->stream) != CUFFT_SUCCESS) {
             set_error("cufftSetStream failed"); return fail(DH_ERR_CUFFT);
         }
+        if (own_fft_supported(grid_n)) {
+            if ((rc = own_fft_init(c)) != DH_OK) return fail(rc);
+            c->own_fft = true;
+        }
     }
     if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp, 5, c->n3)) != DH_OK) return fail(rc);
     if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp2, 5, c->n3)) != DH_OK) return fail(rc);
@@ -348,6 +352,7 @@ int dh_free(dh_ctx* c) {
     if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->plans) { cufftDestroy(c->plan_r2c); cufftDestroy(c->plan_c2r); }
     cudaFree(c->fft_work);
+    cudaFree(c->fft_tw);
     cudaFree(c->delta);
     for (auto p : c->spec) cudaFree(p);
     for (auto p : c->gp) cudaFree(p);
@@ -379,7 +384,7 @@ int dh_sync(dh_ctx* c) {
 static const char* const PROF_NAMES[PROF_N] = {
     "source_init", "deposit", "fft_r2c", "green", "fft_c2r", "kick_drift", "sweep_x", "sweep_y", "sweep_z",
     "sweep_x_adj", "sweep_y_adj", "sweep_z_adj", "kick_drift_adj", "green_adj", "deposit_adj", "axpy", "dot3", "fill",
-    "copy"};
+    "copy", "fft_x1", "fft_x3", "fft_y1", "fft_y3"};
 
 int dh_profile_enable(dh_ctx* c, int on) {
     if (!c) return DH_ERR_INVALID;
@@ -411,6 +416,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
     else if (!strcmp(key, "tape")) c->tune_tape = value;
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
+    else if (!strcmp(key, "own_fft")) c->tune_own_fft = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }

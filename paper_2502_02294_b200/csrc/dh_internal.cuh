@@ -46,7 +46,8 @@ struct StepScalars { double dtau, kappa, K, A; };
 enum ProfCat {
     PROF_SOURCE_INIT = 0, PROF_DEPOSIT, PROF_FFT_R2C, PROF_GREEN, PROF_FFT_C2R, PROF_KICK_DRIFT,
     PROF_SWEEP_X, PROF_SWEEP_Y, PROF_SWEEP_Z, PROF_SWEEP_X_ADJ, PROF_SWEEP_Y_ADJ, PROF_SWEEP_Z_ADJ,
-    PROF_KICK_DRIFT_ADJ, PROF_GREEN_ADJ, PROF_DEPOSIT_ADJ, PROF_AXPY, PROF_DOT3, PROF_FILL, PROF_COPY, PROF_N
+    PROF_KICK_DRIFT_ADJ, PROF_GREEN_ADJ, PROF_DEPOSIT_ADJ, PROF_AXPY, PROF_DOT3, PROF_FILL, PROF_COPY,
+    PROF_FFT_X1, PROF_FFT_X3, PROF_FFT_Y1, PROF_FFT_Y3, PROF_N
 };
 
 struct Snapshot {
@@ -92,6 +93,9 @@ struct dh_ctx {
     bool plans = false;
     void* fft_work = nullptr;
     size_t fft_work_bytes = 0;
+    float2* fft_tw = nullptr;      // own FFT passes (fft.cu): (cos, sin)(2 pi j / N)
+    bool own_fft = false;          // grid side is a power of two in [32, 1024]
+    int tune_own_fft = 1;          // 0: Poisson solve through cuFFT + green kernels (pm.cu)
 
     // scratch
     float* delta = nullptr;        // N^3 real (Poisson source / delta_bar)
@@ -181,6 +185,12 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
 int launch_dot3(dh_ctx* c, float* const a[3], float* const b[3], double scale, double* out);
 int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t* i1);
 int launch_fill(dh_ctx* c, float* p, int64_t n, float v);
+
+// ---- own FFT passes fused with the Green multiply (fft.cu) ----
+bool own_fft_supported(int N);
+int own_fft_init(dh_ctx* c);
+int own_poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]);
+int own_poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar);
 
 int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]);
 int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar);

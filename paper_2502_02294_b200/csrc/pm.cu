@@ -460,6 +460,7 @@ int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat) 
 }
 
 int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]) {
+    if (c->own_fft && c->tune_own_fft) return own_poisson_forward(c, delta, A, g_out);
     {
         Prof prof(c, PROF_FFT_R2C);
         DH_CUFFT(cufftExecR2C(c->plan_r2c, const_cast<float*>(delta), reinterpret_cast<cufftComplex*>(c->spec[0])));
@@ -474,6 +475,7 @@ int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3
 }
 
 int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar) {
+    if (c->own_fft && c->tune_own_fft) return own_poisson_adjoint(c, g_bar, A, delta_bar);
     float2* gh[3] = {c->spec[1], c->spec[2], c->spec[3]};
     for (int d = 0; d < 3; ++d) {
         Prof prof(c, PROF_FFT_R2C);

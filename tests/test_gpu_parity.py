@@ -104,18 +104,57 @@ def test_cell_index_bit_exact_and_deposit(api, torch_, O, N, nps):
     ctx.close()
 
 
-@pytest.mark.parametrize("N", [32, 64])
-def test_poisson_and_its_transpose(api, torch_, O, N):
+@pytest.mark.parametrize("own_fft", [1, 0])
+@pytest.mark.parametrize("N", [32, 64, 128])
+def test_poisson_and_its_transpose(api, torch_, O, N, own_fft):
+    """S2 and its transpose through both routes of the library: its own FFT passes fused with the Green multiply
+    (csrc/fft.cu, the default) and cuFFT + multiply kernels (csrc/pm.cu), against the oracle's plain DFT-based solve."""
     rng = np.random.default_rng(N)
     L, A = 20.0, 1.5e4
     delta = rng.standard_normal((N, N, N)).astype(np.float32)
     ctx = api.Context(N, L, 5.0 / 3.0, n_part_side=0, e_floor=1e-6)
+    ctx.dh_tune("own_fft", own_fft)
     g = ctx.dh_poisson(_gpu(torch_, delta), A).cpu().numpy()
     ref = O.poisson(N, L, A, delta.astype(np.float64))
     assert PT.max_rel(g, ref) < TOL_STEP
     gb = rng.standard_normal((3, N, N, N)).astype(np.float32)
     db = ctx.dh_poisson_vjp(_gpu(torch_, gb), A).cpu().numpy()
     assert PT.max_rel(db, O.poisson_vjp(N, L, A, gb.astype(np.float64))) < TOL_STEP
+    ctx.close()
+
+
+@pytest.mark.parametrize("N", [256, 512])
+def test_poisson_full_size_closed_form_and_route_agreement(api, torch_, N):
+    """At the bench sizes the oracle is too slow for a dense check; what holds at any size (SURVEY.md 8(c) pins): a
+    single Fourier mode delta = cos(k0.x) gives g' = -A k0 sin(k0.x) / k0^2 exactly; the Nyquist mode gives 0; the
+    two routes of the library agree; <G delta, w> = <delta, G^T w>."""
+    L, A = 100.0, 1.5e4
+    n0 = np.array([3, -5, 7])
+    ax = np.arange(N, dtype=np.float64)
+    ph = 2 * np.pi / N * (n0[0] * ax[None, None, :] + n0[1] * ax[None, :, None] + n0[2] * ax[:, None, None])
+    k0 = 2 * np.pi / L * n0
+    delta = np.cos(ph).astype(np.float32)
+    ctx = api.Context(N, L, 5.0 / 3.0, n_part_side=0, e_floor=1e-6)
+    d_gpu = _gpu(torch_, delta)
+    g = ctx.dh_poisson(d_gpu, A)
+    for d in range(3):
+        ref = -A * k0[d] / float(k0 @ k0) * np.sin(ph)
+        assert PT.max_rel(g[d].cpu().numpy(), ref) < TOL_STEP
+    nyq = np.cos(np.pi * ax)[None, None, :] * np.ones((N, N, 1))
+    gn = ctx.dh_poisson(_gpu(torch_, nyq.astype(np.float32)), A)
+    assert float(gn[0].abs().max()) < 1e-3 * A * L / (2 * np.pi)          # x-Nyquist mode: k~_x = 0, no other component
+    rng = np.random.default_rng(5)
+    rnd = _gpu(torch_, rng.standard_normal((N, N, N)).astype(np.float32))
+    w = _gpu(torch_, rng.standard_normal((3, N, N, N)).astype(np.float32))
+    g_own = ctx.dh_poisson(rnd, A)
+    gt_own = ctx.dh_poisson_vjp(w, A)
+    lhs = float((g_own.double() * w.double()).sum()); rhs = float((rnd.double() * gt_own.double()).sum())
+    assert abs(lhs - rhs) < 1e-5 * (abs(lhs) + float(g_own.double().norm() * w.double().norm()))
+    ctx.dh_tune("own_fft", 0)
+    g_lib = ctx.dh_poisson(rnd, A)
+    gt_lib = ctx.dh_poisson_vjp(w, A)
+    assert float((g_own - g_lib).abs().max() / g_lib.abs().max()) < TOL_STEP
+    assert float((gt_own - gt_lib).abs().max() / gt_lib.abs().max()) < TOL_STEP
     ctx.close()
 
 
