@@ -300,12 +300,25 @@ def test_step_vjp_matches_oracle(api, torch_, O, W, case):
     cg = rng.standard_normal(gas.shape).astype(np.float32)
     cp = rng.standard_normal(part.shape).astype(np.float32)
     rg, rp, rdp = O.step_vjp(P, so, dt_s[k], a_s[k + 1], cg, cp)
+    # Conditioning of the reference itself (reading R28): the oracle's VJP with its inputs moved by one fp32
+    # rounding.  The recomputed g' carries the deposit's fp32 atomic order, so from run to run a handful of limiter
+    # gates sit on the other side of ab > 0 than in the oracle; each moves a few entries by O(1).  The untrimmed bound
+    # is therefore max(north star, 1.5 x what the fp64 oracle does to itself); the trimmed bound below stays tight.
+    sens = 0.0
+    for s in (7, 8, 9):
+        prng = np.random.default_rng(s)
+        sp = O.State(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)),
+                     part.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(part.shape)), a_s[k],
+                     dt_prev=dt_s[k - 1], step=k)
+        sens = max(sens, PT.rel_l2(O.step_vjp(P, sp, dt_s[k], a_s[k + 1], cg, cp)[0], rg))
+    tol_g = max(TOL_GRAD, 1.5 * sens)
     ctx = api.context_for(cfg, **kw)
     sg = api.State(gas, part, so.a, so.dt_prev, so.step)
     co = api.Cot(cg, cp); ci = api.Cot(np.zeros_like(cg), np.zeros_like(cp))
     dp = ctx.dh_step_vjp(sg, dt_s[k], a_s[k + 1], co, ci)
-    # north-star bound on everything; tight bound on all but the few entries a gate flip at fp32 rounding level moves
-    assert PT.rel_l2(ci.gas.cpu().numpy(), rg) < TOL_GRAD
+    eg = PT.rel_l2(ci.gas.cpu().numpy(), rg)
+    print(f"step vjp [{case}]: gas {eg:.2e} (ref moves {sens:.2e})")
+    assert eg < tol_g, (eg, sens)
     assert PT.rel_l2(ci.part.cpu().numpy(), rp) < 1e-4
     assert PT.rel_l2_trimmed(ci.gas.cpu().numpy(), rg, frac=1e-3) < 2e-5
     got = np.array([dp.dgamma, dp.dDtau, dp.dkappa, dp.dK, dp.dA])
@@ -313,7 +326,8 @@ def test_step_vjp_matches_oracle(api, torch_, O, W, case):
     assert np.all(np.abs(got - rdp) < 2e-3 * scale), (got, rdp)
     # aliasing cot_in = cot_out is allowed
     dp2 = ctx.dh_step_vjp(sg, dt_s[k], a_s[k + 1], co, co)
-    assert PT.rel_l2(co.gas.cpu().numpy(), rg) < TOL_GRAD and PT.rel_l2(co.part.cpu().numpy(), rp) < 1e-4
+    assert PT.rel_l2(co.gas.cpu().numpy(), rg) < tol_g and PT.rel_l2(co.part.cpu().numpy(), rp) < 1e-4
+    assert PT.rel_l2_trimmed(co.gas.cpu().numpy(), rg, frac=1e-3) < 2e-5
     ctx.close()
 
 
