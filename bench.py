@@ -211,6 +211,8 @@ def main():
     ap.add_argument("--stride", type=int, default=-1, help="checkpoint stride (default: the workload's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="dh_tune knob for A/B runs (e.g. part_pipe=0); recorded in config")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "own" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
@@ -241,6 +243,9 @@ def main():
     gas_h, part_h, target_h = build_inputs(W, cfg, rank)
     a_s, dt_s = schedule(api, cfg, K)
     ctx = api.context_for(cfg, want_dA=0)
+    for kv in args.tune:
+        key, val = kv.split("=")
+        ctx.dh_tune(key, int(val))
     ctx.dh_reserve(K, stride)
     gas0 = torch.from_numpy(gas_h).cuda()
     part0 = torch.from_numpy(part_h).cuda()
@@ -392,7 +397,7 @@ def main():
                "config": {"workload": cfg.name, "grid": N, "particles": cfg.n_side ** 3, "box": cfg.box,
                           "checkpoint_stride": stride, "schedule": f"first {K} of {cfg.n_steps} ln-a steps"
                           if not cfg.static_mode else f"{K} steps at CFL 0.4",
-                          "loss": "sum (rho_gas - rho_target)^2", "parallelism": f"replicas x{world}",
+                          "loss": "sum (rho_gas - rho_target)^2", "parallelism": f"replicas x{world}", "tune": args.tune,
                           "l2": "working set (state + scratch >= 0.7 GB at 256^3) exceeds the 126 MB L2; no flush"},
                "fwd": {"value": value_fwd, "unit": UNIT, "ms_per_step": ms_fwd / K},
                "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,

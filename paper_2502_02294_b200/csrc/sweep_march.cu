@@ -21,6 +21,7 @@
 // lam_b is formed without carrying D or Psi:  stage B by summation by parts, sum_n Psi_n Psi_b_n / lam; stage A from
 // u*_n - u_n - (kap/2) S = -(lam/4)(D_n - D_{n-1}).
 #include "sweep_common.cuh"
+#include "async_copy.cuh"
 
 namespace dh {
 
@@ -100,14 +101,6 @@ struct FwdPipe {
 // them back with conflict-free LDS; since a thread only ever reads what it copied itself, cp.async.wait_group is the
 // only synchronisation -- no barrier.  The ring hides the HBM latency that 12-16 resident warps of a register-heavy
 // kernel cannot, and in the adjoint doubles as the window of already-visited cells (re-read instead of carried).
-__device__ __forceinline__ void cp_async4(float* smem_dst, const float* gsrc) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int PENDING>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(PENDING) : "memory"); }
-
 constexpr int RING = 8;          // stages (power of two)
 constexpr int NTHR = 128;        // threads per block, fixed: ring offsets are immediates
 constexpr int PF_FWD = 3;        // iterations of prefetch, forward
