@@ -115,6 +115,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(values, dist, device):
+    """Replicas only: the ranks share nothing but the clock.  Every timed quantity is the MAX
+    over ranks (the job is as slow as its slowest replica); dist is torch.distributed or None for a single process."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def job_throughput(world, n3, steps, ms):
+    """Whole-job Gcell-updates/s: every rank advanced its own n3-cell box by `steps` steps in `ms` (max over ranks)."""
+    return world * n3 * steps / (ms * 1e-3) / 1e9
+
+
 def make_workload(W, name, rank=0):
     if name == "cfg3":
         cfg = W.CONFIGS[3]
@@ -307,12 +323,9 @@ def main():
     cmax = ctx.dh_get_cmax(K)
 
     # ---- max over ranks
-    if dist is not None:
-        t = torch.tensor([ms_total, ms_fwd], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_fwd = float(t[0]), float(t[1])
-    value = world * n3 * K / (ms_total * 1e-3) / 1e9
-    value_fwd = world * n3 * K / (ms_fwd * 1e-3) / 1e9
+    ms_total, ms_fwd = max_over_ranks([ms_total, ms_fwd], dist, "cuda")
+    value = job_throughput(world, n3, K, ms_total)
+    value_fwd = job_throughput(world, n3, K, ms_fwd)
 
     # ---- per-kernel pass (untimed for `value`): CUDA events around every launch of the same K steps + reverse
     peak, peak_src = measured_peak()
@@ -371,12 +384,9 @@ def main():
         loss_grad_norm = float(hcg[0, 0, 0, 0])                        # the result is on the host
         barrier()
         sec = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([sec], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            sec = float(t[0])
+        sec = max_over_ranks([sec], dist, "cuda")[0]
         state_bytes = 4 * (gas_h.size + part_h.size)
-        e2e = {"value": world * n3 * K / sec / 1e9, "unit": UNIT,
+        e2e = {"value": job_throughput(world, n3, K, 1e3 * sec), "unit": UNIT,
                "h2d_bytes_per_step": 2 * state_bytes / K, "d2h_bytes_per_step": 2 * state_bytes / K,
                "ms_per_step": 1e3 * sec / K, "timer": "host wall clock around dh_run_host + loss cotangent on the host + "
                "dh_run_vjp_host, device synchronised on both sides"}
