@@ -160,8 +160,21 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
     const bool grav = c->opt.gravity_on != 0;
     float* const* gp = gp_keep ? gp_keep : (tape ? tape->gp : c->gp);
     if (grav && !gp_ready) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp));
-    if (c->np > 0 && part_out)
+    // S3 beside S4: fork the particle update onto the side stream (not while per-kernel events are being recorded)
+    const bool particles = c->np > 0 && part_out;
+    const bool beside = particles && c->opt.hydro_on && c->tune_overlap && c->side && !c->prof_on;
+    if (beside) {
+        DH_CUDA(cudaEventRecord(c->ev_fork, c->stream));
+        DH_CUDA(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+        cudaStream_t main_stream = c->stream;
+        c->stream = c->side;
+        const int rc = launch_kick_drift(c, grav ? gp : nullptr, part, part_out, (float)s.K, (float)(s.dtau / c->dx));
+        c->stream = main_stream;
+        DH_TRY(rc);
+        DH_CUDA(cudaEventRecord(c->ev_join, c->side));
+    } else if (particles) {
         DH_TRY(launch_kick_drift(c, grav ? gp : nullptr, part, part_out, (float)s.K, (float)(s.dtau / c->dx)));
+    }
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
         const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
@@ -175,6 +188,7 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
             DH_TRY(launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr));
             for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
         }
+        if (beside) DH_CUDA(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     } else if (gas_out[0] != gas[0]) {
         for (int k = 0; k < 5; ++k)
             DH_CUDA(cudaMemcpyAsync(gas_out[k], gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
@@ -340,6 +354,12 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
     }
     if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp, 5, c->n3)) != DH_OK) return fail(rc);
     if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp2, 5, c->n3)) != DH_OK) return fail(rc);
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        set_error("dh_init: side stream / events: %s", cudaGetErrorString(cudaGetLastError()));
+        return fail(DH_ERR_CUDA);
+    }
     if ((rc = dev_alloc(c, (void**)&c->cmax_step, 3 * sizeof(float))) != DH_OK) return fail(rc);
     if ((rc = dev_alloc(c, (void**)&c->scal_dev, 8 * sizeof(double))) != DH_OK) return fail(rc);
     if (cudaMemsetAsync(c->scal_dev, 0, 8 * sizeof(double), c->stream) != cudaSuccess) return fail(DH_ERR_CUDA);
@@ -369,6 +389,9 @@ int dh_free(dh_ctx* c) {
     for (auto& t : c->tapes) cudaFree(t.buf);
     for (auto& t : c->gstore) cudaFree(t.buf);
     for (auto e : c->prof_ev) cudaEventDestroy(e);
+    if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     cudaGetLastError();
     delete c;
@@ -417,6 +440,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "tape")) c->tune_tape = value;
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
     else if (!strcmp(key, "own_fft")) c->tune_own_fft = value;
+    else if (!strcmp(key, "overlap")) c->tune_overlap = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }

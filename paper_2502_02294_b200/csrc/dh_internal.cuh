@@ -82,11 +82,17 @@ struct dh_ctx {
     double f_b = 0, m_p = 0, rho_bar = 0;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
+    // Side stream: the particle update of a step shares only the read-only g' with the step's three sweeps (reading
+    // R16), so it runs beside them; forked from and joined back into `stream` with events inside every step, so callers
+    // still see one stream.
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int sm_count = 148;
     int64_t launches = 0;
     int64_t bytes = 0;
     // tuning knobs (dh_tune): 0 = built-in choice
     int tune_march_s_fwd = 0, tune_march_s_adj = 0;   // segment length of the marching y/z sweeps
+    int tune_overlap = 1;                             // 0: kick_drift on the main stream, after which the sweeps start
     int tune_yz_chain = 0;                            // 1: y/z sweeps through the chain kernels of sweep.cu
 
     cufftHandle plan_r2c = 0, plan_c2r = 0;

@@ -255,6 +255,51 @@ def test_config1_hydro_sod_sphere_at_64(api, torch_, O, W):
     ctx.close()
 
 
+def test_config3_full_size_step_and_vjp(api, torch_, O, W):
+    """Config 3 at its full size (256^3 cells, 256^3 particles, the launch configuration bench.py times): one coupled
+    step (Strang order YXZ, so the chain x kernel and both marching kernels run) and that step's VJP against the oracle
+    on EVERY cell and particle; cell indices of all 3 x 2^24 coordinates bit-exact; conservation of gas mass."""
+    cfg = W.CONFIGS[3]
+    delta, gas, part = W.coupled_ic(cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    k = 3
+    ctx = api.context_for(cfg)
+    tp = _gpu(torch_, part)
+    for ax in range(3):
+        i0, i1 = ctx.dh_debug_cell_index(tp[ax])
+        r0, r1 = O.cell_index(part[ax], cfg.N)
+        assert np.array_equal(i0.cpu().numpy(), r0) and np.array_equal(i1.cpu().numpy(), r1)
+    del tp
+    so = O.State(gas, part, a_s[k], dt_prev=dt_s[k - 1], step=k)
+    sg = api.State(gas, part, so.a, so.dt_prev, so.step)
+    cm_ref, _ = O.step(P, so, dt_s[k], a_s[k + 1])
+    cm = torch_.zeros(3, device="cuda")
+    ctx.dh_step(sg, dt_s[k], a_s[k + 1], cm)
+    out = sg.gas.cpu().numpy()
+    e = PT.field_err(out, so.gas)
+    e.update(PT.part_err(sg.part.cpu().numpy(), so.part, cfg.N))
+    print("config3 full-size step:", e)
+    assert max(e.values()) < TOL_STEP, e
+    assert np.max(np.abs(cm.cpu().numpy() / cm_ref - 1)) < TOL_STEP
+    assert abs(out[0].astype(np.float64).sum() / gas[0].astype(np.float64).sum() - 1) < 1e-6
+    # the step's VJP with the bench loss's cotangent 2 (rho - rho_target) on the gas density and none on the particles
+    target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.target_seed, cfg.rms_delta))
+    cg = np.zeros_like(gas); cg[0] = 2.0 * (gas[0] - target)
+    cp = np.zeros_like(part)
+    s_in = O.State(gas, part, a_s[k], dt_prev=dt_s[k - 1], step=k)
+    rg, rp, rdp = O.step_vjp(P, s_in, dt_s[k], a_s[k + 1], cg, cp)
+    s_gpu = api.State(gas, part, s_in.a, s_in.dt_prev, s_in.step)
+    co = api.Cot(cg, cp)
+    dp = ctx.dh_step_vjp(s_gpu, dt_s[k], a_s[k + 1], co, co)
+    eg, ep = PT.rel_l2(co.gas.cpu().numpy(), rg), PT.rel_l2(co.part.cpu().numpy(), rp)
+    print(f"config3 full-size step VJP: gas {eg:.2e}, particles {ep:.2e}, dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}")
+    assert eg < TOL_GRAD and ep < TOL_GRAD
+    assert PT.rel_l2_trimmed(co.gas.cpu().numpy(), rg, frac=1e-3) < 2e-5
+    assert abs(dp.dgamma - rdp[0]) < TOL_GRAD * max(abs(rdp[0]), 1e-3 * np.sqrt(gas[0].size))
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------------ adjoint
 @pytest.mark.parametrize("N", [32, 64])
 @pytest.mark.parametrize("d", [0, 1, 2])
