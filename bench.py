@@ -146,17 +146,17 @@ def make_workload(W, name, rank=0):
 
 
 def build_inputs(W, cfg, rank):
-    """Seeded synthetic inputs: fp32 gas (5,N,N,N), part (6,N_p), loss target rho_t (N,N,N)."""
+    """Seeded synthetic inputs.  Coupled configs: the initial density contrast delta (N,N,N) and
+    the loss target rho_t (N,N,N), fp32 -- the state is made from delta on the device (dh_ic_zeldovich).  Config 1: the
+    gas state itself (spherical Sod, no particles)."""
     N = cfg.N
     if cfg.static_mode:                                   # config 1: spherical Sod, hydro only
         gas = W.sod_sphere(N, cfg.gamma)
-        part = np.zeros((6, 0), dtype=np.float32)
-        target = np.full((N, N, N), 0.5, dtype=np.float32)
-    else:
-        _, gas, part = W.coupled_ic(cfg, seed=cfg.seed + rank)
-        tseed = (cfg.target_seed or cfg.seed + 1000) + rank
-        target = (cfg.f_b * (1.0 + W.gaussian_field(N, cfg.box, tseed, cfg.rms_delta))).astype(np.float32)
-    return gas, part, target
+        return None, gas, np.zeros((6, 0), dtype=np.float32), np.full((N, N, N), 0.5, dtype=np.float32)
+    delta = W.gaussian_field(N, cfg.box, cfg.seed + rank, cfg.rms_delta).astype(np.float32)
+    tseed = (cfg.target_seed or cfg.seed + 1000) + rank
+    target = (cfg.f_b * (1.0 + W.gaussian_field(N, cfg.box, tseed, cfg.rms_delta))).astype(np.float32)
+    return delta, None, None, target
 
 
 def schedule(api, cfg, K):
@@ -171,7 +171,7 @@ def schedule(api, cfg, K):
 def oracle_sample(W, cfg, n_side, n_steps, with_vjp=True):
     """The CPU oracle on a bounded sample of the workload: the same recipe (cell size, IC, schedule) on an n_side^3
     sub-box, n_steps steps forward + the reverse pass.  Returns (cell-updates/s, threads, seconds)."""
-    from oracle import oracle as O
+    from oracle import oracle as O, ic as IC
     sub = W.scaled_config({"cfg3_256_coupled": 3, "cfg4_512_coupled": 4, "cfg1_128_hydro": 1}.get(cfg.name, 3), n_side)
     if sub.static_mode:
         gas = W.sod_sphere(n_side, sub.gamma).astype(np.float64)
@@ -180,7 +180,7 @@ def oracle_sample(W, cfg, n_side, n_steps, with_vjp=True):
         P = O.make_params(n_side, sub.box, sub.gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=sub.e_floor())
         a0 = 1.0
     else:
-        _, gas, part = W.coupled_ic(sub)
+        _, gas, part = IC.coupled_ic(W, sub)
         P = O.make_params(n_side, sub.box, sub.gamma, n_part_side=sub.n_side, H0=sub.H0, Omega_m=sub.Omega_m,
                           Omega_b=sub.Omega_b, Omega_L=sub.Omega_L, e_floor=sub.e_floor(), lim_eps=sub.lim_eps)
         a_full, dt_full = O.schedule_lna(P, sub.a0, sub.a1, max(sub.n_steps, n_steps))
@@ -256,17 +256,31 @@ def main():
     K, Wm = args.steps, args.warmup
     stride = args.stride if args.stride >= 0 else (cfg.checkpoint_stride or 10)
     N, n3 = cfg.N, cfg.N ** 3
-    gas_h, part_h, target_h = build_inputs(W, cfg, rank)
+    delta_h, gas_h, part_h, target_h = build_inputs(W, cfg, rank)
     a_s, dt_s = schedule(api, cfg, K)
     ctx = api.context_for(cfg, want_dA=0)
     for kv in args.tune:
         key, val = kv.split("=")
         ctx.dh_tune(key, int(val))
     ctx.dh_reserve(K, stride)
-    gas0 = torch.from_numpy(gas_h).cuda()
-    part0 = torch.from_numpy(part_h).cuda()
     target = torch.from_numpy(target_h).cuda()
     a0 = 1.0 if cfg.static_mode else cfg.a0
+    ic_ms = None
+    if delta_h is not None:
+        # the state comes from delta on the device (dh_ic_zeldovich); timed on its own, outside the step loop
+        delta_d = torch.from_numpy(delta_h).cuda()
+        vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+        ctx.dh_ic_zeldovich(delta_d, cfg.a0, vf, e0)                    # warm-up
+        ev_ic = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        torch.cuda.synchronize()
+        ev_ic[0].record()
+        st_ic = ctx.dh_ic_zeldovich(delta_d, cfg.a0, vf, e0)
+        ev_ic[1].record()
+        gas0, part0 = st_ic.gas, st_ic.part
+        gas_h, part_h = gas0.cpu().numpy(), part0.cpu().numpy()        # host copies for the end-to-end leg
+    else:
+        gas0 = torch.from_numpy(gas_h).cuda()
+        part0 = torch.from_numpy(part_h).cuda()
 
     def barrier():
         torch.cuda.synchronize()
@@ -309,6 +323,17 @@ def main():
     launches = ctx.dh_launch_count() - l0
     ms_total = ev[0].elapsed_time(ev[1])
     grad_norm = float(ct.gas.double().norm())
+    grad_delta_norm = None
+    if delta_h is not None:
+        ctx.dh_ic_zeldovich_vjp(delta_d, vf, e0, ct)                    # warm-up (allocates nothing new)
+        torch.cuda.synchronize()
+        ev_ic[2].record()
+        grad_delta = ctx.dh_ic_zeldovich_vjp(delta_d, vf, e0, ct)       # dL / d delta_init of the K-step run
+        ev_ic[3].record()
+        torch.cuda.synchronize()
+        ic_ms = {"ic_map_ms": ev_ic[0].elapsed_time(ev_ic[1]), "ic_map_vjp_ms": ev_ic[2].elapsed_time(ev_ic[3]),
+                 "note": "dh_ic_zeldovich / dh_ic_zeldovich_vjp once per run, outside the per-step timed regions"}
+        grad_delta_norm = float(grad_delta.double().norm())
 
     # ---- timed region 2: forward only
     st2 = api.State(gas0.clone(), part0.clone(), a0)
@@ -412,7 +437,9 @@ def main():
                "fwd": {"value": value_fwd, "unit": UNIT, "ms_per_step": ms_fwd / K},
                "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,
                "cpu_baseline": cpu, "clocks": clocks,
-               "check": {"cfl_cmax_last": float(np.max(cmax[-1])), "grad_norm": grad_norm, "dgamma": dp.dgamma,
+               "ic": ic_ms,
+               "check": {"cfl_cmax_last": float(np.max(cmax[-1])), "grad_norm": grad_norm,
+                         "grad_delta_init_norm": grad_delta_norm, "dgamma": dp.dgamma,
                          "device_bytes": ctx.dh_device_bytes()}}
         print(json.dumps(out))
     ctx.close()

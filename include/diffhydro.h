@@ -192,6 +192,23 @@ int dh_poisson_vjp(dh_ctx* ctx, float* const g_bar[3], double A, float* delta_ba
 /* S3 in place on part[6]. */
 int dh_kick_drift(dh_ctx* ctx, float* const g[3], float* const part[6], double K, double dtau_over_dx);
 
+/* ---- the step on the input side of the path: initial-condition map and its transpose ----
+ * PAPER.md:49 (section 2.1): initial conditions by Lagrangian perturbation theory; reading R19 of DESIGN.md: first
+ * order (the Zel'dovich map) of a density contrast delta_init given at scale factor a0, one particle per cell:
+ *   psi^_d = i k~_d delta^ / k^2;  x = wrap(q + psi/dx), w = vel_factor psi;
+ *   rho = f_b (1 + delta), m = rho w, eps = rho (e_tilde0 + |w|^2 / 2),   f_b = Omega_b / Omega_m of dh_init.
+ * delta_init: DEVICE, N^3 floats, [z][y][x], not modified.  vel_factor = a0^2 H(a0) f(a0) (EdS: H0 sqrt(a0)), km/s per
+ * h^-1 Mpc; e_tilde0 = a0^2 times the initial thermal energy per unit mass.  state_out: caller-owned DEVICE arrays,
+ * overwritten; its scalars are set to (a0, dt_prev = 0, step = 0).  Needs gravity_on and n_part_side == grid_n, else
+ * DH_ERR_INVALID.  Asynchronous on the context's stream. */
+int dh_ic_zeldovich(dh_ctx* ctx, const float* delta_init, double a0, double vel_factor, double e_tilde0,
+                    dh_state* state_out);
+/* Transpose of the Jacobian of dh_ic_zeldovich at delta_init applied to cot_state (gas cotangents required, particle
+ * cotangent pointers may be NULL = zero): grad_delta (DEVICE, N^3 floats) is OVERWRITTEN with dL/d delta_init.
+ * Together with dh_run_vjp this is "gradient w.r.t. the initial density field" in device memory. */
+int dh_ic_zeldovich_vjp(dh_ctx* ctx, const float* delta_init, double vel_factor, double e_tilde0,
+                        const dh_cot* cot_state, float* grad_delta);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,7 +28,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_last_error", "dh_get_cmax", "dh_schedule_lna", "dh_step_scalars", "dh_debug_cell_index",
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
-           "dh_profile_read", "dh_reserve", "dh_tune"]
+           "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp"]
 
 
 class DhError(RuntimeError):
@@ -104,6 +104,8 @@ _lib.dh_deposit.argtypes = [C.c_void_p, C.c_void_p, _P3, C.c_void_p]
 _lib.dh_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_double, _P3]
 _lib.dh_poisson_vjp.argtypes = [C.c_void_p, _P3, C.c_double, C.c_void_p]
 _lib.dh_kick_drift.argtypes = [C.c_void_p, _P3, _P6, C.c_double, C.c_double]
+_lib.dh_ic_zeldovich.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(dh_state)]
+_lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
 
 
 def _check(rc, where):
@@ -307,6 +309,26 @@ class Context:
     def dh_kick_drift(self, g: torch.Tensor | None, part: torch.Tensor, K, dtau_over_dx):
         gp = _ptrs(g, 3, _P3) if g is not None else _P3()
         _check(_lib.dh_kick_drift(self._h, gp, _ptrs(part, 6, _P6), float(K), float(dtau_over_dx)), "dh_kick_drift")
+
+    def dh_ic_zeldovich(self, delta_init: torch.Tensor, a0, vel_factor, e_tilde0) -> State:
+        """delta_init (N,N,N) fp32 CUDA tensor -> a new State (tensors allocated here, filled by the library)."""
+        assert delta_init.is_cuda and delta_init.dtype == torch.float32 and delta_init.is_contiguous()
+        n3 = self.N ** 3
+        st = State(torch.empty((5, self.N, self.N, self.N), dtype=torch.float32, device=delta_init.device),
+                   torch.empty((6, n3), dtype=torch.float32, device=delta_init.device), a0)
+        cs = st.c_struct()
+        _check(_lib.dh_ic_zeldovich(self._h, delta_init.data_ptr(), float(a0), float(vel_factor), float(e_tilde0),
+                                    C.byref(cs)), "dh_ic_zeldovich")
+        st.a, st.dt_prev, st.step = cs.a, cs.dt_prev, cs.step
+        return st
+
+    def dh_ic_zeldovich_vjp(self, delta_init: torch.Tensor, vel_factor, e_tilde0, cot_state: Cot) -> torch.Tensor:
+        assert delta_init.is_cuda and delta_init.dtype == torch.float32 and delta_init.is_contiguous()
+        grad = torch.empty_like(delta_init)
+        cs = cot_state.c_struct()
+        _check(_lib.dh_ic_zeldovich_vjp(self._h, delta_init.data_ptr(), float(vel_factor), float(e_tilde0), C.byref(cs),
+                                        grad.data_ptr()), "dh_ic_zeldovich_vjp")
+        return grad
 
 
 def dh_schedule_lna(a0, a1, n, H0=100.0, Omega_m=1.0, Omega_b=0.16, Omega_L=0.0):

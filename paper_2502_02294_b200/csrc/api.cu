@@ -711,6 +711,39 @@ int dh_poisson_vjp(dh_ctx* c, float* const g_bar[3], double A, float* delta_bar_
     return poisson_adjoint(c, g_bar, (float)A, delta_bar_out);
 }
 
+static int check_ic(const dh_ctx* c, const float* delta_init, const char* who) {
+    if (!c || !delta_init) { set_error("%s: null argument", who); return DH_ERR_INVALID; }
+    if (!c->opt.gravity_on || c->nps != c->N) {
+        set_error("%s: needs gravity_on and one particle per cell (n_part_side == grid_n)", who);
+        return DH_ERR_INVALID;
+    }
+    return DH_OK;
+}
+
+int dh_ic_zeldovich(dh_ctx* c, const float* delta_init, double a0, double vel_factor, double e_tilde0, dh_state* out) {
+    DH_TRY(check_ic(c, delta_init, "dh_ic_zeldovich"));
+    if (!out) { set_error("dh_ic_zeldovich: null state"); return DH_ERR_INVALID; }
+    DH_TRY(check_state(c, out->gas, out->part));
+    DH_TRY(poisson_forward(c, delta_init, 1.f, c->gp));                    // psi = grad^-1 of -delta: the A = 1 solve
+    DH_TRY(launch_ic_state(c, delta_init, c->gp, out->gas, out->part, (float)vel_factor, (float)e_tilde0));
+    out->a = a0; out->dt_prev = 0.0; out->step = 0;
+    return DH_OK;
+}
+
+int dh_ic_zeldovich_vjp(dh_ctx* c, const float* delta_init, double vel_factor, double e_tilde0, const dh_cot* cot_state,
+                        float* grad_delta) {
+    DH_TRY(check_ic(c, delta_init, "dh_ic_zeldovich_vjp"));
+    if (!cot_state || !grad_delta) { set_error("dh_ic_zeldovich_vjp: null argument"); return DH_ERR_INVALID; }
+    for (int k = 0; k < 5; ++k) if (!cot_state->gas[k]) { set_error("dh_ic_zeldovich_vjp: null gas cotangent %d", k); return DH_ERR_INVALID; }
+    DH_TRY(ensure_adjoint_scratch(c));
+    DH_TRY(poisson_forward(c, delta_init, 1.f, c->gp));
+    DH_TRY(launch_ic_state_vjp(c, delta_init, c->gp, cot_state->gas, cot_state->part, grad_delta, c->gpb,
+                               (float)vel_factor, (float)e_tilde0));
+    DH_TRY(poisson_adjoint(c, c->gpb, 1.f, c->delta));
+    DH_TRY(launch_axpy(c, c->delta, grad_delta, 1.f));
+    return DH_OK;
+}
+
 int dh_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], double K, double dtau_over_dx) {
     if (!c || !part) { set_error("dh_kick_drift: bad argument"); return DH_ERR_INVALID; }
     return launch_kick_drift(c, g, part, part, (float)K, (float)dtau_over_dx);

@@ -191,6 +191,12 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
 int launch_dot3(dh_ctx* c, float* const a[3], float* const b[3], double scale, double* out);
 int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t* i1);
 int launch_fill(dh_ctx* c, float* p, int64_t n, float v);
+int launch_axpy(dh_ctx* c, const float* x, float* y, float a);
+// ---- initial-condition map (ic.cu) ----
+int launch_ic_state(dh_ctx* c, const float* delta, float* const psi[3], float* const gas[5], float* const part[6],
+                    float vf, float e0);
+int launch_ic_state_vjp(dh_ctx* c, const float* delta, float* const psi[3], const float* const cot_gas[5],
+                        const float* const cot_part[6], float* grad, float* const psi_b[3], float vf, float e0);
 
 // ---- own FFT passes fused with the Green multiply (fft.cu) ----
 bool own_fft_supported(int N);

@@ -566,16 +566,20 @@ int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6],
     return DH_OK;
 }
 
+// y += a x over one mesh
+int launch_axpy(dh_ctx* c, const float* x, float* y, float a) {
+    const int64_t n4 = c->n3 / 4;
+    Prof prof(c, PROF_AXPY);
+    axpy_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(reinterpret_cast<const float4*>(x),
+                                                                         reinterpret_cast<float4*>(y), n4, a);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
 int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6], float* rho_bar_gas,
                        float* const xbar[3]) {
-    if (c->opt.gas_sources_gravity && rho_bar_gas) {
-        const int64_t n4 = c->n3 / 4;
-        Prof prof(c, PROF_AXPY);
-        axpy_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
-            reinterpret_cast<const float4*>(delta_bar), reinterpret_cast<float4*>(rho_bar_gas), n4, 1.f);
-        c->launches++;
-        DH_CUDA(cudaGetLastError());
-    }
+    if (c->opt.gas_sources_gravity && rho_bar_gas) DH_TRY(launch_axpy(c, delta_bar, rho_bar_gas, 1.f));
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT_ADJ);
         deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(

@@ -4,8 +4,8 @@ This module is the ONE thing the CPU oracle's tests and the CUDA path's tests sh
 recipes only (numpy on the host) -- none of the step's arithmetic, no CUDA, no oracle import:
   * a seeded Gaussian random field with P(k) = A k^-2 exp(-(k/k_c)^2), k_c = k_Nyq/2, rescaled to the stated rms
     (stand-in for the paper's Eisenstein-Hu + LPT initial conditions, PAPER.md:49; reading R19 in DESIGN.md);
-  * the Zel'dovich map  delta -> (gas, particles)  at the starting scale factor, and its transpose (used to
-    express "gradient w.r.t. the initial density field" for configs 0, 2, 3 on either side);
+    -- the field is the input; the Zel'dovich map  delta -> (gas, particles)  is part of the method: the CUDA path does
+    it on the device (dh_ic_zeldovich), the oracle in oracle/ic.py;
   * the spherical Sod-type Riemann problem of config 1 and a 1-D Sod tube;
   * the config table and the (a, dt) schedule in ln a for an EdS cosmology.
 Units (reading R18): length h^-1 Mpc, velocity km/s, H0 = 100, density in units of the mean comoving total
@@ -119,87 +119,10 @@ def gaussian_field(N: int, L: float, seed: int, rms: float) -> np.ndarray:
     return d
 
 
-def _psi_operator(N, L):
-    """Fourier multipliers i k~_d / k^2 (d = x, y, z) on the rfftn layout; k~_d = 0 on its Nyquist plane."""
-    kf, nx, ny, nz = _kgrid(N, L)
-    k2 = kf * kf * (nx * nx + ny * ny + nz * nz) + 0.0 * (nx + ny + nz)
-    inv = np.zeros_like(k2)
-    inv[k2 > 0] = 1.0 / k2[k2 > 0]
-    comps = []
-    for n in (nx, ny, nz):
-        nt = np.where(np.abs(n) == N // 2, 0.0, n) + 0.0 * k2
-        comps.append(1j * kf * nt * inv)
-    return comps
-
-
-def displacement(delta: np.ndarray, L: float) -> np.ndarray:
-    """Zel'dovich displacement psi (3,N,N,N) in h^-1 Mpc with div psi = -delta."""
-    N = delta.shape[0]
-    dh = np.fft.rfftn(delta)
-    return np.stack([np.fft.irfftn(op * dh, s=(N, N, N), axes=(0, 1, 2)) for op in _psi_operator(N, L)])
-
-
-def displacement_T(psib: np.ndarray, L: float) -> np.ndarray:
-    """Transpose of `displacement` (the multipliers are odd and imaginary, so each is antisymmetric)."""
-    N = psib.shape[1]
-    acc = 0.0
-    for d, op in enumerate(_psi_operator(N, L)):
-        acc = acc - np.fft.irfftn(op * np.fft.rfftn(psib[d]), s=(N, N, N), axes=(0, 1, 2))
-    return acc
-
-
 def velocity_factor(cfg: Config, a: float) -> float:
     """w = a^2 H(a) f(a) psi; EdS: H0 sqrt(a)."""
     assert cfg.Omega_L == 0.0 and abs(cfg.Omega_m - 1.0) < 1e-15, "only EdS ICs are provided"
     return cfg.H0 * np.sqrt(a)
-
-
-def zeldovich_state(delta: np.ndarray, cfg: Config):
-    """delta (N^3, at a0) -> gas (5,N,N,N), part (6,N^3), float64.  Reading R19."""
-    N, L, a = cfg.N, cfg.box, cfg.a0
-    assert cfg.n_side == N, "one particle per cell"
-    dx = L / N
-    psi = displacement(delta, L)
-    vf = velocity_factor(cfg, a)
-    q = np.arange(N) + 0.5
-    Q = np.stack(np.meshgrid(q, q, q, indexing="ij")[::-1])     # (x,y,z) components on the [z][y][x] grid
-    pos = (Q + psi / dx).reshape(3, -1)
-    pos = pos - N * np.floor(pos / N)
-    w = (vf * psi).reshape(3, -1)
-    part = np.concatenate([pos, w], axis=0)
-    rho = cfg.f_b * (1.0 + delta)
-    v = vf * psi
-    e0 = cfg.e_tilde0()
-    gas = np.empty((5, N, N, N))
-    gas[0] = rho
-    gas[1:4] = rho[None] * v
-    gas[4] = rho * (e0 + 0.5 * np.sum(v * v, axis=0))
-    return gas, part
-
-
-def zeldovich_state_vjp(delta: np.ndarray, cfg: Config, cot_gas: np.ndarray, cot_part: np.ndarray) -> np.ndarray:
-    """Transpose of d(zeldovich_state)/d(delta) applied to (cot_gas, cot_part) -> cotangent of delta."""
-    N, L, a = cfg.N, cfg.box, cfg.a0
-    dx = L / N
-    psi = displacement(delta, L)
-    vf = velocity_factor(cfg, a)
-    rho = cfg.f_b * (1.0 + delta)
-    v = vf * psi
-    e0 = cfg.e_tilde0()
-    cg = np.asarray(cot_gas, dtype=np.float64).reshape(5, N, N, N)
-    cp = np.asarray(cot_part, dtype=np.float64).reshape(6, N, N, N)
-    rho_b = cg[0] + np.sum(cg[1:4] * v, axis=0) + cg[4] * (e0 + 0.5 * np.sum(v * v, axis=0))
-    v_b = cg[1:4] * rho[None] + cg[4][None] * rho[None] * v
-    psi_b = vf * v_b + cp[0:3] / dx + vf * cp[3:6]
-    return cfg.f_b * rho_b + displacement_T(psi_b, L)
-
-
-def coupled_ic(cfg: Config, seed=None):
-    """Seeded IC of a coupled config.  Returns (delta f64, gas f32, part f32) -- the fp32 arrays are THE inputs
-    both the oracle (promoted to fp64) and the CUDA path receive (reading R24)."""
-    delta = gaussian_field(cfg.N, cfg.box, cfg.seed if seed is None else seed, cfg.rms_delta)
-    gas, part = zeldovich_state(delta, cfg)
-    return delta, gas.astype(np.float32), part.astype(np.float32)
 
 
 # ------------------------------------------------------------------ hydro ICs ------

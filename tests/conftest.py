@@ -24,3 +24,10 @@ def O():
 def W():
     from paper_2502_02294_b200 import workloads
     return workloads
+
+
+@pytest.fixture(scope="session")
+def IC():
+    """The CPU oracle of the initial-condition map (oracle/ic.py)."""
+    from oracle import ic
+    return ic

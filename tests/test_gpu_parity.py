@@ -182,8 +182,9 @@ def test_kick_drift_matches_oracle(api, torch_, O, W):
 
 # ------------------------------------------------------------------------------------------------- coupled step
 def _coupled_case(W, N, n_steps, **kw):
+    from oracle import ic as IC
     cfg = W.scaled_config(0, N, n_steps=n_steps, **kw)
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     return cfg, delta, gas, part
 
 
@@ -211,10 +212,10 @@ def test_one_coupled_step_matches_oracle(api, torch_, O, W, N, nps):
     ctx.close()
 
 
-def test_config0_full_run_and_cfl_log(api, torch_, O, W):
+def test_config0_full_run_and_cfl_log(api, torch_, O, W, IC):
     """Config 0 (32^3 coupled, 20 steps in ln a to a = 0.1): protocol (ii), <= 1e-3 at the end; CFL maxima (v)."""
     cfg = W.CONFIGS[0]
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     P = PT.oracle_params(O, cfg)
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
     g_ref, p_ref, cm_ref, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
@@ -255,12 +256,12 @@ def test_config1_hydro_sod_sphere_at_64(api, torch_, O, W):
     ctx.close()
 
 
-def test_config3_full_size_step_and_vjp(api, torch_, O, W):
+def test_config3_full_size_step_and_vjp(api, torch_, O, W, IC):
     """Config 3 at its full size (256^3 cells, 256^3 particles, the launch configuration bench.py times): one coupled
     step (Strang order YXZ, so the chain x kernel and both marching kernels run) and that step's VJP against the oracle
     on EVERY cell and particle; cell indices of all 3 x 2^24 coordinates bit-exact; conservation of gas mass."""
     cfg = W.CONFIGS[3]
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     P = PT.oracle_params(O, cfg)
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
     k = 3
@@ -376,17 +377,17 @@ def test_step_vjp_matches_oracle(api, torch_, O, W, case):
     ctx.close()
 
 
-def test_config0_gradient_of_final_density_norm(api, torch_, O, W):
+def test_config0_gradient_of_final_density_norm(api, torch_, O, W, IC):
     """Config 0: L = ||rho_gas(final)||_2; gradient w.r.t. the initial state (and through the Zel'dovich map w.r.t. the
     initial density field) and w.r.t. gamma: protocol (iv), relative L2 <= 1e-3; independent of checkpoint_stride."""
     cfg = W.CONFIGS[0]
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     P = PT.oracle_params(O, cfg)
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
     g_ref, p_ref, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
     cot_g = np.zeros_like(g_ref); cot_g[0] = g_ref[0] / np.linalg.norm(g_ref[0])
     rg, rp, rdp = O.run_vjp(P, gas, part, cfg.a0, a_s[1:], dt_s, cot_g, np.zeros_like(p_ref))
-    grad_delta_ref = W.zeldovich_state_vjp(delta, cfg, rg, rp)
+    grad_delta_ref = IC.state_vjp_of(delta, cfg, W, rg, rp)
     # Conditioning of the reference itself (DESIGN.md reading R28): the same oracle gradient with its fp32 inputs moved
     # by one fp32 rounding (6e-8 relative).  The limiter gate, the floor and |v| make the derivative piecewise, so a few
     # hundred of the ~2e7 gate decisions of this run flip and the fp64 gradient itself moves by ~2e-3.
@@ -397,7 +398,7 @@ def test_config0_gradient_of_final_density_norm(api, torch_, O, W):
     cot_p = np.zeros_like(g_p); cot_p[0] = g_p[0] / np.linalg.norm(g_p[0])
     rg_p, rp_p, rdp_p = O.run_vjp(P, gas_p, part_p, cfg.a0, a_s[1:], dt_s, cot_p, np.zeros_like(p_p))
     sens_g, sens_p = PT.rel_l2(rg_p, rg), PT.rel_l2(rp_p, rp)
-    sens_d = PT.rel_l2(W.zeldovich_state_vjp(delta, cfg, rg_p, rp_p), grad_delta_ref)
+    sens_d = PT.rel_l2(IC.state_vjp_of(delta, cfg, W, rg_p, rp_p), grad_delta_ref)
     tol_g, tol_p, tol_d = (max(TOL_GRAD, 1.5 * s) for s in (sens_g, sens_p, sens_d))
     ctx = api.context_for(cfg)
     results = []
@@ -408,10 +409,12 @@ def test_config0_gradient_of_final_density_norm(api, torch_, O, W):
         cg = torch_.zeros_like(sg.gas); cg[0] = (rho / rho.norm()).float()
         ct = api.Cot(cg, torch_.zeros_like(sg.part))
         dp = ctx.dh_run_vjp(ct, ct)
-        results.append((ct.gas.cpu().numpy(), ct.part.cpu().numpy(), dp.as_dict()))
-    for (gg, gp, dp) in results:
+        # the chain to the initial density field on the device as well (dh_ic_zeldovich_vjp)
+        gd = ctx.dh_ic_zeldovich_vjp(_gpu(torch_, delta), W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0(), ct)
+        results.append((ct.gas.cpu().numpy(), ct.part.cpu().numpy(), dp.as_dict(), gd.cpu().numpy()))
+    for (gg, gp, dp, gd) in results:
         eg, ep = PT.rel_l2(gg, rg), PT.rel_l2(gp, rp)
-        ed = PT.rel_l2(W.zeldovich_state_vjp(delta, cfg, gg, gp), grad_delta_ref)
+        ed = PT.rel_l2(gd, grad_delta_ref)
         print(f"config0 gradient: gas {eg:.2e} (ref moves {sens_g:.2e}), part {ep:.2e} ({sens_p:.2e}), "
               f"d/d delta {ed:.2e} ({sens_d:.2e}), dgamma {dp['dgamma'] / rdp[0] - 1:.2e}")
         assert eg < tol_g and ep < tol_p and ed < tol_d, (eg, ep, ed, sens_g, sens_p, sens_d)
@@ -426,12 +429,50 @@ def test_config0_gradient_of_final_density_norm(api, torch_, O, W):
     ctx.close()
 
 
-def test_reverse_pass_storage_policies_agree(api, torch_, W):
+@pytest.mark.parametrize("N", [32, 64, 128])
+def test_ic_map_and_its_transpose_match_oracle(api, torch_, W, IC, N):
+    """dh_ic_zeldovich / dh_ic_zeldovich_vjp (reading R19) against oracle/ic.py on the same seeded
+    delta: state within 1e-5 in the R25 norms; the transposed Jacobian applied to a random cotangent, relative L2 <= 1e-5
+    (both maps are smooth: no gates, no floor)."""
+    cfg = W.scaled_config(0, N, rms_delta=0.05)
+    delta = W.gaussian_field(N, cfg.box, 77 + N, cfg.rms_delta).astype(np.float32)
+    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+    g_ref, p_ref = IC.zeldovich_state(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf, e0)
+    ctx = api.context_for(cfg)
+    dd = _gpu(torch_, delta)
+    st = ctx.dh_ic_zeldovich(dd, cfg.a0, vf, e0)
+    e = PT.field_err(st.gas.cpu().numpy(), g_ref)
+    e.update(PT.part_err(st.part.cpu().numpy(), p_ref, N))
+    assert max(e.values()) < TOL_STEP, e
+    assert st.a == cfg.a0 and st.step == 0 and st.dt_prev == 0.0
+    rng = np.random.default_rng(N)
+    cg = rng.standard_normal(g_ref.shape).astype(np.float32)
+    cp = rng.standard_normal(p_ref.shape).astype(np.float32)
+    ref = IC.zeldovich_state_vjp(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf, e0, cg, cp)
+    got = ctx.dh_ic_zeldovich_vjp(dd, vf, e0, api.Cot(cg, cp)).cpu().numpy()
+    assert PT.rel_l2(got, ref) < 1e-5, PT.rel_l2(got, ref)
+    # the state it makes is the state the step accepts: one step runs and stays finite
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx.dh_step(st, dt_s[0], a_s[1])
+    assert bool(torch_.isfinite(st.gas).all()) and st.step == 1
+    ctx.close()
+
+
+def test_ic_map_rejects_wrong_setups(api, torch_, W):
+    cfg = W.scaled_config(0, 32)
+    ctx = api.Context(32, cfg.box, cfg.gamma, n_part_side=24, e_floor=1e-6)
+    with pytest.raises(api.DhError) as ei:
+        ctx.dh_ic_zeldovich(torch_.zeros((32, 32, 32), device="cuda"), 0.01, 10.0, 1e-3)
+    assert ei.value.code == -1
+    ctx.close()
+
+
+def test_reverse_pass_storage_policies_agree(api, torch_, W, IC):
     """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
     ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
     policies differ by the order of the deposit's fp32 atomics in the recomputed g' (last-bit), nothing more."""
     cfg = W.scaled_config(0, 32, n_steps=7, a1=0.03)
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
     out = []
     for tape, gstore in ((1, 1), (0, 1), (1, 0), (0, 0)):
@@ -452,9 +493,9 @@ def test_reverse_pass_storage_policies_agree(api, torch_, W):
     assert out[0][3] < out[2][3] and out[1][3] < out[3][3]
 
 
-def test_run_host_variant_matches_device_variant(api, torch_, W):
+def test_run_host_variant_matches_device_variant(api, torch_, W, IC):
     cfg = W.scaled_config(0, 32, n_steps=4, a1=0.02)
-    delta, gas, part = W.coupled_ic(cfg)
+    delta, gas, part = IC.coupled_ic(W, cfg)
     a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
     ctx = api.context_for(cfg)
     sg = api.State(gas, part, cfg.a0)

@@ -130,12 +130,12 @@ def test_step_vjp_dot_product(O, W, case):
     assert _rel(lhs, rhs) < 1e-11
 
 
-def test_run_vjp_equals_chained_step_vjps_and_fd_of_loss(O, W):
+def test_run_vjp_equals_chained_step_vjps_and_fd_of_loss(O, W, IC):
     """Reverse sweep over a 6-step run (one full Strang cycle) with the cosmological scalars: the gradient of
     L = sum(rho_final^2)/2 w.r.t. the initial state agrees with central differences along a random direction, and
     dgamma with a central difference in gamma."""
     cfg = W.scaled_config(0, 8, n_steps=6, a1=0.02, rms_delta=0.05)
-    delta, gas, part = W.coupled_ic(cfg, seed=5)
+    delta, gas, part = IC.coupled_ic(W, cfg, seed=5)
     gas = gas.astype(np.float64); part = part.astype(np.float64)
 
     def params(gamma):

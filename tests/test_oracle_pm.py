@@ -230,12 +230,12 @@ def test_zeldovich_pancake_before_shell_crossing(O):
     assert 0.975 < coeff < 1.0, coeff
 
 
-def test_linear_growth_of_3d_field_in_eds(O, W):
+def test_linear_growth_of_3d_field_in_eds(O, W, IC):
     """Small 3-D perturbation, DM only: the fundamental modes grow ~ a (growing mode, EdS).  Only |n| <= 1 modes are
     compared: the CIC window sinc^4 lowers the growth of shorter waves (at N = 32 the fundamental loses < 1 %)."""
     cfg = W.scaled_config(0, 32, n_steps=24, a1=0.08, rms_delta=1e-3, Omega_b=0.0)
     delta = W.gaussian_field(cfg.N, cfg.box, 7, cfg.rms_delta)
-    gas, part = W.zeldovich_state(delta, cfg)
+    gas, part = IC.state_of(delta, cfg, W)
     P = O.make_params(cfg.N, cfg.box, cfg.gamma, hydro_on=0, gas_sources_gravity=0, Omega_b=0.0)
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
     _, part1, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
@@ -261,13 +261,13 @@ def test_uniform_gas_hubble_drag_and_adiabatic_cooling_bitwise(O):
     assert np.array_equal(g1, gas)
 
 
-def test_cold_gas_tracks_dark_matter_in_linear_regime(O, W):
+def test_cold_gas_tracks_dark_matter_in_linear_regime(O, W, IC):
     """Pressureless gas obeys the same linear growth as the DM: on the fundamental modes delta_gas = delta_dm and both
     have grown by a1/a0 (shorter waves differ: CIC window for the DM, numerical diffusion for the gas)."""
     N = 16
     cfg = W.scaled_config(0, N, n_steps=16, a1=0.04, rms_delta=2e-3)
     cfg.T0 = 1.0     # cold: negligible pressure
-    delta, gas, part = W.coupled_ic(cfg, seed=21)
+    delta, gas, part = IC.coupled_ic(W, cfg, seed=21)
     P = O.make_params(cfg.N, cfg.box, cfg.gamma, e_floor=cfg.e_floor())
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
     g1, p1, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
@@ -286,11 +286,11 @@ def test_cold_gas_tracks_dark_matter_in_linear_regime(O, W):
     assert abs(g1[0].sum() / gas[0].astype(np.float64).sum() - 1.0) < 1e-13
 
 
-def test_workload_generators(W):
+def test_workload_generators(W, IC):
     d = W.gaussian_field(16, 20.0, 1000, 0.02)
     assert abs(np.sqrt(np.mean(d * d)) - 0.02) < 1e-15 and abs(d.mean()) < 1e-15
     assert np.array_equal(d, W.gaussian_field(16, 20.0, 1000, 0.02))            # seeded
-    psi = W.displacement(d, 20.0)
+    psi = IC.displacement(d, 20.0)
     # div psi = -delta (spectral, away from the zeroed Nyquist planes): check in Fourier space
     dh = np.fft.fftn(d); k = 2 * np.pi / 20.0 * np.fft.fftfreq(16, 1 / 16.0)
     div = 1j * (k[None, None, :] * np.fft.fftn(psi[0]) + k[None, :, None] * np.fft.fftn(psi[1])
@@ -303,8 +303,33 @@ def test_workload_generators(W):
     rng = np.random.default_rng(0)
     d = W.gaussian_field(8, cfg.box, 3, 0.05)
     v = rng.standard_normal((8, 8, 8)); h = 1e-6
-    gp, pp = W.zeldovich_state(d + h * v, cfg); gm, pm = W.zeldovich_state(d - h * v, cfg)
+    gp, pp = IC.state_of(d + h * v, cfg, W); gm, pm = IC.state_of(d - h * v, cfg, W)
     cg = rng.standard_normal(gp.shape); cp = rng.standard_normal(pp.shape)
     lhs = (np.sum(cg * (gp - gm)) + np.sum(cp * (pp - pm))) / (2 * h)
-    rhs = np.sum(v * W.zeldovich_state_vjp(d, cfg, cg, cp))
+    rhs = np.sum(v * IC.state_vjp_of(d, cfg, W, cg, cp))
     assert abs(lhs - rhs) < 1e-6 * abs(lhs)
+
+
+@pytest.mark.parametrize("mode", [(1, 0, 0), (0, 2, 0), (2, -1, 3)])
+def test_ic_oracle_single_mode_analytic(IC, mode):
+    """Pin of oracle/ic.py against the closed form: delta = eps cos(k.x) gives psi = -eps (k / k^2) sin(k.x) (div psi =
+    -delta), positions q + psi/dx, w = vf psi, rho = f_b (1 + delta)."""
+    N, L, eps, f_b, vf, e0 = 16, 20.0, 0.03, 0.16, 7.0, 1e-3
+    c = (np.arange(N) + 0.5) * L / N
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+    k = 2 * np.pi / L * np.array(mode, dtype=float)
+    ph = k[0] * x + k[1] * y + k[2] * z
+    delta = eps * np.cos(ph)
+    gas, part = IC.zeldovich_state(delta, N, L, f_b, vf, e0)
+    psi = [-eps * k[d] / np.dot(k, k) * np.sin(ph) for d in range(3)]
+    q = [x / (L / N), y / (L / N), z / (L / N)]
+    for d in range(3):
+        want = (q[d] + psi[d] / (L / N)).ravel()
+        diff = part[d] - want
+        diff -= N * np.round(diff / N)
+        assert np.max(np.abs(diff)) < 1e-12
+        assert np.max(np.abs(part[3 + d] - vf * psi[d].ravel())) < 1e-12
+        assert np.max(np.abs(gas[1 + d] - f_b * (1 + delta) * vf * psi[d])) < 1e-12
+    assert np.max(np.abs(gas[0] - f_b * (1 + delta))) < 1e-15
+    v2 = vf * vf * sum(p * p for p in psi)
+    assert np.max(np.abs(gas[4] - f_b * (1 + delta) * (e0 + 0.5 * v2))) < 1e-12
