@@ -209,6 +209,16 @@ int dh_ic_zeldovich(dh_ctx* ctx, const float* delta_init, double a0, double vel_
 int dh_ic_zeldovich_vjp(dh_ctx* ctx, const float* delta_init, double vel_factor, double e_tilde0,
                         const dh_cot* cot_state, float* grad_delta);
 
+/* ---- the step on the output side: the data term of Eq. 27 and its cotangent ----
+ *   L = weight * sum_i (scale * O_i - data_i)^2 / noise_var_i        (Eq. 27: weight = 1/2)
+ * observable 0: O = rho_gas (the loss of BASELINE.json's configs, reading R21); 1: O = eps - |m|^2 / (2 rho), the
+ * internal energy density the paper's mock observable delta_b T is proportional to.
+ * gas, data, noise_var (NULL = 1 everywhere), cot_gas: DEVICE, N^3 floats each.  cot_gas (may be NULL) is OVERWRITTEN
+ * with dL/d(gas) -- the cot_final of dh_run_vjp (its particle cotangent is zero).  loss_out: HOST double, may be NULL;
+ * when given the call synchronises the stream, otherwise it is asynchronous. */
+int dh_data_term(dh_ctx* ctx, int observable, float* const gas[5], const float* data, const float* noise_var,
+                 double scale, double weight, float* const cot_gas[5], double* loss_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,4 +1,5 @@
-"""CPU ORACLE of the initial-condition map  delta_init -> (gas, particles)  and its transpose.
+"""CPU ORACLE of the two ends of the path: the initial-condition map  delta_init -> (gas, particles)  with its
+transpose, and (at the bottom) the data term of Eq. 27 with its cotangent.
 
 TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 --impl reference legs may import this module; it never imports the CUDA package and shares no code with it.
@@ -102,3 +103,28 @@ def coupled_ic(W, cfg, seed=None):
     delta = W.gaussian_field(cfg.N, cfg.box, cfg.seed if seed is None else seed, cfg.rms_delta)
     gas, part = state_of(delta, cfg, W)
     return delta, gas.astype(np.float32), part.astype(np.float32)
+
+
+# ------------------------------------------------------------------ output end: the data term of Eq. 27 ------
+def data_term(gas, data, noise_var=None, scale=1.0, weight=0.5, observable=0):
+    """PAPER.md:341, Eq. 27, first term:  L = weight sum_i (scale O_i - d_i)^2 / N_i  (Eq. 27: weight = 1/2) and
+    dL/d(gas) (5,N,N,N), fp64.  observable 0: O = rho (reading R21, the configs' loss); 1: O = eps - |m|^2/(2 rho), the
+    internal energy density the mock observable delta_b T is proportional to.
+    Pins (tests/test_oracle_pm.py): closed form on constant fields, central finite differences of L."""
+    g = np.asarray(gas, dtype=np.float64)
+    d = np.asarray(data, dtype=np.float64)
+    iv = 1.0 if noise_var is None else 1.0 / np.asarray(noise_var, dtype=np.float64)
+    rho, m, eps = g[0], g[1:4], g[4]
+    m2 = np.sum(m * m, axis=0)
+    obs = rho if observable == 0 else eps - 0.5 * m2 / rho
+    r = scale * obs - d
+    L = weight * np.sum(r * r * iv)
+    ob = 2.0 * weight * scale * r * iv
+    cot = np.zeros_like(g)
+    if observable == 0:
+        cot[0] = ob
+    else:
+        cot[0] = ob * 0.5 * m2 / rho ** 2
+        cot[1:4] = -ob[None] * m / rho[None]
+        cot[4] = ob
+    return L, cot

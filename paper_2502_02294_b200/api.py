@@ -28,7 +28,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_last_error", "dh_get_cmax", "dh_schedule_lna", "dh_step_scalars", "dh_debug_cell_index",
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
-           "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp"]
+           "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term"]
 
 
 class DhError(RuntimeError):
@@ -105,6 +105,7 @@ _lib.dh_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_double, _P3]
 _lib.dh_poisson_vjp.argtypes = [C.c_void_p, _P3, C.c_double, C.c_void_p]
 _lib.dh_kick_drift.argtypes = [C.c_void_p, _P3, _P6, C.c_double, C.c_double]
 _lib.dh_ic_zeldovich.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(dh_state)]
+_lib.dh_data_term.argtypes = [C.c_void_p, C.c_int, _P5, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, _dp]
 _lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
 
 
@@ -321,6 +322,16 @@ class Context:
                                     C.byref(cs)), "dh_ic_zeldovich")
         st.a, st.dt_prev, st.step = cs.a, cs.dt_prev, cs.step
         return st
+
+    def dh_data_term(self, observable: int, gas: torch.Tensor, data: torch.Tensor, noise_var: torch.Tensor | None = None,
+                     scale=1.0, weight=0.5, cot_gas: torch.Tensor | None = None, want_loss=True):
+        """L = weight sum (scale O - data)^2 / noise_var; fills cot_gas (5,N,N,N) if given; returns L (host) or None."""
+        loss = C.c_double(0.0)
+        cg = C.cast(_ptrs(cot_gas, 5, _P5), C.c_void_p) if cot_gas is not None else None
+        _check(_lib.dh_data_term(self._h, int(observable), _ptrs(gas, 5, _P5), data.data_ptr(),
+                                 noise_var.data_ptr() if noise_var is not None else None, float(scale), float(weight), cg,
+                                 C.byref(loss) if want_loss else None), "dh_data_term")
+        return loss.value if want_loss else None
 
     def dh_ic_zeldovich_vjp(self, delta_init: torch.Tensor, vel_factor, e_tilde0, cot_state: Cot) -> torch.Tensor:
         assert delta_init.is_cuda and delta_init.dtype == torch.float32 and delta_init.is_contiguous()

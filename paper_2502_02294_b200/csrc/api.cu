@@ -744,6 +744,24 @@ int dh_ic_zeldovich_vjp(dh_ctx* c, const float* delta_init, double vel_factor, d
     return DH_OK;
 }
 
+int dh_data_term(dh_ctx* c, int observable, float* const gas[5], const float* data, const float* noise_var, double scale,
+                 double weight, float* const cot_gas[5], double* loss_out) {
+    if (!c || !gas || !data || (observable != 0 && observable != 1)) {
+        set_error("dh_data_term: bad argument (observable is 0 = rho or 1 = internal energy density)");
+        return DH_ERR_INVALID;
+    }
+    for (int k = 0; k < 5; ++k)
+        if (!gas[k] || (cot_gas && !cot_gas[k])) { set_error("dh_data_term: null array %d", k); return DH_ERR_INVALID; }
+    double* loss_dev = c->scal_dev + 6;                                    // spare slot of the scalar accumulators
+    DH_CUDA(cudaMemsetAsync(loss_dev, 0, sizeof(double), c->stream));
+    DH_TRY(launch_data_term(c, observable, gas, data, noise_var, (float)scale, (float)weight, cot_gas, loss_dev));
+    if (loss_out) {
+        DH_CUDA(cudaMemcpyAsync(loss_out, loss_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        DH_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    return DH_OK;
+}
+
 int dh_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], double K, double dtau_over_dx) {
     if (!c || !part) { set_error("dh_kick_drift: bad argument"); return DH_ERR_INVALID; }
     return launch_kick_drift(c, g, part, part, (float)K, (float)dtau_over_dx);

@@ -198,6 +198,9 @@ int launch_ic_state(dh_ctx* c, const float* delta, float* const psi[3], float* c
 int launch_ic_state_vjp(dh_ctx* c, const float* delta, float* const psi[3], const float* const cot_gas[5],
                         const float* const cot_part[6], float* grad, float* const psi_b[3], float vf, float e0);
 
+int launch_data_term(dh_ctx* c, int observable, const float* const gas[5], const float* data, const float* noise_var,
+                     float scale, float weight, float* const cot[5], double* loss_dev);
+
 // ---- own FFT passes fused with the Green multiply (fft.cu) ----
 bool own_fft_supported(int N);
 int own_fft_init(dh_ctx* c);

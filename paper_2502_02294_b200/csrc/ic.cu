@@ -96,3 +96,80 @@ int launch_ic_state_vjp(dh_ctx* c, const float* delta, float* const psi[3], cons
 }
 
 }  // namespace dh
+
+// ------------------------------------------------------------------------------------------------ data term ----
+// The output end of the path: the noise-weighted squared error of Eq. 27,
+//   L = weight * sum_i (scale * O_i - d_i)^2 / N_i,    Eq. 27: weight = 1/2,
+// and its cotangent w.r.t. the gas state, in one pass (20 + 4 [+ 4] B/cell in, 20 out).  Observable O:
+//   0: gas density rho                                   (the loss of BASELINE.json's configs 0, 2-4, reading R21)
+//   1: internal energy density eps - |m|^2 / (2 rho)     ("delta_b T ... corresponds roughly to the internal energy
+//      density of the field"; = a^2 rho e in the tilde variables, the constant goes into `scale`)
+// The prior term of Eq. 27 acts on the input phases and is not part of this kernel.
+namespace dh {
+
+struct Gas5c { const float* p[5]; };
+struct Gas5m { float* p[5]; };
+
+template <int OBS, bool COT>
+__global__ void __launch_bounds__(256) data_term_kernel(Gas5c gas, const float* __restrict__ data,
+                                                        const float* __restrict__ noise_var, Gas5m cot, int64_t n,
+                                                        float scale, float weight, double* loss) {
+    __shared__ double sm[8];
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float rho = __ldg(gas.p[0] + i);
+        float obs, m[3] = {0.f, 0.f, 0.f}, rinv = 0.f;
+        if (OBS == 0) {
+            obs = rho;
+        } else {
+            rinv = 1.f / rho;
+            m[0] = __ldg(gas.p[1] + i); m[1] = __ldg(gas.p[2] + i); m[2] = __ldg(gas.p[3] + i);
+            obs = __ldg(gas.p[4] + i) - 0.5f * (m[0] * m[0] + m[1] * m[1] + m[2] * m[2]) * rinv;
+        }
+        const float r = fmaf(scale, obs, -__ldg(data + i));
+        const float iv = noise_var ? 1.f / __ldg(noise_var + i) : 1.f;
+        acc += (double)(r * r * iv);
+        if (COT) {
+            const float ob = 2.f * weight * scale * r * iv;          // dL / dO_i
+            if (OBS == 0) {
+                cot.p[0][i] = ob; cot.p[1][i] = 0.f; cot.p[2][i] = 0.f; cot.p[3][i] = 0.f; cot.p[4][i] = 0.f;
+            } else {
+                cot.p[0][i] = ob * 0.5f * (m[0] * m[0] + m[1] * m[1] + m[2] * m[2]) * rinv * rinv;
+                cot.p[1][i] = -ob * m[0] * rinv; cot.p[2][i] = -ob * m[1] * rinv; cot.p[3][i] = -ob * m[2] * rinv;
+                cot.p[4][i] = ob;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) atomicAdd(loss, (double)weight * v);
+    }
+}
+
+int launch_data_term(dh_ctx* c, int observable, const float* const gas[5], const float* data, const float* noise_var,
+                     float scale, float weight, float* const cot[5], double* loss_dev) {
+    Gas5c g; Gas5m q;
+    for (int k = 0; k < 5; ++k) { g.p[k] = gas[k]; q.p[k] = cot ? cot[k] : nullptr; }
+    const int64_t n = c->n3;
+    int64_t blocks = (n + 255) / 256;
+    const int64_t cap = (int64_t)c->sm_count * 8;
+    const unsigned grid = (unsigned)(blocks < cap ? blocks : cap);
+    if (observable == 0) {
+        if (cot) data_term_kernel<0, true><<<grid, 256, 0, c->stream>>>(g, data, noise_var, q, n, scale, weight, loss_dev);
+        else data_term_kernel<0, false><<<grid, 256, 0, c->stream>>>(g, data, noise_var, q, n, scale, weight, loss_dev);
+    } else {
+        if (cot) data_term_kernel<1, true><<<grid, 256, 0, c->stream>>>(g, data, noise_var, q, n, scale, weight, loss_dev);
+        else data_term_kernel<1, false><<<grid, 256, 0, c->stream>>>(g, data, noise_var, q, n, scale, weight, loss_dev);
+    }
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+}  // namespace dh

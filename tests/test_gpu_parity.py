@@ -467,6 +467,27 @@ def test_ic_map_rejects_wrong_setups(api, torch_, W):
     ctx.close()
 
 
+@pytest.mark.parametrize("observable", [0, 1])
+def test_data_term_matches_oracle(api, torch_, W, IC, observable):
+    """dh_data_term (Eq. 27 data term and its cotangent) against oracle/ic.py on an evolved-looking gas state."""
+    N = 64
+    cfg = W.scaled_config(0, N, rms_delta=0.05)
+    _, gas, _ = IC.coupled_ic(W, cfg)
+    rng = np.random.default_rng(observable)
+    scale = 1.0 if observable == 0 else 1.0 / cfg.e_tilde0()
+    data = rng.standard_normal((N, N, N)).astype(np.float32)
+    nv = (1.0 + rng.uniform(size=(N, N, N))).astype(np.float32)
+    L_ref, cot_ref = IC.data_term(gas, data, nv, scale, 0.5, observable)
+    ctx = api.context_for(cfg)
+    cot = torch_.empty((5, N, N, N), device="cuda")
+    L = ctx.dh_data_term(observable, _gpu(torch_, gas), _gpu(torch_, data), _gpu(torch_, nv), scale, 0.5, cot)
+    assert abs(L / L_ref - 1) < 1e-5
+    assert PT.rel_l2(cot.cpu().numpy(), cot_ref) < 1e-5
+    L2 = ctx.dh_data_term(observable, _gpu(torch_, gas), _gpu(torch_, data), None, scale, 1.0, None)
+    assert abs(L2 / IC.data_term(gas, data, None, scale, 1.0, observable)[0] - 1) < 1e-5
+    ctx.close()
+
+
 def test_reverse_pass_storage_policies_agree(api, torch_, W, IC):
     """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
     ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two

@@ -333,3 +333,21 @@ def test_ic_oracle_single_mode_analytic(IC, mode):
     assert np.max(np.abs(gas[0] - f_b * (1 + delta))) < 1e-15
     v2 = vf * vf * sum(p * p for p in psi)
     assert np.max(np.abs(gas[4] - f_b * (1 + delta) * (e0 + 0.5 * v2))) < 1e-12
+
+
+@pytest.mark.parametrize("observable", [0, 1])
+def test_data_term_oracle_closed_form_and_finite_differences(IC, observable):
+    """Pins of oracle/ic.py data_term (Eq. 27): constant fields give weight n (scale O - d)^2 / N in closed
+    form; the cotangent equals the central finite difference of L along a random direction."""
+    n = 6
+    gas = np.zeros((5, n, n, n)); gas[0] = 2.0; gas[1] = 1.0; gas[2] = -2.0; gas[3] = 0.5; gas[4] = 7.0
+    O = 2.0 if observable == 0 else 7.0 - 0.5 * (1 + 4 + 0.25) / 2.0
+    L, cot = IC.data_term(gas, np.full((n, n, n), 1.5), np.full((n, n, n), 4.0), scale=3.0, weight=0.5, observable=observable)
+    assert abs(L - 0.5 * n ** 3 * (3.0 * O - 1.5) ** 2 / 4.0) < 1e-10
+    rng = np.random.default_rng(3)
+    gas = gas + 0.1 * rng.standard_normal(gas.shape)
+    d = rng.standard_normal((n, n, n)); nv = 1.0 + rng.uniform(size=(n, n, n))
+    v = rng.standard_normal(gas.shape); h = 1e-6
+    Lp, _ = IC.data_term(gas + h * v, d, nv, 1.3, 0.5, observable); Lm, _ = IC.data_term(gas - h * v, d, nv, 1.3, 0.5, observable)
+    _, cot = IC.data_term(gas, d, nv, 1.3, 0.5, observable)
+    assert abs((Lp - Lm) / (2 * h) - np.sum(cot * v)) < 1e-7 * abs(np.sum(cot * v))
