@@ -301,6 +301,41 @@ def test_config3_full_size_step_and_vjp(api, torch_, O, W, IC):
     ctx.close()
 
 
+def test_config4_full_size_properties(api, torch_, W):
+    """Config 4 at its full size (512^3 cells and particles, beyond what the fp64 oracle holds in seconds): properties
+    that hold at any size.  State from dh_ic_zeldovich; one coupled step: gas mass conserved to round-off, particles stay
+    in [0, N), every value finite, CFL maxima positive; the Poisson source has zero mean and so has every g' component;
+    a second run of the same step agrees to the deposit's atomic order (5e-6)."""
+    cfg = W.CONFIGS[4]
+    N = cfg.N
+    delta = torch_.from_numpy(W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)).cuda()
+    ctx = api.context_for(cfg)
+    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+    st0 = ctx.dh_ic_zeldovich(delta, cfg.a0, vf, e0)
+    assert abs(float(st0.gas[0].double().mean()) / cfg.f_b - 1) < 1e-6            # delta has zero mean
+    src = ctx.dh_deposit(st0.gas[0], st0.part[:3].contiguous())
+    assert abs(float(src.double().mean())) < 1e-6                                  # all mass deposited: mean-free source
+    g = ctx.dh_poisson(src, 1.5 * cfg.Omega_m * cfg.H0 ** 2)
+    gmax = float(g.abs().max())
+    assert all(abs(float(g[d].double().mean())) < 1e-6 * gmax for d in range(3))
+    del src, g
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    outs = []
+    for _ in range(2):
+        st = st0.clone()
+        cm = torch_.zeros(3, device="cuda")
+        ctx.dh_step(st, dt_s[0], a_s[1], cm)
+        assert bool(torch_.isfinite(st.gas).all()) and bool(torch_.isfinite(st.part).all())
+        assert abs(float(st.gas[0].double().sum()) / float(st0.gas[0].double().sum()) - 1) < 1e-7
+        assert float(st.part[:3].min()) >= 0.0 and float(st.part[:3].max()) < N
+        assert float(cm.min()) > 0.0
+        outs.append(st)
+    for k in range(5):
+        scale = float(outs[0].gas[k].abs().max())
+        assert float((outs[0].gas[k] - outs[1].gas[k]).abs().max()) <= 5e-6 * scale
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------------ adjoint
 @pytest.mark.parametrize("N", [32, 64])
 @pytest.mark.parametrize("d", [0, 1, 2])
