@@ -219,6 +219,15 @@ int dh_ic_zeldovich_vjp(dh_ctx* ctx, const float* delta_init, double vel_factor,
 int dh_data_term(dh_ctx* ctx, int observable, float* const gas[5], const float* data, const float* noise_var,
                  double scale, double weight, float* const cot_gas[5], double* loss_out);
 
+/* Binned power spectrum of a real mesh field and its transpose ("power spectra of the baryon density
+ * using a differentiable routine").  With F = FFT3(field), n the integer wave vector and
+ * bin b = round(|n|), b = 1 .. N/2:   P_b = (box^3 / N^6) sum_{k in b} |F_k|^2 / count_b   (sums over the full spectrum),
+ * k_b = 2 pi b / box.  field: DEVICE, N^3 floats, not modified.  power_out, count_out (may be NULL), power_bar: HOST,
+ * N/2 doubles, index b - 1.  field_bar: DEVICE, N^3 floats, OVERWRITTEN with sum_b power_bar_b dP_b/dfield.
+ * Both calls synchronise the stream.  Need gravity_on and a power-of-two grid, else DH_ERR_INVALID. */
+int dh_power_spectrum(dh_ctx* ctx, const float* field, double* power_out, double* count_out);
+int dh_power_spectrum_vjp(dh_ctx* ctx, const float* field, const double* power_bar, float* field_bar);
+
 #ifdef __cplusplus
 }
 #endif

@@ -128,3 +128,37 @@ def data_term(gas, data, noise_var=None, scale=1.0, weight=0.5, observable=0):
         cot[1:4] = -ob[None] * m / rho[None]
         cot[4] = ob
     return L, cot
+
+
+# ------------------------------------------------------------------ output end: binned power spectrum ------
+def _ps_bins(N):
+    n1 = np.fft.fftfreq(N, d=1.0 / N)
+    nz = n1[:, None, None]; ny = n1[None, :, None]; nx = n1[None, None, :]
+    return np.rint(np.sqrt(nx * nx + ny * ny + nz * nz)).astype(np.int64)      # full spectrum, [z][y][x]
+
+
+def power_spectrum(field, L):
+    """PAPER.md:310 ("power spectra of the baryon density"): with F = FFT3(field) over the FULL spectrum and bins
+    b = round(|n|), b = 1 .. N/2:  P_b = (L^3 / N^6) sum_{k in b} |F_k|^2 / count_b.  Returns (P, count), index b - 1.
+    Pins (tests/test_oracle_pm.py): a single cosine puts (amplitude^2 L^3 / 4) * 2 / count_b into exactly its own bin;
+    sum_b count_b P_b + the dropped modes = Parseval; central finite differences of the transpose."""
+    f = np.asarray(field, dtype=np.float64)
+    N = f.shape[0]
+    F2 = np.abs(np.fft.fftn(f)) ** 2
+    b = _ps_bins(N).ravel()
+    nb = N // 2
+    s = np.bincount(b, weights=F2.ravel(), minlength=nb + 1)[1:nb + 1]
+    cnt = np.bincount(b, minlength=nb + 1)[1:nb + 1].astype(np.float64)
+    return (L ** 3 / float(N) ** 6) * s / cnt, cnt
+
+
+def power_spectrum_vjp(field, L, power_bar):
+    """sum_b power_bar_b dP_b/dfield:  d/df(x) sum_k g_k |F_k|^2 = 2 N^3 IFFT3(g F)(x),  g_k = (L^3/N^6) power_bar_b / count_b."""
+    f = np.asarray(field, dtype=np.float64)
+    N = f.shape[0]
+    nb = N // 2
+    b = _ps_bins(N)
+    cnt = np.bincount(b.ravel(), minlength=nb + 1).astype(np.float64)
+    g = np.zeros(b.max() + 1)
+    g[1:nb + 1] = (L ** 3 / float(N) ** 6) * np.asarray(power_bar, dtype=np.float64) / cnt[1:nb + 1]
+    return 2.0 * N ** 3 * np.real(np.fft.ifftn(g[b] * np.fft.fftn(f)))

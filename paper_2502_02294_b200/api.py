@@ -28,7 +28,8 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_last_error", "dh_get_cmax", "dh_schedule_lna", "dh_step_scalars", "dh_debug_cell_index",
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
-           "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term"]
+           "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
+           "dh_power_spectrum_vjp"]
 
 
 class DhError(RuntimeError):
@@ -106,6 +107,8 @@ _lib.dh_poisson_vjp.argtypes = [C.c_void_p, _P3, C.c_double, C.c_void_p]
 _lib.dh_kick_drift.argtypes = [C.c_void_p, _P3, _P6, C.c_double, C.c_double]
 _lib.dh_ic_zeldovich.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(dh_state)]
 _lib.dh_data_term.argtypes = [C.c_void_p, C.c_int, _P5, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, _dp]
+_lib.dh_power_spectrum.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
+_lib.dh_power_spectrum_vjp.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p]
 _lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
 
 
@@ -322,6 +325,22 @@ class Context:
                                     C.byref(cs)), "dh_ic_zeldovich")
         st.a, st.dt_prev, st.step = cs.a, cs.dt_prev, cs.step
         return st
+
+    def dh_power_spectrum(self, field: torch.Tensor):
+        """(P_b, count_b), b = 1 .. N/2, as host float64 arrays."""
+        nb = self.N // 2
+        P = np.zeros(nb); cnt = np.zeros(nb)
+        _check(_lib.dh_power_spectrum(self._h, field.data_ptr(), P.ctypes.data_as(_dp), cnt.ctypes.data_as(_dp)),
+               "dh_power_spectrum")
+        return P, cnt
+
+    def dh_power_spectrum_vjp(self, field: torch.Tensor, power_bar) -> torch.Tensor:
+        pb = np.ascontiguousarray(power_bar, dtype=np.float64)
+        assert pb.shape == (self.N // 2,)
+        out = torch.empty_like(field)
+        _check(_lib.dh_power_spectrum_vjp(self._h, field.data_ptr(), pb.ctypes.data_as(_dp), out.data_ptr()),
+               "dh_power_spectrum_vjp")
+        return out
 
     def dh_data_term(self, observable: int, gas: torch.Tensor, data: torch.Tensor, noise_var: torch.Tensor | None = None,
                      scale=1.0, weight=0.5, cot_gas: torch.Tensor | None = None, want_loss=True):

@@ -382,7 +382,7 @@ int dh_free(dh_ctx* c) {
     for (auto p : c->gpb) cudaFree(p);
     for (auto p : c->cot_tmp) cudaFree(p);
     for (auto p : c->part_tmp) cudaFree(p);
-    cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev);
+    cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev); cudaFree(c->ps_bins);
     cudaFree(c->hv_state); cudaFree(c->hv_cot);
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
@@ -741,6 +741,53 @@ int dh_ic_zeldovich_vjp(dh_ctx* c, const float* delta_init, double vel_factor, d
                                (float)vel_factor, (float)e_tilde0));
     DH_TRY(poisson_adjoint(c, c->gpb, 1.f, c->delta));
     DH_TRY(launch_axpy(c, c->delta, grad_delta, 1.f));
+    return DH_OK;
+}
+
+static int ps_scratch(dh_ctx* c, const char* who) {
+    if (!c->opt.gravity_on || !c->own_fft) {
+        set_error("%s: needs gravity_on and a power-of-two grid in [32, 1024] (the own FFT passes)", who);
+        return DH_ERR_INVALID;
+    }
+    const int nb1 = c->N / 2 + 1;
+    if (!c->ps_bins) DH_TRY(dev_alloc(c, (void**)&c->ps_bins, (size_t)nb1 * (2 * sizeof(double) + sizeof(float))));
+    return DH_OK;
+}
+
+int dh_power_spectrum(dh_ctx* c, const float* field, double* power_out, double* count_out) {
+    if (!c || !field || !power_out) { set_error("dh_power_spectrum: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(ps_scratch(c, "dh_power_spectrum"));
+    const int nb1 = c->N / 2 + 1;
+    DH_CUDA(cudaMemsetAsync(c->ps_bins, 0, (size_t)2 * nb1 * sizeof(double), c->stream));
+    DH_TRY(own_power_spectrum(c, field, c->ps_bins));
+    std::vector<double> h(2 * nb1);
+    DH_CUDA(cudaMemcpyAsync(h.data(), c->ps_bins, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    const double norm = c->box * c->box * c->box / ((double)c->n3 * (double)c->n3);
+    for (int b = 1; b < nb1; ++b) {
+        power_out[b - 1] = h[nb1 + b] > 0 ? norm * h[b] / h[nb1 + b] : 0.0;
+        if (count_out) count_out[b - 1] = h[nb1 + b];
+    }
+    return DH_OK;
+}
+
+int dh_power_spectrum_vjp(dh_ctx* c, const float* field, const double* power_bar, float* field_bar) {
+    if (!c || !field || !power_bar || !field_bar) { set_error("dh_power_spectrum_vjp: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(ps_scratch(c, "dh_power_spectrum_vjp"));
+    const int nb1 = c->N / 2 + 1;
+    // mode counts per bin (a property of the grid): one pass of the forward kernel gives them
+    DH_CUDA(cudaMemsetAsync(c->ps_bins, 0, (size_t)2 * nb1 * sizeof(double), c->stream));
+    DH_TRY(own_power_spectrum(c, field, c->ps_bins));
+    std::vector<double> h(2 * nb1);
+    DH_CUDA(cudaMemcpyAsync(h.data(), c->ps_bins, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    const double norm = c->box * c->box * c->box / ((double)c->n3 * (double)c->n3);
+    std::vector<float> g(nb1, 0.f);
+    for (int b = 1; b < nb1; ++b) g[b] = h[nb1 + b] > 0 ? (float)(2.0 * norm * power_bar[b - 1] / h[nb1 + b]) : 0.f;
+    float* gtab = reinterpret_cast<float*>(c->ps_bins + 2 * nb1);
+    DH_CUDA(cudaMemcpyAsync(gtab, g.data(), nb1 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));             // g is a local: the copy must finish before it goes away
+    DH_TRY(own_power_spectrum_adjoint(c, field, gtab, field_bar));
     return DH_OK;
 }
 

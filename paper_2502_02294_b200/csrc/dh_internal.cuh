@@ -113,6 +113,7 @@ struct dh_ctx {
     float* cmax_log = nullptr;     // 3 * cmax_cap floats
     int cmax_cap = 0;
     int cmax_n = 0;
+    double* ps_bins = nullptr;     // power spectrum: [2][N/2+1] doubles + (behind them) N/2+1 floats of the transpose's table
     double* scal_dev = nullptr;    // 8 doubles: (lam_b, kap_b, gamma_b, K_b, dtau_drift_b, A_b, spare, spare)
 
     // adjoint scratch (allocated on first use)
@@ -206,6 +207,8 @@ bool own_fft_supported(int N);
 int own_fft_init(dh_ctx* c);
 int own_poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]);
 int own_poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar);
+int own_power_spectrum(dh_ctx* c, const float* field, double* bins_dev /* [2][N/2+1]: sum w |F|^2, sum w */);
+int own_power_spectrum_adjoint(dh_ctx* c, const float* field, const float* gtab_dev /* [N/2+1] */, float* field_bar);
 
 int poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_out[3]);
 int poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar);

@@ -406,6 +406,102 @@ __global__ void __launch_bounds__(PP * Plan<N>::T, (N <= 256 ? 2 : 1)) fft_z_gre
     store_A<N>(acc, dbhat + off, tl.es, t);
 }
 
+// ------------------------------------------------------------------------------------------ power spectrum ----
+// Binned power spectrum of a real field ("power spectra of the baryon density using a differentiable
+// routine") on the same passes: x R2C -> y C2C -> [ z C2C -> |F|^2 into bins ].
+//   bin b = round(|n|), n = integer wave vector, 1 <= b <= N/2;  P_b = (L^3 / N^6) sum_{k in b} |F_k|^2 / count_b,
+// the sums over the FULL spectrum: a half-spectrum element counts twice unless kx = 0 or kx = N/2.
+// Transpose: field_bar = 2 IFFT3_unnormalised( g_b(k) F_k ), g_b = (L^3 / N^6) P_bar_b / count_b -- the fused z pass of the
+// Poisson solve with a real, bin-indexed symbol and one component.
+__device__ __forceinline__ int ps_bin(int ix, int iy, int iz, int N) {
+    const int ny = kint(iy, N), nz = kint(iz, N);
+    const int n2 = ix * ix + ny * ny + nz * nz;
+    return (int)(sqrtf((float)n2) + 0.5f);         // exact: sqrt(n2) is never within 2.8e-4 of a half-integer for N <= 1024
+}
+
+template <int N>
+__global__ void __launch_bounds__(PP * Plan<N>::T, (N <= 256 ? 2 : 1)) fft_z_power_kernel(const float2* __restrict__ fhat,
+                                                                      const float2* __restrict__ tw_g,
+                                                                      double* __restrict__ bins /* [2][N/2 + 1] */) {
+    using PN = Pencil<N>;
+    using P = Plan<N>;
+    constexpr int E = PN::E, NTHR = PP * PN::T, NB = N / 2 + 1;
+    extern __shared__ float smem_f[];
+    __shared__ float hist[2 * NB];
+    float2* tw = reinterpret_cast<float2*>(smem_f);
+    float* ex_re = smem_f + 2 * N;
+    float* ex_im = ex_re + PN::EX * PP;
+    load_tw<N>(tw, tw_g, NTHR);
+    for (int j = threadIdx.x; j < 2 * NB; j += NTHR) hist[j] = 0.f;
+    const int p = threadIdx.x % PP, t = threadIdx.x / PP;
+    const Tile tl = z_tile(blockIdx.x, N);
+    const long off = tl.base + (long)p * tl.ps;
+    const int ix = tl.nyq ? N / 2 : tl.i1 + p, iy = tl.nyq ? tl.i0 + p : tl.i0;
+    const float w = (ix == 0 || ix == N / 2) ? 1.f : 2.f;
+    float2 b[E];
+    load_A<N>(b, fhat + off, tl.es, t);
+    __syncthreads();
+    PN::fwd1(b, t, ex_re + p, ex_im + p, PP, tw, 1);
+    __syncthreads();
+    PN::fwd2(b, t, ex_re + p, ex_im + p, PP);          // b[s R2 + j] = F(kz = k1 + R1 brev(j))
+#pragma unroll
+    for (int s = 0; s < P::S2; ++s)
+#pragma unroll
+        for (int k2 = 0; k2 < P::R2; ++k2) {
+            const int bin = ps_bin(ix, iy, t + P::T * s + P::R1 * k2, N);
+            const float2 v = b[s * P::R2 + brev<P::R2>(k2)];
+            if (bin >= 1 && bin <= N / 2) {
+                atomicAdd(&hist[bin], w * fmaf(v.x, v.x, v.y * v.y));
+                atomicAdd(&hist[NB + bin], w);
+            }
+        }
+    __syncthreads();
+    for (int j = threadIdx.x; j < 2 * NB; j += NTHR)
+        if (hist[j] != 0.f) atomicAdd(bins + j, (double)hist[j]);
+}
+
+// z pass of the transpose: F -> z C2C -> times gtab[bin] -> z C2C^-1, in place
+template <int N>
+__global__ void __launch_bounds__(PP * Plan<N>::T, (N <= 256 ? 2 : 1)) fft_z_power_adj_kernel(float2* __restrict__ fhat,
+                                                                          const float2* __restrict__ tw_g,
+                                                                          const float* __restrict__ gtab_g /* [N/2 + 1] */) {
+    using PN = Pencil<N>;
+    using P = Plan<N>;
+    constexpr int E = PN::E, NTHR = PP * PN::T, NB = N / 2 + 1;
+    extern __shared__ float smem_f[];
+    __shared__ float gtab[NB];
+    float2* tw = reinterpret_cast<float2*>(smem_f);
+    float* ex_re = smem_f + 2 * N;
+    float* ex_im = ex_re + PN::EX * PP;
+    load_tw<N>(tw, tw_g, NTHR);
+    for (int j = threadIdx.x; j < NB; j += NTHR) gtab[j] = gtab_g[j];
+    const int p = threadIdx.x % PP, t = threadIdx.x / PP;
+    const Tile tl = z_tile(blockIdx.x, N);
+    const long off = tl.base + (long)p * tl.ps;
+    const int ix = tl.nyq ? N / 2 : tl.i1 + p, iy = tl.nyq ? tl.i0 + p : tl.i0;
+    float2 b[E];
+    load_A<N>(b, fhat + off, tl.es, t);
+    __syncthreads();
+    PN::fwd1(b, t, ex_re + p, ex_im + p, PP, tw, 1);
+    __syncthreads();
+    PN::fwd2(b, t, ex_re + p, ex_im + p, PP);
+    float2 c[E];
+#pragma unroll
+    for (int s = 0; s < P::S2; ++s)
+#pragma unroll
+        for (int k2 = 0; k2 < P::R2; ++k2) {
+            const int bin = ps_bin(ix, iy, t + P::T * s + P::R1 * k2, N);
+            const float g = (bin >= 1 && bin <= N / 2) ? gtab[bin] : 0.f;
+            const float2 v = b[s * P::R2 + brev<P::R2>(k2)];
+            c[s * P::R2 + k2] = make_float2(g * v.x, g * v.y);
+        }
+    __syncthreads();
+    PN::inv1(c, t, ex_re + p, ex_im + p, PP, tw, 1);
+    __syncthreads();
+    PN::inv2(c, t, ex_re + p, ex_im + p, PP);
+    store_A<N>(c, fhat + off, tl.es, t);
+}
+
 // ---------------------------------------------------------------------------------------------- x passes ----
 // A real row r[0 .. N) is transformed through the M = N/2 point complex transform of z[n] = r[2n] + i r[2n+1]:
 //   X[k] = (Z[k] + conj Z[M-k]) / 2 - (i/2) w_N^k (Z[k] - conj Z[M-k]),  k = 0 .. M  (Z[M] = Z[0]),  w_N = exp(-2 pi i / N)
@@ -616,6 +712,49 @@ static int own_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_b
     return DH_OK;
 }
 
+// x and y forward passes of `field` into spec[0]
+template <int N>
+static int own_xy_forward(dh_ctx* c, const float* field) {
+    using C = RowCfg<N>;
+    Spec3 s0{{c->spec[0], c->spec[0], c->spec[0]}};
+    const unsigned row_blocks = (unsigned)((long)N * N / C::RB), tiles = (unsigned)tiles_per_pass(N);
+    DH_CUDA(cudaFuncSetAttribute(fft_x_r2c_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+    DH_CUDA(cudaFuncSetAttribute(fft_y_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem<N>()));
+    fft_x_r2c_kernel<N><<<dim3(row_blocks, 1), C::NTHR, C::SMEM, c->stream>>>(field, field, field, s0, c->fft_tw);
+    fft_y_kernel<N, false><<<dim3(tiles, 1), PP * Plan<N>::T, tile_smem<N>(), c->stream>>>(s0, c->fft_tw);
+    c->launches += 2;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+template <int N>
+static int own_power(dh_ctx* c, const float* field, double* bins_dev) {
+    DH_TRY(own_xy_forward<N>(c, field));
+    DH_CUDA(cudaFuncSetAttribute(fft_z_power_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem<N>()));
+    fft_z_power_kernel<N><<<(unsigned)tiles_per_pass(N), PP * Plan<N>::T, tile_smem<N>(), c->stream>>>(c->spec[0], c->fft_tw,
+                                                                                                      bins_dev);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+template <int N>
+static int own_power_adj(dh_ctx* c, const float* field, const float* gtab_dev, float* field_bar) {
+    using C = RowCfg<N>;
+    DH_TRY(own_xy_forward<N>(c, field));
+    Spec3 s0{{c->spec[0], c->spec[0], c->spec[0]}};
+    const unsigned row_blocks = (unsigned)((long)N * N / C::RB), tiles = (unsigned)tiles_per_pass(N);
+    DH_CUDA(cudaFuncSetAttribute(fft_z_power_adj_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem<N>()));
+    DH_CUDA(cudaFuncSetAttribute(fft_y_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem<N>()));
+    DH_CUDA(cudaFuncSetAttribute(fft_x_c2r_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+    fft_z_power_adj_kernel<N><<<tiles, PP * Plan<N>::T, tile_smem<N>(), c->stream>>>(c->spec[0], c->fft_tw, gtab_dev);
+    fft_y_kernel<N, true><<<dim3(tiles, 1), PP * Plan<N>::T, tile_smem<N>(), c->stream>>>(s0, c->fft_tw);
+    fft_x_c2r_kernel<N><<<dim3(row_blocks, 1), C::NTHR, C::SMEM, c->stream>>>(s0, field_bar, field_bar, field_bar, c->fft_tw);
+    c->launches += 3;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
 #define DH_FFT_DISPATCH(FN, ...)                           \
     switch (c->N) {                                        \
         case 32: return FN<32>(__VA_ARGS__);               \
@@ -632,6 +771,12 @@ int own_poisson_forward(dh_ctx* c, const float* delta, float A, float* const g_o
 }
 int own_poisson_adjoint(dh_ctx* c, float* const g_bar[3], float A, float* delta_bar) {
     DH_FFT_DISPATCH(own_adjoint, c, g_bar, A, delta_bar)
+}
+int own_power_spectrum(dh_ctx* c, const float* field, double* bins_dev) {
+    DH_FFT_DISPATCH(own_power, c, field, bins_dev)
+}
+int own_power_spectrum_adjoint(dh_ctx* c, const float* field, const float* gtab_dev, float* field_bar) {
+    DH_FFT_DISPATCH(own_power_adj, c, field, gtab_dev, field_bar)
 }
 
 // (cos, sin)(2 pi j / N), j = 0 .. N-1, computed in double on the host

@@ -351,3 +351,28 @@ def test_data_term_oracle_closed_form_and_finite_differences(IC, observable):
     Lp, _ = IC.data_term(gas + h * v, d, nv, 1.3, 0.5, observable); Lm, _ = IC.data_term(gas - h * v, d, nv, 1.3, 0.5, observable)
     _, cot = IC.data_term(gas, d, nv, 1.3, 0.5, observable)
     assert abs((Lp - Lm) / (2 * h) - np.sum(cot * v)) < 1e-7 * abs(np.sum(cot * v))
+
+
+def test_power_spectrum_oracle_single_mode_parseval_and_transpose(IC):
+    """Pins of oracle/ic.py power_spectrum: f = A cos(k.x) with |n| = 3 has |F|^2 = (A N^3 / 2)^2 at +-k only, so
+    P_3 = 2 (A/2)^2 L^3 / count_3 and every other bin is empty; Parseval over all bins of a random field (the corner
+    modes beyond N/2 and the mean are added back); the transpose against central finite differences."""
+    N, L, A = 16, 20.0, 0.7
+    c = (np.arange(N) + 0.5) / N
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+    f = A * np.cos(2 * np.pi * (2 * x + 2 * y - 1 * z))                         # |n| = 3 exactly
+    P, cnt = IC.power_spectrum(f, L)
+    assert abs(P[2] - 2 * (A / 2) ** 2 * L ** 3 / cnt[2]) < 1e-12 * P[2]
+    assert np.max(np.abs(np.delete(P, 2))) < 1e-20
+    assert cnt[0] == 18 and cnt[1] == 62                                         # |n| rounds to 1: 6 + 12 modes; to 2: 62
+    rng = np.random.default_rng(0)
+    f = rng.standard_normal((N, N, N))
+    P, cnt = IC.power_spectrum(f, L)
+    F2 = np.abs(np.fft.fftn(f)) ** 2
+    b = IC._ps_bins(N)
+    rest = F2[(b == 0) | (b > N // 2)].sum()
+    assert abs((np.sum(P * cnt) * N ** 6 / L ** 3 + rest) / (N ** 3 * np.sum(f * f)) - 1) < 1e-12
+    pb = rng.standard_normal(N // 2); v = rng.standard_normal(f.shape); h = 1e-6
+    lhs = np.sum(pb * (IC.power_spectrum(f + h * v, L)[0] - IC.power_spectrum(f - h * v, L)[0])) / (2 * h)
+    rhs = np.sum(v * IC.power_spectrum_vjp(f, L, pb))
+    assert abs(lhs - rhs) < 1e-7 * abs(lhs)
