@@ -6,7 +6,7 @@ recipes only (numpy on the host) -- none of the step's arithmetic, no CUDA, no o
     (stand-in for the paper's Eisenstein-Hu + LPT initial conditions, PAPER.md:49; reading R19 in DESIGN.md);
     -- the field is the input; the Zel'dovich map  delta -> (gas, particles)  is part of the method: the CUDA path does
     it on the device (dh_ic_zeldovich), the oracle in oracle/ic.py;
-  * the spherical Sod-type Riemann problem of config 1 and a 1-D Sod tube;
+  * the spherical Sod-type Riemann problem of config 1, a 1-D Sod tube and the paper's Sedov blast (PAPER.md:177-196);
   * the config table and the (a, dt) schedule in ln a for an EdS cosmology.
 Units (reading R18): length h^-1 Mpc, velocity km/s, H0 = 100, density in units of the mean comoving total
 matter density, positions in grid units [0, N).
@@ -137,6 +137,22 @@ def sod_sphere(N: int, gamma: float = 1.4, r0: float = 0.2):
     gas[0] = rho
     gas[4] = p / (gamma - 1.0)
     return gas.astype(np.float32)
+
+
+def sedov_ic(N: int, gamma: float = 5.0 / 3.0, E0: float = 1.0, rho1: float = 1.0, p0: float = 1e-5):
+    """Sedov-Taylor blast: uniform density rho1, negligible pressure p0, energy E0 in the central cell
+    (cell units: dx = 1, box = N).  gas (5,N,N,N) f32."""
+    gas = np.zeros((5, N, N, N))
+    gas[0] = rho1
+    gas[4] = p0 / (gamma - 1.0)
+    c = N // 2
+    gas[4, c, c, c] += E0
+    return gas.astype(np.float32)
+
+
+def sedov_time(r_sh: float, E0: float = 1.0, rho1: float = 1.0, phi0: float = 1.15) -> float:
+    """Time at which Eq. 21, r_sh = phi0 (E0 t^2 / rho1)^(1/5), reaches r_sh."""
+    return float(np.sqrt((r_sh / phi0) ** 5 * rho1 / E0))
 
 
 def sod_tube(nx: int, gamma: float = 1.4, axis: int = 0, ny: int = 1, nz: int = 1, mirror: bool = False):

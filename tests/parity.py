@@ -49,3 +49,38 @@ def oracle_params(O, cfg, **kw):
                 static_mode=cfg.static_mode, gravity_on=cfg.gravity_on, e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
     args.update(kw)
     return O.make_params(cfg.N, cfg.box, cfg.gamma, **args)
+
+
+def shock_radii(rho):
+    """Position of the density maximum of a centred blast wave (cell units): along the angle-averaged radial profile
+    (0.5-cell bins) and along 9 rays (axes, face and body diagonals).  Returns (profile_peak, ray_min, ray_max)."""
+    rho = np.asarray(rho, dtype=np.float64)
+    N = rho.shape[0]
+    c = N // 2
+    q = np.arange(N) + 0.5 - (c + 0.5)
+    z, y, x = np.meshgrid(q, q, q, indexing="ij")
+    r = np.sqrt(x * x + y * y + z * z)
+    bins = np.arange(0, N // 2, 0.5)
+    idx = np.digitize(r.ravel(), bins)
+    prof = np.bincount(idx, weights=rho.ravel(), minlength=len(bins) + 1) / np.maximum(np.bincount(idx, minlength=len(bins) + 1), 1)
+    peak = bins[np.argmax(prof[1:])] + 0.25
+    rays = []
+    for dv in [(1, 0, 0), (0, 1, 0), (0, 0, 1), (1, 1, 0), (1, 0, 1), (0, 1, 1), (1, 1, 1), (-1, 1, 0), (1, -1, 1)]:
+        dv = np.array(dv, float) / np.linalg.norm(dv)
+        ss = np.arange(0, N / 2 - 2, 0.25)
+        ii = np.floor((c + 0.5) + np.outer(ss, dv)).astype(int)
+        rays.append(ss[np.argmax(rho[ii[:, 2], ii[:, 1], ii[:, 0]])])
+    return peak, min(rays), max(rays)
+
+
+def golden(name):
+    """A text fixture under tests/golden/ (name value per line, '#' comments carry the citation) as a dict of floats."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)) as f:
+        for line in f:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                k, v = line.split()[:2]
+                out[k] = float(v)
+    return out

@@ -216,3 +216,28 @@ def test_cfl_maximum_is_max_freezing_speed(O):
     for d, expect in ((0, max(cs_bg, cs_hot)), (1, 3.0 + cs_hot), (2, max(cs_bg, cs_hot))):
         _, cm = O.sweep(gas, d, 0.0, 0.0, g)
         assert abs(cm - expect) < 1e-14
+
+
+def test_sedov_blast_radius_matches_eq21(O, W):
+    """The paper's own closed-form anchor for the hydro solver (PAPER.md:185, Eq. 21): r_sh = 1.15 (E0 t^2 / rho1)^(1/5);
+    "shock-front well resolved within roughly 2 pixels, and angular variation of the shock profile of less than 1 pixel"
+    (PAPER.md:196).  48^3 cells, gamma = 5/3, energy in the central cell, CFL 0.4 steps up to the time Eq. 21 gives
+    r_sh = 8 cells."""
+    import parity as PT
+    N, g, target = 48, 5.0 / 3.0, 8.0
+    gas0 = W.sedov_ic(N, g)
+    P = O.make_params(N, float(N), g, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-12)
+    so = O.State(gas0, np.zeros((6, 0)), 1.0)
+    ref = PT.golden("sedov_eq21.txt")
+    tf, t = W.sedov_time(target, phi0=ref["phi0"]), 0.0
+    while t < tf * (1 - 1e-12):
+        cm = max(O.sweep(so.gas, d, 0.0, 0.0, g)[1] for d in range(3))
+        dt = min(0.4 / cm, tf - t)
+        O.step(P, so, dt, 1.0)
+        t += dt
+    peak, rmin, rmax = PT.shock_radii(so.gas[0])
+    assert abs(peak - target) <= 0.5 * ref["shock_width_cells"], peak
+    assert rmax - rmin <= ref["angular_variation_cells"] + 0.5 and abs(0.5 * (rmin + rmax) - target) <= 1.0, (rmin, rmax)
+    assert abs(so.gas[0].sum() / gas0[0].astype(np.float64).sum() - 1) < 1e-13      # conservative scheme (PAPER.md:37)
+    assert abs(so.gas[4].sum() / gas0[4].astype(np.float64).sum() - 1) < 1e-13
+    assert 1.5 < so.gas[0].max() < 4.0                           # compression below the strong-shock limit (gamma+1)/(gamma-1)
