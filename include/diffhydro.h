@@ -228,6 +228,30 @@ int dh_data_term(dh_ctx* ctx, int observable, float* const gas[5], const float* 
 int dh_power_spectrum(dh_ctx* ctx, const float* field, double* power_out, double* count_out);
 int dh_power_spectrum_vjp(dh_ctx* ctx, const float* field, const double* power_bar, float* field_bar);
 
+/* ---- sub-grid star formation and energy injection (section 2.4, :226-283) ----
+ * Applied to the gas state between coupled steps.  Per cell, with delta = rho/rho_mean - 1 and T = t_per_e * e~
+ * (e~ = eps/rho - |m|^2/(2 rho^2); the caller folds (gamma-1) mu m_p / (k_B a^2) into t_per_e, reading R27):
+ *   pi0 = Pi0 sigma((delta - delta_c)/a_width) sigma((T_c - T)/b_width)                        Eq. 25
+ *   z   = relaxed Bernoulli of Eq. 24 with temperature tau and the caller's Gumbel(0,1) draws g0, g1 (inputs: Eq. 22-23)
+ *   eps += e_inject * rho * z                   (E_0 per unit star-forming gas mass; the caller folds a^2 and units in)
+ * Requires 0 < Pi0 < 1, a_width, b_width, tau, rho_mean > 0. */
+typedef struct {
+    double rho_mean;   /* mean gas density in the state's units (f_b in the configs' units) */
+    double t_per_e;    /* temperature per unit e~ */
+    double T_c, delta_c, Pi0, e_inject;   /* the model's parameters (T_c, rho_c as delta_c, Pi_0, E_0), :242 */
+    double a_width, b_width, tau;         /* hyper-parameters: sigmoid widths of Eq. 25, Gumbel-softmax temperature (0.1, :273) */
+} dh_subgrid_params;
+/* gas: DEVICE, eps (gas[4]) updated in place, the other fields read only.  g0, g1: DEVICE, N^3 floats.  z_out (may be
+ * NULL): DEVICE N^3 floats, the star-forming field of this step.  If aux and pos are given (DEVICE, N_p floats each) the
+ * cloud-in-cell readout of z at the particle positions is ADDED to aux (:244, diagnostic; needs z_out). */
+int dh_subgrid_step(dh_ctx* ctx, float* const gas[5], const float* g0, const float* g1, const dh_subgrid_params* par,
+                    float* z_out, float* const pos[3], float* aux);
+/* Transpose at gas_in = the state BEFORE the injection.  cot_gas: in = cotangent of the step's output, out (in place) =
+ * cotangent of gas_in.  cot_z (may be NULL): cotangent of z_out.  dpar_out: HOST double[4] += (dT_c, ddelta_c, dPi0,
+ * de_inject); synchronises the stream. */
+int dh_subgrid_step_vjp(dh_ctx* ctx, float* const gas_in[5], const float* g0, const float* g1,
+                        const dh_subgrid_params* par, float* const cot_gas[5], const float* cot_z, double* dpar_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,7 +29,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
-           "dh_power_spectrum_vjp"]
+           "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp"]
 
 
 class DhError(RuntimeError):
@@ -57,6 +57,12 @@ class dh_state(C.Structure):
 
 class dh_cot(C.Structure):
     _fields_ = [("gas", C.c_void_p * 5), ("part", C.c_void_p * 6)]
+
+
+class dh_subgrid_params(C.Structure):
+    _fields_ = [("rho_mean", C.c_double), ("t_per_e", C.c_double), ("T_c", C.c_double), ("delta_c", C.c_double),
+                ("Pi0", C.c_double), ("e_inject", C.c_double), ("a_width", C.c_double), ("b_width", C.c_double),
+                ("tau", C.c_double)]
 
 
 class dh_dparams(C.Structure):
@@ -107,6 +113,10 @@ _lib.dh_poisson_vjp.argtypes = [C.c_void_p, _P3, C.c_double, C.c_void_p]
 _lib.dh_kick_drift.argtypes = [C.c_void_p, _P3, _P6, C.c_double, C.c_double]
 _lib.dh_ic_zeldovich.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(dh_state)]
 _lib.dh_data_term.argtypes = [C.c_void_p, C.c_int, _P5, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, _dp]
+_lib.dh_subgrid_step.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POINTER(dh_subgrid_params), C.c_void_p,
+                                 C.c_void_p, C.c_void_p]
+_lib.dh_subgrid_step_vjp.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POINTER(dh_subgrid_params), _P5,
+                                     C.c_void_p, _dp]
 _lib.dh_power_spectrum.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
 _lib.dh_power_spectrum_vjp.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p]
 _lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
@@ -325,6 +335,27 @@ class Context:
                                     C.byref(cs)), "dh_ic_zeldovich")
         st.a, st.dt_prev, st.step = cs.a, cs.dt_prev, cs.step
         return st
+
+    def dh_subgrid_step(self, gas: torch.Tensor, g0: torch.Tensor, g1: torch.Tensor, par: dict, want_z=True,
+                        pos: torch.Tensor | None = None, aux: torch.Tensor | None = None):
+        """Sub-grid step in place on gas (5,N,N,N); returns z (N,N,N) or None.  par: the fields of dh_subgrid_params."""
+        q = dh_subgrid_params(**{k: float(v) for k, v in par.items()})
+        z = torch.empty_like(g0) if (want_z or aux is not None) else None
+        pp = C.cast(_ptrs(pos, 3, _P3), C.c_void_p) if pos is not None else None
+        _check(_lib.dh_subgrid_step(self._h, _ptrs(gas, 5, _P5), g0.data_ptr(), g1.data_ptr(), C.byref(q),
+                                    z.data_ptr() if z is not None else None, pp,
+                                    aux.data_ptr() if aux is not None else None), "dh_subgrid_step")
+        return z
+
+    def dh_subgrid_step_vjp(self, gas_in: torch.Tensor, g0: torch.Tensor, g1: torch.Tensor, par: dict,
+                            cot_gas: torch.Tensor, cot_z: torch.Tensor | None = None):
+        """cot_gas (5,N,N,N) is transformed in place; returns (dT_c, ddelta_c, dPi0, de_inject) as a float64 array."""
+        q = dh_subgrid_params(**{k: float(v) for k, v in par.items()})
+        d = np.zeros(4)
+        _check(_lib.dh_subgrid_step_vjp(self._h, _ptrs(gas_in, 5, _P5), g0.data_ptr(), g1.data_ptr(), C.byref(q),
+                                        _ptrs(cot_gas, 5, _P5), cot_z.data_ptr() if cot_z is not None else None,
+                                        d.ctypes.data_as(_dp)), "dh_subgrid_step_vjp")
+        return d
 
     def dh_power_spectrum(self, field: torch.Tensor):
         """(P_b, count_b), b = 1 .. N/2, as host float64 arrays."""

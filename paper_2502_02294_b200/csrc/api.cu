@@ -791,6 +791,50 @@ int dh_power_spectrum_vjp(dh_ctx* c, const float* field, const double* power_bar
     return DH_OK;
 }
 
+static int check_subgrid(const dh_ctx* c, float* const gas[5], const float* g0, const float* g1, const dh_subgrid_params* q,
+                         const char* who) {
+    if (!c || !gas || !g0 || !g1 || !q) { set_error("%s: null argument", who); return DH_ERR_INVALID; }
+    for (int k = 0; k < 5; ++k) if (!gas[k]) { set_error("%s: null gas pointer %d", who, k); return DH_ERR_INVALID; }
+    if (!(q->Pi0 > 0 && q->Pi0 < 1) || !(q->a_width > 0) || !(q->b_width > 0) || !(q->tau > 0) || !(q->rho_mean > 0)) {
+        set_error("%s: need 0 < Pi0 < 1 and a_width, b_width, tau, rho_mean > 0", who);
+        return DH_ERR_INVALID;
+    }
+    return DH_OK;
+}
+
+int dh_subgrid_step(dh_ctx* c, float* const gas[5], const float* g0, const float* g1, const dh_subgrid_params* par,
+                    float* z_out, float* const pos[3], float* aux) {
+    DH_TRY(check_subgrid(c, gas, g0, g1, par, "dh_subgrid_step"));
+    if (aux && (!z_out || !pos || !pos[0] || !pos[1] || !pos[2])) {
+        set_error("dh_subgrid_step: the particle readout needs z_out and the three position arrays");
+        return DH_ERR_INVALID;
+    }
+    DH_TRY(launch_subgrid(c, gas, g0, g1, *par, z_out));
+    if (aux) DH_TRY(launch_cic_readout(c, z_out, pos, aux));
+    return DH_OK;
+}
+
+int dh_subgrid_step_vjp(dh_ctx* c, float* const gas_in[5], const float* g0, const float* g1, const dh_subgrid_params* par,
+                        float* const cot_gas[5], const float* cot_z, double* dpar_out) {
+    DH_TRY(check_subgrid(c, gas_in, g0, g1, par, "dh_subgrid_step_vjp"));
+    if (!cot_gas) { set_error("dh_subgrid_step_vjp: null cotangent"); return DH_ERR_INVALID; }
+    for (int k = 0; k < 5; ++k) if (!cot_gas[k]) { set_error("dh_subgrid_step_vjp: null cotangent %d", k); return DH_ERR_INVALID; }
+    double* scal = nullptr;
+    DH_TRY(dev_alloc(c, (void**)&scal, 4 * sizeof(double)));
+    int rc = DH_OK;
+    double h[4] = {0, 0, 0, 0};
+    if (cudaMemsetAsync(scal, 0, 4 * sizeof(double), c->stream) != cudaSuccess) rc = DH_ERR_CUDA;
+    if (rc == DH_OK) rc = launch_subgrid_vjp(c, gas_in, g0, g1, *par, cot_gas, cot_z, scal);
+    if (rc == DH_OK && (cudaMemcpyAsync(h, scal, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                        cudaStreamSynchronize(c->stream) != cudaSuccess)) {
+        set_error("dh_subgrid_step_vjp: %s", cudaGetErrorString(cudaGetLastError()));
+        rc = DH_ERR_CUDA;
+    }
+    dev_free(c, scal, 4 * sizeof(double));
+    if (rc == DH_OK && dpar_out) for (int j = 0; j < 4; ++j) dpar_out[j] += h[j];
+    return rc;
+}
+
 int dh_data_term(dh_ctx* c, int observable, float* const gas[5], const float* data, const float* noise_var, double scale,
                  double weight, float* const cot_gas[5], double* loss_out) {
     if (!c || !gas || !data || (observable != 0 && observable != 1)) {

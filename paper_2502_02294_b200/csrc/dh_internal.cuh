@@ -202,6 +202,13 @@ int launch_ic_state_vjp(dh_ctx* c, const float* delta, float* const psi[3], cons
 int launch_data_term(dh_ctx* c, int observable, const float* const gas[5], const float* data, const float* noise_var,
                      float scale, float weight, float* const cot[5], double* loss_dev);
 
+// ---- sub-grid step (subgrid.cu) ----
+int launch_subgrid(dh_ctx* c, float* const gas[5], const float* g0, const float* g1, const dh_subgrid_params& q,
+                   float* zout);
+int launch_subgrid_vjp(dh_ctx* c, float* const gas_in[5], const float* g0, const float* g1, const dh_subgrid_params& q,
+                       float* const cot[5], const float* cot_z, double* scal4_dev);
+int launch_cic_readout(dh_ctx* c, const float* mesh, float* const pos[3], float* aux);
+
 // ---- own FFT passes fused with the Green multiply (fft.cu) ----
 bool own_fft_supported(int N);
 int own_fft_init(dh_ctx* c);

@@ -591,6 +591,50 @@ def test_power_spectrum_and_its_transpose_match_oracle(api, torch_, W, IC, N):
     ctx.close()
 
 
+def test_subgrid_step_and_its_transpose_match_oracle(api, torch_, O, W, IC):
+    """dh_subgrid_step / dh_subgrid_step_vjp (section 2.4, Eq. 24-25) against
+    oracle/subgrid.py on the same gas state and the same Gumbel draws (inputs, Eq. 23); the CIC readout of the
+    star-forming field at the particles against the oracle's gather."""
+    from oracle import subgrid as SG
+    N = 64
+    cfg = W.scaled_config(0, N, rms_delta=0.3)
+    _, gas, part = IC.coupled_ic(W, cfg)
+    gas[1:4] *= 0.1; gas[4] = gas[0] * cfg.e_tilde0() * (1 + 0.3 * np.sin(np.arange(N))[None, None, :]) \
+        + 0.5 * np.sum(gas[1:4].astype(np.float64) ** 2, axis=0).astype(np.float32) / gas[0]      # moderate Mach number
+    rng = np.random.default_rng(11)
+    g0 = rng.gumbel(size=(N, N, N)).astype(np.float32); g1 = rng.gumbel(size=(N, N, N)).astype(np.float32)
+    e0 = cfg.e_tilde0()
+    T0 = 1e4
+    par = dict(rho_mean=cfg.f_b, t_per_e=T0 / e0, T_c=1.2e4, delta_c=0.2, Pi0=0.3, e_inject=3.0 * e0, a_width=0.25,
+               b_width=2e3, tau=0.1)
+    okw = dict(rho_mean=par["rho_mean"], t_per_e=par["t_per_e"], T_c=par["T_c"], delta_c=par["delta_c"], Pi0=par["Pi0"],
+               e_inject=par["e_inject"], a_w=par["a_width"], b_w=par["b_width"], tau=par["tau"])
+    out_ref, z_ref = SG.step(gas, g0, g1, **okw)
+    assert 0.01 < z_ref.mean() < 0.5                                   # the case exercises both branches
+    ctx = api.context_for(cfg)
+    gd = _gpu(torch_, gas); g0d = _gpu(torch_, g0); g1d = _gpu(torch_, g1); pd = _gpu(torch_, part)
+    aux = torch_.zeros(N ** 3, device="cuda")
+    z = ctx.dh_subgrid_step(gd, g0d, g1d, par, pos=pd[:3].contiguous(), aux=aux)
+    ez = np.max(np.abs(z.cpu().numpy() - z_ref))
+    print(f"subgrid: max |z - z_ref| = {ez:.2e}, mean z = {z_ref.mean():.3f}")
+    # z in [0, 1]: absolute.  The log-odds are divided by tau = 0.1 and T comes out of the fp32 cancellation eps - ke
+    # (reading R17): |dz| <= (1/4)(1/tau)(dT/b) with dT/T ~ 6e-8 (1 + ke/(rho e~)) ~ 2e-6 here (DESIGN.md section 16)
+    assert ez < 5e-5
+    assert max(PT.field_err(gd.cpu().numpy(), out_ref).values()) < TOL_STEP
+    assert torch_.equal(gd[:4].cpu(), torch_.from_numpy(gas[:4]))      # only the energy changes
+    aux_ref = O.gather(N, part[:3].astype(np.float64), z_ref)
+    assert np.max(np.abs(aux.cpu().numpy() - aux_ref)) < 5e-5
+    cg = rng.standard_normal(gas.shape).astype(np.float32); cz = rng.standard_normal((N, N, N)).astype(np.float32)
+    cin_ref, dpar_ref = SG.step_vjp(gas, g0, g1, cot_gas=cg, cot_z=cz, **okw)
+    cgd = _gpu(torch_, cg)
+    dpar = ctx.dh_subgrid_step_vjp(_gpu(torch_, gas), g0d, g1d, par, cgd, _gpu(torch_, cz))
+    assert PT.rel_l2(cgd.cpu().numpy(), cin_ref) < 1e-4, PT.rel_l2(cgd.cpu().numpy(), cin_ref)
+    assert np.all(np.abs(dpar - dpar_ref) < 1e-4 * (np.abs(dpar_ref) + 1e-3 * np.max(np.abs(dpar_ref)))), (dpar, dpar_ref)
+    with pytest.raises(api.DhError):
+        ctx.dh_subgrid_step(gd, g0d, g1d, dict(par, Pi0=1.0))
+    ctx.close()
+
+
 def test_reverse_pass_storage_policies_agree(api, torch_, W, IC):
     """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
     ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
