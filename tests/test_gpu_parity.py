@@ -635,7 +635,7 @@ def test_subgrid_step_and_its_transpose_match_oracle(api, torch_, O, W, IC):
     ctx.close()
 
 
-def test_reverse_pass_storage_policies_agree(api, torch_, W, IC):
+def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
     """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
     ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
     policies differ by the order of the deposit's fp32 atomics in the recomputed g' (last-bit), nothing more."""
@@ -653,10 +653,28 @@ def test_reverse_pass_storage_policies_agree(api, torch_, W, IC):
         dp = ctx.dh_run_vjp(ct, ct)
         out.append((ct.gas.cpu().numpy(), ct.part.cpu().numpy(), dp.dgamma, ctx.dh_launch_count()))
         ctx.close()
+    # Bound as for "gradient independent of checkpoint_stride" (reading R28): what the fp64 oracle's own
+    # gradient of this run does when its inputs move by one fp32 rounding -- a recomputed g' differs from a kept one by
+    # exactly such last-bit changes (atomic order), and a flipped limiter gate moves a few entries by O(1).
+    P = PT.oracle_params(O, cfg)
+    a_o, dt_o = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+
+    def oracle_grad(gas_, part_):
+        gr, pr, _, _ = O.run(P, gas_, part_, cfg.a0, a_o[1:], dt_o)
+        cot = np.zeros_like(gr); cot[0] = gr[0]
+        return O.run_vjp(P, gas_, part_, cfg.a0, a_o[1:], dt_o, cot, np.zeros_like(pr))[:2]
+    rg, rp = oracle_grad(gas, part)
+    sens_g = sens_p = 0.0
+    for seed in (7, 8):
+        prng = np.random.default_rng(seed)
+        rg2, rp2 = oracle_grad(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)),
+                               part.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(part.shape)))
+        sens_g, sens_p = max(sens_g, PT.rel_l2(rg2, rg)), max(sens_p, PT.rel_l2(rp2, rp))
+    tol_g, tol_p = max(TOL_GRAD, 1.5 * sens_g), max(TOL_GRAD, 1.5 * sens_p)
     g0, p0, dg0, n0 = out[0]
     for g, p_, dg, n in out[1:]:
-        # same bound as "gradient independent of checkpoint_stride" (reading R28)
-        assert PT.rel_l2(g, g0) < TOL_GRAD and PT.rel_l2(p_, p0) < TOL_GRAD and abs(dg / dg0 - 1) < 1e-4
+        assert PT.rel_l2(g, g0) < tol_g and PT.rel_l2(p_, p0) < tol_p and abs(dg / dg0 - 1) < 1e-4, (sens_g, sens_p)
+        assert PT.rel_l2_trimmed(g, g0, frac=1e-2) < TOL_GRAD
     # keeping g' removes deposit + Poisson from the segment re-run: fewer launches than recomputing it
     assert out[0][3] < out[2][3] and out[1][3] < out[3][3]
 
