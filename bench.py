@@ -258,7 +258,9 @@ def main():
     N, n3 = cfg.N, cfg.N ** 3
     delta_h, gas_h, part_h, target_h = build_inputs(W, cfg, rank)
     a_s, dt_s = schedule(api, cfg, K)
-    ctx = api.context_for(cfg, want_dA=0)
+    # dparams: gamma (and K, the particles' Dtau part); the cotangents of the schedule scalars A, Dtau, kappa are not part
+    # of config 3's outputs (gradients w.r.t. the initial density field and gamma) and are switched off
+    ctx = api.context_for(cfg, want_dA=0, want_dsched=0)
     for kv in args.tune:
         key, val = kv.split("=")
         ctx.dh_tune(key, int(val))
@@ -432,7 +434,7 @@ def main():
                "config": {"workload": cfg.name, "grid": N, "particles": cfg.n_side ** 3, "box": cfg.box,
                           "checkpoint_stride": stride, "schedule": f"first {K} of {cfg.n_steps} ln-a steps"
                           if not cfg.static_mode else f"{K} steps at CFL 0.4",
-                          "loss": "sum (rho_gas - rho_target)^2", "parallelism": f"replicas x{world}", "tune": args.tune,
+                          "loss": "sum (rho_gas - rho_target)^2", "gradients": "d/d(initial state), d/d(delta_init), d/d(gamma); want_dA=0, want_dsched=0", "parallelism": f"replicas x{world}", "tune": args.tune,
                           "l2": "working set (state + scratch >= 0.7 GB at 256^3) exceeds the 126 MB L2; no flush"},
                "fwd": {"value": value_fwd, "unit": UNIT, "ms_per_step": ms_fwd / K},
                "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,

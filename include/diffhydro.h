@@ -58,6 +58,9 @@ typedef struct {
     double lim_eps;               /* epsilon of the altered Van Leer limiter, Eq. 18 (reading R8) */
     void* cuda_stream;            /* cudaStream_t to issue all work on; NULL = the legacy default stream */
     int32_t want_dA;              /* 1: dh_step_vjp also accumulates dparams.dA (one extra pass over g') */
+    int32_t want_dsched;          /* 1: the sweep adjoints also accumulate the cotangents of Dtau and kappa (dparams.dDtau,
+                                   * dparams.dkappa: needed for cosmological-parameter gradients); 0: they are skipped (about
+                                   * 6 % of the adjoint sweeps' arithmetic) and both fields come back as NaN */
 } dh_options;
 
 /* State of the simulation.  gas/part: caller-owned DEVICE pointers (N^3 and N_p floats each).

@@ -47,7 +47,7 @@ class dh_cosmology(C.Structure):
 class dh_options(C.Structure):
     _fields_ = [("n_part_side", C.c_int32), ("gravity_on", C.c_int32), ("hydro_on", C.c_int32),
                 ("gas_sources_gravity", C.c_int32), ("e_floor", C.c_double), ("lim_eps", C.c_double),
-                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32)]
+                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32), ("want_dsched", C.c_int32)]
 
 
 class dh_state(C.Structure):
@@ -174,7 +174,7 @@ class Context:
     """Owner of a dh_ctx*.  Methods are the C calls with tensors marshalled to pointers."""
 
     def __init__(self, N, box, gamma, n_part_side=None, H0=100.0, Omega_m=1.0, Omega_b=0.16, Omega_L=0.0, static_mode=0,
-                 gravity_on=1, hydro_on=1, gas_sources_gravity=1, e_floor=1e-12, lim_eps=1e-20, want_dA=1,
+                 gravity_on=1, hydro_on=1, gas_sources_gravity=1, e_floor=1e-12, lim_eps=1e-20, want_dA=1, want_dsched=1,
                  stream: torch.cuda.Stream | None = None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2502_02294_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -184,7 +184,7 @@ class Context:
         self.cosmo = dh_cosmology(H0, Omega_m, Omega_b, Omega_L, int(static_mode))
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         self.opt = dh_options(self.nps, int(gravity_on), int(hydro_on), int(gas_sources_gravity), float(e_floor),
-                              float(lim_eps), C.c_void_p(self.stream.cuda_stream), int(want_dA))
+                              float(lim_eps), C.c_void_p(self.stream.cuda_stream), int(want_dA), int(want_dsched))
         self._h = C.c_void_p()
         _check(_lib.dh_init(C.byref(self._h), self.N, float(box), float(gamma), C.byref(self.cosmo), C.byref(self.opt)),
                "dh_init")

@@ -255,8 +255,13 @@ static int harvest_scalars(dh_ctx* c, dh_dparams* dp) {
     DH_CUDA(cudaStreamSynchronize(c->stream));
     if (dp) {
         dp->dgamma += h[2];
-        dp->dDtau += (h[0] + h[4]) / c->dx;
-        dp->dkappa += h[1];
+        if (c->opt.want_dsched || !c->opt.hydro_on) {
+            dp->dDtau += (h[0] + h[4]) / c->dx;
+            dp->dkappa += h[1];
+        } else {                                   // not computed by the sweep adjoints (dh_options.want_dsched = 0): say so
+            dp->dDtau = nan("");
+            dp->dkappa = nan("");
+        }
         dp->dK += h[3];
         dp->dA += h[5];
     }

@@ -129,7 +129,8 @@ __device__ __forceinline__ void sweep_forward_core(const float (&u)[K][5], const
 
 // Adjoint core.  In: u (sweep input), g, ob (cotangent of the sweep output).  Out: ub (cotangent of u), gb (of g) and
 // per-thread partial sums of the scalar cotangents over the cells flagged in `count` (each global cell once).
-template <int K, bool HAS_G>
+// LK = false drops the cotangents of lam and kap (dh_options.want_dsched = 0) and with them the arrays only they need.
+template <int K, bool HAS_G, bool LK = true>
 __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const float (&g)[K], const float (&ob)[K][5],
                                                    const bool (&count)[K], const Chain& ch, const SweepConst& sc,
                                                    float (&ub)[K][5], float (&gb)[K], float& lam_b, float& kap_b,
@@ -156,8 +157,9 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
             for (int j = 0; j < K; ++j) {
                 const float Dn = G[j][k] - (j + 1 < K ? H[j + 1][k] : HK);
                 const float Dm = (j > 0 ? G[j - 1][k] : Gm1) - H[j][k];
-                dD[j][k] = Dn - Dm;
-                us[j][k] = fmaf(-0.25f * sc.lam, dD[j][k], u[j][k]);
+                const float dd = Dn - Dm;
+                if (LK) dD[j][k] = dd;
+                us[j][k] = fmaf(-0.25f * sc.lam, dd, u[j][k]);
             }
         }
         if (HAS_G) {
@@ -224,9 +226,11 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
             exC[(20 + k) * nt + ch.tid] = psi[K - 1];
 #pragma unroll
             for (int j = 0; j < K; ++j) { GsB[j][k] = gB[j + 1]; HsB[j][k] = hB[j]; }
+            if (LK) {
 #pragma unroll
-            for (int j = 1; j < K; ++j) dpsi[j][k] = psi[j] - psi[j - 1];
-            dpsi[0][k] = psi[0];                          // Psi_{-1} subtracted after the exchange
+                for (int j = 1; j < K; ++j) dpsi[j][k] = psi[j] - psi[j - 1];
+                dpsi[0][k] = psi[0];                      // Psi_{-1} subtracted after the exchange
+            }
         }
         __syncthreads();
 #pragma unroll
@@ -235,7 +239,7 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
             GsB[0][k] += exC[(5 + k) * nt + ch.ltid];
             HsB[0][k] += exC[(10 + k) * nt + ch.ltid];
             if (K > 1) HsB[1][k] += exC[(15 + k) * nt + ch.ltid];
-            dpsi[0][k] -= exC[(20 + k) * nt + ch.ltid];
+            if (LK) dpsi[0][k] -= exC[(20 + k) * nt + ch.ltid];
         }
         // K == 1: H*_1 of the left neighbour's view is the cell after me -- not supported (K >= 2 required)
     }
@@ -247,9 +251,11 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
         float gm_j = 0.f;
         prim_GH_vjp(us[j], sc, GsB[j], HsB[j], usb[j], gm_j);
         float l_j = 0.f;
+        if (LK) {
 #pragma unroll
-        for (int k = 0; k < 5; ++k) l_j = fmaf(ob[j][k], dpsi[j][k], l_j);
-        l_j *= -0.5f;
+            for (int k = 0; k < 5; ++k) l_j = fmaf(ob[j][k], dpsi[j][k], l_j);
+            l_j *= -0.5f;
+        }
         float k_j = 0.f;
         gb[j] = 0.f;
         if (HAS_G) {
@@ -258,7 +264,7 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
             usb[j][1] = fmaf(kg, ob[j][4], usb[j][1]);
             const float t = us[j][0] * ob[j][1] + us[j][1] * ob[j][4];
             gb[j] = sc.kap * t;
-            k_j = g[j] * t;
+            if (LK) k_j = g[j] * t;
         }
         if (count[j]) { gacc += gm_j; lacc += l_j; kacc += k_j; }
     }
@@ -292,7 +298,7 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
             ub[j][k] += ob[j][k] + usb[j][k];
-            l_j = fmaf(usb[j][k], dD[j][k], l_j);
+            if (LK) l_j = fmaf(usb[j][k], dD[j][k], l_j);
         }
         l_j *= -0.25f;
         float k_j = 0.f;
@@ -302,7 +308,7 @@ __device__ __forceinline__ void sweep_adjoint_core(const float (&u)[K][5], const
             ub[j][1] = fmaf(hk, usb[j][4], ub[j][1]);
             const float t = u[j][0] * usb[j][1] + u[j][1] * usb[j][4];
             gb[j] = fmaf(0.5f * sc.kap, t, gb[j]);
-            k_j = 0.5f * g[j] * t;
+            if (LK) k_j = 0.5f * g[j] * t;
         }
         if (count[j]) { gacc += gm_j; lacc += l_j; kacc += k_j; }
     }
@@ -377,7 +383,7 @@ __global__ void __launch_bounds__(512) sweep_x_fwd_kernel(Ptr5 in, const float* 
     }
 }
 
-template <int K, bool HAS_G>
+template <int K, bool HAS_G, bool LK>
 __global__ void __launch_bounds__(512) sweep_x_adj_kernel(Ptr5 in, const float* __restrict__ gfield, Ptr5 cot_out,
                                                           MPtr5 cot_in, float* __restrict__ gbar, double* scal,
                                                           SweepConst sc, long nrows) {
@@ -408,7 +414,7 @@ __global__ void __launch_bounds__(512) sweep_x_adj_kernel(Ptr5 in, const float* 
     for (int j = 0; j < K; ++j) count[j] = valid;
     Chain ch{smem, nthr, r * Cx + cx, r * Cx + (cx == 0 ? Cx - 1 : cx - 1), r * Cx + (cx == Cx - 1 ? 0 : cx + 1)};
     float lb, kb, gmb;
-    sweep_adjoint_core<K, HAS_G>(u, g, ob, count, ch, sc, ub, gb, lb, kb, gmb);
+    sweep_adjoint_core<K, HAS_G, LK>(u, g, ob, count, ch, sc, ub, gb, lb, kb, gmb);
     if (valid) {
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
@@ -632,8 +638,13 @@ int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float
         dim3 block; unsigned grid; long nrows = (long)N * N;
         x_geometry<KA>(N, block, grid, nrows);
         size_t sm = (size_t)ADJ_SLOTS * block.x * block.y * sizeof(float);
-        if (g) DH_LAUNCH((sweep_x_adj_kernel<KA, true>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
-        else DH_LAUNCH((sweep_x_adj_kernel<KA, false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+        if (c->opt.want_dsched) {
+            if (g) DH_LAUNCH((sweep_x_adj_kernel<KA, true, true>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+            else DH_LAUNCH((sweep_x_adj_kernel<KA, false, true>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+        } else {
+            if (g) DH_LAUNCH((sweep_x_adj_kernel<KA, true, false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+            else DH_LAUNCH((sweep_x_adj_kernel<KA, false, false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+        }
     } else if (!c->tune_yz_chain) {
         DH_TRY(launch_sweep_march_vjp(c, d, pin, g, pco, pci, g_bar, scal_bar, sc));
     } else {

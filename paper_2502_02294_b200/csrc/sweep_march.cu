@@ -171,7 +171,8 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
 }
 
 // ------------------------------------------------------------------------------------------------- adjoint ----
-template <bool HAS_G, bool EPS>
+// LK = false drops the cotangents of lam and kap (dh_options.want_dsched = 0): gamma_b only.
+template <bool HAS_G, bool EPS, bool LK>
 struct AdjPipe {
     // forward recompute
     float u1[5], g1, G1[5], D2[5];         // u_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
@@ -231,8 +232,10 @@ struct AdjPipe {
             const float dob1 = ob2[k] - ob1[k];           // ob_{q-3} - ob_{q-2}
             const float pb0 = -0.5f * sc.lam * dob0;      // Psi_b of interface q-2
             const float pb1 = -0.5f * sc.lam * dob1;      // Psi_b of interface q-3
-            lg = fmaf(Gs[k] + L, dob0, lg);               // PsiG_{q-2} (ob_{q-2} - ob_{q-1})
-            lh = fmaf(Hs[k] - M, dob1, lh);               // PsiH_{q-3} (ob_{q-3} - ob_{q-2})
+            if (LK) {
+                lg = fmaf(Gs[k] + L, dob0, lg);           // PsiG_{q-2} (ob_{q-2} - ob_{q-1})
+                lh = fmaf(Hs[k] - M, dob1, lh);           // PsiH_{q-3} (ob_{q-3} - ob_{q-2})
+            }
             GsB[k] = fmaf(-LA, pb0, GB0[k]);
             GB0[k] = fmaf(1.f + LA - LB, pb0, GB1[k]);
             GB1[k] = LB * pb0;
@@ -257,8 +260,10 @@ struct AdjPipe {
 #pragma unroll
         for (int k = 0; k < 5; ++k) acc[k] = ob2[k] + usb[k];
         float dA = 0.f;                                   // sum_k u*_b (u - u* + (kap/2) g S(u))
+        if (LK) {
 #pragma unroll
-        for (int k = 0; k < 5; ++k) dA = fmaf(usb[k], uM[k] - us2[k], dA);
+            for (int k = 0; k < 5; ++k) dA = fmaf(usb[k], uM[k] - us2[k], dA);
+        }
         if (HAS_G) {
             const float hk = 0.5f * sc.kap * gM;
             acc[0] = fmaf(hk, usb[1], acc[0]);
@@ -267,8 +272,7 @@ struct AdjPipe {
             const float tA = uM[0] * usb[1] + uM[1] * usb[4];
             const float t = fmaf(0.5f, tA, tB);
             gb = sc.kap * t;
-            kapM = gM * t;
-            dA = fmaf(hk, tA, dA);
+            if (LK) { kapM = gM * t; dA = fmaf(hk, tA, dA); }
         }
         lamA = -sc.inv_lam * dA;
         // ---- cell r = q-4: stage-A transpose
@@ -295,7 +299,7 @@ struct AdjPipe {
     }
 };
 
-template <int DIR, bool HAS_G, bool EPS>
+template <int DIR, bool HAS_G, bool EPS, bool LK>
 __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 in, const float* __restrict__ gfield,
                                                                           Ptr5 cot_out, MPtr5 cot_in,
                                                                           float* __restrict__ gbar, double* scal,
@@ -338,7 +342,7 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
         if (it < niter) issue(it);
         cp_async_commit();
     }
-    AdjPipe<HAS_G, EPS> pipe;
+    AdjPipe<HAS_G, EPS, LK> pipe;
     pipe.init();
     float lacc = 0.f, kacc = 0.f, gacc = 0.f;
 #pragma unroll 1
@@ -365,11 +369,12 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
         float ub[5], gb, lamG, lamH, lamA, kapM, gamM, gamR;
         pipe.push(u0, g0, ob0, ob1, ob2, uM, gM, uR, sc, ub, gb, lamG, lamH, lamA, kapM, gamM, gamR);
         // interface q-2 = p0 + i - 6, cell / interface q-3 = p0 + i - 7, cell q-4 = p0 + i - 8
-        if (i >= 6 && i < len + 6) lacc += lamG;
+        if (LK && i >= 6 && i < len + 6) lacc += lamG;
         if (i >= 7) {
             off_m += stride;
             if (i < len + 7) {
-                lacc += lamH + lamA; kacc += kapM; gacc += gamM;
+                if (LK) { lacc += lamH + lamA; kacc += kapM; }
+                gacc += gamM;
                 if (HAS_G) gbar[off_m] = gb;
             }
         }
@@ -421,17 +426,17 @@ static int march_fwd_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin,
     return DH_OK;
 }
 
-template <int DIR>
+template <int DIR, bool LK>
 static int march_adj_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const Ptr5& pco,
                               const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S, bool eps) {
     if (g) {
         const size_t sm = (size_t)RING * 11 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, true, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, false, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
     } else {
         const size_t sm = (size_t)RING * 10 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, true, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, false, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
     }
     return DH_OK;
 }
@@ -456,8 +461,9 @@ int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, co
     const dim3 block = march_block(N);
     const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
     const bool eps = c->opt.lim_eps > 1e-18;
-    if (d == 1) march_adj_dispatch<1>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
-    else march_adj_dispatch<2>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    const bool lk = c->opt.want_dsched != 0;
+    if (d == 1) { if (lk) march_adj_dispatch<1, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); else march_adj_dispatch<1, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); }
+    else { if (lk) march_adj_dispatch<2, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); else march_adj_dispatch<2, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); }
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }

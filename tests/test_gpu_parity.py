@@ -679,6 +679,28 @@ def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
     assert out[0][3] < out[2][3] and out[1][3] < out[3][3]
 
 
+def test_want_dsched_off_changes_only_the_schedule_cotangents(api, torch_, W, IC):
+    """dh_options.want_dsched = 0 skips the cotangents of Dtau and kappa in the sweep adjoints: the state cotangents and
+    d gamma are the same numbers (hydro only, so no atomics: bit for bit), dDtau and dkappa come back as NaN."""
+    cfg = W.scaled_config(0, 32, n_steps=5, a1=0.03)
+    _, gas, part = IC.coupled_ic(W, cfg)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    res = []
+    for flag in (1, 0):
+        ctx = api.context_for(cfg, gravity_on=0, n_part_side=0, want_dsched=flag)
+        sg = api.State(gas, np.zeros((6, 0), dtype=np.float32), cfg.a0)
+        ctx.dh_run(sg, a_s[1:], dt_s, 2)
+        cg = torch_.zeros_like(sg.gas); cg[0] = sg.gas[0]
+        ct = api.Cot(cg, torch_.zeros((6, 0), device="cuda"))
+        dp = ctx.dh_run_vjp(ct, ct)
+        res.append((ct.gas.cpu().numpy(), dp.as_dict()))
+        ctx.close()
+    assert np.array_equal(res[0][0], res[1][0])
+    assert abs(res[0][1]["dgamma"] / res[1][1]["dgamma"] - 1) < 1e-12
+    assert np.isfinite(res[0][1]["dDtau"]) and np.isfinite(res[0][1]["dkappa"])
+    assert np.isnan(res[1][1]["dDtau"]) and np.isnan(res[1][1]["dkappa"])
+
+
 def test_run_host_variant_matches_device_variant(api, torch_, W, IC):
     cfg = W.scaled_config(0, 32, n_steps=4, a1=0.02)
     delta, gas, part = IC.coupled_ic(W, cfg)
