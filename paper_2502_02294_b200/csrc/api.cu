@@ -142,8 +142,9 @@ static void free_snaps(dh_ctx* c, std::vector<Snapshot>& v) {
 }
 
 // S1 + S2: delta_tot and g' from the state's gas density and particle positions.
-static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A, float* const gp[3]) {
-    DH_TRY(launch_deposit(c, gas[0], part[0], part[1], part[2], c->delta));
+static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A, float* const gp[3],
+                           bool delta_primed = false) {
+    DH_TRY(launch_deposit(c, gas[0], part[0], part[1], part[2], c->delta, delta_primed));
     DH_TRY(poisson_forward(c, c->delta, A, gp));
     return DH_OK;
 }
@@ -156,10 +157,14 @@ static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6],
 // needs nothing more of a segment's last step).
 static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], float* const gas_out[5],
                        float* const part_out[6], const StepScalars& s, int64_t step, float* cmax3, StepTape* tape,
-                       bool last_sweep, float* const* gp_keep = nullptr, bool gp_ready = false) {
+                       bool last_sweep, float* const* gp_keep = nullptr, bool gp_ready = false,
+                       bool delta_primed = false, bool prime_next = false) {
+    // delta_primed: c->delta already holds [gas] rho - rho_bar of this state (the previous step's last sweep wrote it);
+    // prime_next: this step's last sweep writes it for the next step (dh_run's loop only: nobody can touch the state
+    // in between), which takes the source-init pass (8 B/cell) off every step but a run's first.
     const bool grav = c->opt.gravity_on != 0;
     float* const* gp = gp_keep ? gp_keep : (tape ? tape->gp : c->gp);
-    if (grav && !gp_ready) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp));
+    if (grav && !gp_ready) DH_TRY(compute_gravity(c, gas, part, (float)s.A, gp, delta_primed));
     // S3 beside S4: fork the particle update onto the side stream (not while per-kernel events are being recorded)
     const bool particles = c->np > 0 && part_out;
     const bool beside = particles && c->opt.hydro_on && c->tune_overlap && c->side && !c->prof_on;
@@ -185,7 +190,8 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
             const int d = order[sidx];
             for (int k = 0; k < 5; ++k)
                 nxt[k] = sidx == 2 ? gas_out[k] : (tape ? tape->sw[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
-            DH_TRY(launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr));
+            DH_TRY(launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr,
+                                (sidx == 2 && prime_next) ? c->delta : nullptr));
             for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
         }
         if (beside) DH_CUDA(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
@@ -446,6 +452,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
     else if (!strcmp(key, "own_fft")) c->tune_own_fft = value;
     else if (!strcmp(key, "overlap")) c->tune_overlap = value;
+    else if (!strcmp(key, "prime")) c->tune_prime = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -532,8 +539,10 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     for (int k = 0; k < n_steps; ++k) {
         if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
+        const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && !c->tune_yz_chain && c->tune_prime;
         DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
-                           c->run_gstore ? c->gstore[k].gp : nullptr, false));
+                           c->run_gstore ? c->gstore[k].gp : nullptr, false, can_prime && k > 0,
+                           can_prime && k + 1 < n_steps));
         st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
         st->dt_prev = dt_sched[k];
         st->step += 1;

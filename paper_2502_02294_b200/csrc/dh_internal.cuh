@@ -92,6 +92,7 @@ struct dh_ctx {
     int64_t bytes = 0;
     // tuning knobs (dh_tune): 0 = built-in choice
     int tune_march_s_fwd = 0, tune_march_s_adj = 0;   // segment length of the marching y/z sweeps
+    int tune_prime = 1;                               // 0: every step of dh_run initialises its Poisson source itself
     int tune_overlap = 1;                             // 0: kick_drift on the main stream, after which the sweeps start
     int tune_yz_chain = 0;                            // 1: y/z sweeps through the chain kernels of sweep.cu
 
@@ -175,12 +176,15 @@ void dev_free(dh_ctx* c, void* p, size_t bytes);
 StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, double dt, double dt_prev);
 
 // ---- kernels (sweep.cu) ----
+// delta_out (may be NULL; not with tune_yz_chain): also write delta = [gas] rho' - rho_bar, the next step's Poisson source
 int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
-                 float* cmax);
+                 float* cmax, float* delta_out = nullptr);
 int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap,
                      float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar);
 // ---- kernels (pm.cu) ----
-int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta);
+// primed: delta already holds [gas] rho_gas - rho_bar (written by the previous step's last sweep): deposit only
+int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta,
+                   bool primed = false);
 int launch_green(dh_ctx* c, const float2* dhat, float A, float2* const ghat[3]);
 int launch_green_adj(dh_ctx* c, float2* const gbhat[3], float A, float2* dbhat);
 int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float* const part_out[6], float K,

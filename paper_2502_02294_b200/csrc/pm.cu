@@ -453,16 +453,17 @@ int launch_cell_index(dh_ctx* c, const float* x, int64_t n, int32_t* i0, int32_t
     return DH_OK;
 }
 
-int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta) {
+int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta,
+                   bool primed) {
     const float flag = (c->opt.gas_sources_gravity && rho_gas) ? 1.f : 0.f;
     const int64_t n4 = c->n3 / 4;
-    {
+    if (!primed) {
         Prof prof(c, PROF_SOURCE_INIT);
         source_init_kernel<<<grid_for(n4, 256, c->sm_count, 8), 256, 0, c->stream>>>(
             reinterpret_cast<const float4*>(flag != 0.f ? rho_gas : nullptr), reinterpret_cast<float4*>(delta), n4, flag,
             (float)c->rho_bar);
+        c->launches++;
     }
-    c->launches++;
     DH_CUDA(cudaGetLastError());
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT);

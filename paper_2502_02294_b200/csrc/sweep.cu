@@ -341,7 +341,8 @@ __device__ __forceinline__ void store_vec(float* p, const float (&v)[K]) {
 // block = (N/K chain threads, R rows); grid.x = ceil(N^2 / R)
 template <int K, bool HAS_G>
 __global__ void __launch_bounds__(512) sweep_x_fwd_kernel(Ptr5 in, const float* __restrict__ gfield, MPtr5 outp,
-                                                          float* cmax, SweepConst sc, long nrows) {
+                                                          float* cmax, SweepConst sc, long nrows,
+                                                          float* __restrict__ delta_out) {
     extern __shared__ float smem[];
     __shared__ int s_max;
     const int Cx = blockDim.x, nthr = blockDim.x * blockDim.y;
@@ -373,6 +374,12 @@ __global__ void __launch_bounds__(512) sweep_x_fwd_kernel(Ptr5 in, const float* 
 #pragma unroll
             for (int j = 0; j < K; ++j) v[j] = out[j][k];
             store_vec<K>(outp.p[k] + base, v);
+        }
+        if (delta_out) {                                   // next step's Poisson source: replaces source_init
+            float v[K];
+#pragma unroll
+            for (int j = 0; j < K; ++j) v[j] = fmaf(sc.src_flag, out[j][0], -sc.src_rho_bar);
+            store_vec<K>(delta_out + base, v);
         }
     }
     if (cmax) {
@@ -532,6 +539,8 @@ static SweepConst make_const(const dh_ctx* c, float lam, float kap) {
     sc.eps4 = (float)(4.0 * c->opt.lim_eps);
     sc.inv_lam = lam != 0.f ? 1.f / lam : 0.f;
     sc.N = c->N;
+    sc.src_flag = c->opt.gas_sources_gravity ? 1.f : 0.f;
+    sc.src_rho_bar = (float)c->rho_bar;
     return sc;
 }
 
@@ -585,7 +594,7 @@ static int yz_chain_threads(int N, int K, int halo, int max_c) {
 }
 
 int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
-                 float* cmax) {
+                 float* cmax, float* delta_out) {
     const int N = c->N;
     Prof prof(c, PROF_SWEEP_X + d);
     SweepConst sc = make_const(c, lam, kap);
@@ -599,10 +608,10 @@ int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam
         dim3 block; unsigned grid; long nrows = (long)N * N;
         x_geometry<KF>(N, block, grid, nrows);
         size_t sm = (size_t)FWD_SLOTS * block.x * block.y * sizeof(float);
-        if (g) DH_LAUNCH((sweep_x_fwd_kernel<KF, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
-        else DH_LAUNCH((sweep_x_fwd_kernel<KF, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
+        if (g) DH_LAUNCH((sweep_x_fwd_kernel<KF, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows, delta_out);
+        else DH_LAUNCH((sweep_x_fwd_kernel<KF, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows, delta_out);
     } else if (!c->tune_yz_chain) {
-        DH_TRY(launch_sweep_march(c, d, pin, g, pout, cmax, sc));
+        DH_TRY(launch_sweep_march(c, d, pin, g, pout, cmax, sc, delta_out));
     } else {
         const int C = yz_chain_threads(N, KF, 3, 16);
         const int S = C * KF - 6;

@@ -14,6 +14,7 @@ struct SweepConst {
     float e_floor;
     float eps4;      // 4 * lim_eps
     float inv_lam;   // 1 / lam (0 when lam == 0): the marching adjoint forms lam_b from u* - u
+    float src_flag, src_rho_bar;   // next step's Poisson source from this sweep's density: delta = src_flag rho' - src_rho_bar
     int N;
 };
 
@@ -190,7 +191,7 @@ __device__ __forceinline__ void block_sum3_to_global(float a, float b, float c, 
 
 // marching y/z kernels (sweep_march.cu); the field pointers are already permuted to (rho, m_n, m_t1, m_t2, eps)
 int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
-                       const SweepConst& sc);
+                       const SweepConst& sc, float* delta_out);
 int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, const Ptr5& pco, const MPtr5& pci,
                            float* gbar, double* scal, const SweepConst& sc);
 

@@ -113,7 +113,8 @@ constexpr int ADJ_BLOCKS = DH_ADJ_BLOCKS;        // adjoint: stages i-4 .. i are
 // block = (BX lanes along x, BY pencils); grid = (N / BX, N / BY, segments along the sweep axis)
 template <int DIR, bool HAS_G, bool EPS>
 __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const float* __restrict__ gfield, MPtr5 outp,
-                                                                 float* cmax, SweepConst sc, int S) {
+                                                                 float* cmax, SweepConst sc, int S,
+                                                                 float* __restrict__ delta_out) {
     constexpr int HALO = 3, NF = HAS_G ? 6 : 5;
     extern __shared__ float ring[];              // [RING][NF][nthr]
     __shared__ int s_max;
@@ -164,6 +165,7 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
         if (i >= 2 * HALO) {
 #pragma unroll
             for (int k = 0; k < 5; ++k) outp.p[k][off_out] = out[k];
+            if (delta_out) delta_out[off_out] = fmaf(sc.src_flag, out[0], -sc.src_rho_bar);   // replaces source_init
             off_out += stride;
         }
     }
@@ -413,15 +415,15 @@ static int march_segment(int N, int tuned, int halo) {
 
 template <int DIR>
 static int march_fwd_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const MPtr5& pout,
-                              float* cmax, const SweepConst& sc, int S, bool eps) {
+                              float* cmax, const SweepConst& sc, int S, bool eps, float* delta_out) {
     if (g) {
         const size_t sm = (size_t)RING * 6 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
-        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
+        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
     } else {
         const size_t sm = (size_t)RING * 5 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
-        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
+        else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
     }
     return DH_OK;
 }
@@ -442,14 +444,14 @@ static int march_adj_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin,
 }
 
 int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
-                       const SweepConst& sc) {
+                       const SweepConst& sc, float* delta_out) {
     const int N = c->N;
     const int S = march_segment(N, c->tune_march_s_fwd, 3);
     const dim3 block = march_block(N);
     const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
     const bool eps = c->opt.lim_eps > 1e-18;
-    if (d == 1) march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps);
-    else march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps);
+    if (d == 1) march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out);
+    else march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out);
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }

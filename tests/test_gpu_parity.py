@@ -701,6 +701,29 @@ def test_want_dsched_off_changes_only_the_schedule_cotangents(api, torch_, W, IC
     assert np.isnan(res[1][1]["dDtau"]) and np.isnan(res[1][1]["dkappa"])
 
 
+def test_run_source_priming_is_bit_identical(api, torch_, W, IC):
+    """Inside dh_run the last sweep of a step also writes the next step's Poisson source rho' - rho_bar (instead of a
+    source-init pass at the start of the next step): same numbers.  Self-gravitating gas without particles has no
+    atomics, so the two schedules must agree bit for bit; with particles they agree to the deposit's atomic order."""
+    cfg = W.scaled_config(0, 64, n_steps=7, a1=0.03)
+    _, gas, part = IC.coupled_ic(W, cfg)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    for nps in (0, cfg.N):
+        outs = []
+        for prime in (1, 0):
+            ctx = api.context_for(cfg, n_part_side=nps)
+            ctx.dh_tune("prime", prime)
+            sg = api.State(gas, part if nps else np.zeros((6, 0), dtype=np.float32), cfg.a0)
+            ctx.dh_run(sg, a_s[1:], dt_s, 3)
+            outs.append((sg.gas.clone(), ctx.dh_launch_count()))
+            ctx.close()
+        if nps == 0:
+            assert torch_.equal(outs[0][0], outs[1][0])
+        else:
+            assert float((outs[0][0] - outs[1][0]).abs().max() / outs[1][0].abs().max()) < 5e-6
+        assert outs[0][1] == outs[1][1] - (cfg.n_steps - 1)            # one launch fewer per step but the first
+
+
 def test_run_host_variant_matches_device_variant(api, torch_, W, IC):
     cfg = W.scaled_config(0, 32, n_steps=4, a1=0.02)
     delta, gas, part = IC.coupled_ic(W, cfg)
