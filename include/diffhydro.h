@@ -255,6 +255,19 @@ int dh_subgrid_step(dh_ctx* ctx, float* const gas[5], const float* g0, const flo
 int dh_subgrid_step_vjp(dh_ctx* ctx, float* const gas_in[5], const float* g0, const float* g1,
                         const dh_subgrid_params* par, float* const cot_gas[5], const float* cot_z, double* dpar_out);
 
+/* ---- cosmological-parameter gradients through the step scalars (sigma_8, Omega_m) --
+ * Every step has its own Dtau, kappa, K, A (reading R15), so chaining to a cosmological parameter needs the cotangents
+ * step by step, not their sums.  After a dh_run_vjp with dh_options.want_dsched = 1, dh_get_step_dparams copies them:
+ * out: HOST double[n_steps][5] = (dgamma, dDtau, dkappa, dK, dA) of steps 0 .. n_steps-1 of the last run (DH_ERR_STATE if
+ * the last dh_run_vjp did not keep them).  dh_chain_cosmology (host only, fp64): for the ln-a schedule of dh_schedule_lna
+ * it returns sum_steps sum_s dL/ds * ds/dtheta for theta = Omega_m (Omega_L fixed) and H0, ds/dtheta by central differences
+ * of the host's closed-form schedule and step factors; the initial state and the baryon fraction are held fixed (its own dependence on cosmology
+ * goes through dh_ic_zeldovich_vjp and the caller's transfer function).  Either output may be NULL.
+ * sigma_8: the state depends on it only through delta_init, dL/dsigma_8 = <dL/d delta_init, delta_init> / sigma_8. */
+int dh_get_step_dparams(dh_ctx* ctx, double* out, int n_steps);
+int dh_chain_cosmology(const dh_cosmology* cosmo, double a0, double a1, int n_steps, const double* step_dparams,
+                       double* dOmega_m, double* dH0);
+
 #ifdef __cplusplus
 }
 #endif

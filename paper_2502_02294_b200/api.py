@@ -29,7 +29,8 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_device_bytes", "dh_launch_count", "dh_sync", "dh_sweep", "dh_sweep_vjp", "dh_deposit", "dh_poisson",
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
-           "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp"]
+           "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
+           "dh_chain_cosmology"]
 
 
 class DhError(RuntimeError):
@@ -117,6 +118,8 @@ _lib.dh_subgrid_step.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POIN
                                  C.c_void_p, C.c_void_p]
 _lib.dh_subgrid_step_vjp.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POINTER(dh_subgrid_params), _P5,
                                      C.c_void_p, _dp]
+_lib.dh_get_step_dparams.argtypes = [C.c_void_p, _dp, C.c_int]
+_lib.dh_chain_cosmology.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_int, _dp, _dp, _dp]
 _lib.dh_power_spectrum.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
 _lib.dh_power_spectrum_vjp.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p]
 _lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
@@ -356,6 +359,20 @@ class Context:
                                         _ptrs(cot_gas, 5, _P5), cot_z.data_ptr() if cot_z is not None else None,
                                         d.ctypes.data_as(_dp)), "dh_subgrid_step_vjp")
         return d
+
+    def dh_get_step_dparams(self, n_steps: int) -> np.ndarray:
+        """(n_steps, 5) = (dgamma, dDtau, dkappa, dK, dA) per step of the last dh_run_vjp (want_dsched = 1)."""
+        out = np.zeros((int(n_steps), 5))
+        _check(_lib.dh_get_step_dparams(self._h, out.ctypes.data_as(_dp), int(n_steps)), "dh_get_step_dparams")
+        return out
+
+    def dh_chain_cosmology(self, a0, a1, step_dparams: np.ndarray):
+        """(dL/dOmega_m, dL/dH0) through the step scalars of the ln-a schedule (host arithmetic in the library)."""
+        sd = np.ascontiguousarray(step_dparams, dtype=np.float64)
+        dom, dh0 = C.c_double(0.0), C.c_double(0.0)
+        _check(_lib.dh_chain_cosmology(C.byref(self.cosmo), float(a0), float(a1), int(sd.shape[0]), sd.ctypes.data_as(_dp),
+                                       C.byref(dom), C.byref(dh0)), "dh_chain_cosmology")
+        return dom.value, dh0.value
 
     def dh_power_spectrum(self, field: torch.Tensor):
         """(P_b, count_b), b = 1 .. N/2, as host float64 arrays."""

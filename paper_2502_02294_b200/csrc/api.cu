@@ -393,7 +393,7 @@ int dh_free(dh_ctx* c) {
     for (auto p : c->gpb) cudaFree(p);
     for (auto p : c->cot_tmp) cudaFree(p);
     for (auto p : c->part_tmp) cudaFree(p);
-    cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev); cudaFree(c->ps_bins);
+    cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev); cudaFree(c->ps_bins); cudaFree(c->sg_scal); cudaFree(c->scal_log);
     cudaFree(c->hv_state); cudaFree(c->hv_cot);
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
@@ -612,6 +612,15 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
     if ((int)c->seg.size() < stride) c->seg.resize(stride);
     const int in_seg = stride < n ? stride : n;
     const bool taped = ensure_tapes(c, in_seg);
+    // per-step scalar cotangents (needed to chain to cosmological parameters: every step has its own d(scalars)/d(theta))
+    const bool per_step = c->opt.want_dsched != 0;
+    if (per_step && c->scal_log_cap < n) {
+        if (c->scal_log) dev_free(c, c->scal_log, (size_t)c->scal_log_cap * 8 * sizeof(double));
+        c->scal_log = nullptr; c->scal_log_cap = 0;
+        DH_TRY(dev_alloc(c, (void**)&c->scal_log, (size_t)n * 8 * sizeof(double)));
+        c->scal_log_cap = n;
+    }
+    c->step_dp.clear();
     for (int sgi = nseg - 1; sgi >= 0; --sgi) {
         const int k0 = sgi * stride, k1 = (k0 + stride < n) ? k0 + stride : n;
         // ---- re-run the segment from its snapshot: step k goes from seg[k - k0] (seg[0] is the snapshot itself) to
@@ -646,9 +655,65 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             DH_TRY(step_vjp_arrays(c, in.gas, in.part, s, in.step, cot_initial->gas, cot_initial->part, cot_initial->gas,
                                    cot_initial->part, taped ? &c->tapes[k - k0] : nullptr,
                                    c->run_gstore ? c->gstore[k].gp : nullptr));
+            if (per_step) {
+                DH_CUDA(cudaMemcpyAsync(c->scal_log + (size_t)8 * k, c->scal_dev, 8 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+                DH_CUDA(cudaMemsetAsync(c->scal_dev, 0, 8 * sizeof(double), c->stream));
+            }
         }
     }
-    return harvest_scalars(c, dp);
+    if (!per_step) return harvest_scalars(c, dp);
+    std::vector<double> h((size_t)8 * n);
+    DH_CUDA(cudaMemcpyAsync(h.data(), c->scal_log, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    c->step_dp.resize((size_t)5 * n);
+    for (int k = 0; k < n; ++k) {
+        const double* q = &h[(size_t)8 * k];
+        double* o = &c->step_dp[(size_t)5 * k];
+        o[0] = q[2]; o[1] = (q[0] + q[4]) / c->dx; o[2] = q[1]; o[3] = q[3]; o[4] = q[5];
+        if (dp) { dp->dgamma += o[0]; dp->dDtau += o[1]; dp->dkappa += o[2]; dp->dK += o[3]; dp->dA += o[4]; }
+    }
+    return DH_OK;
+}
+
+int dh_get_step_dparams(dh_ctx* c, double* out, int n_steps) {
+    if (!c || !out || n_steps <= 0) { set_error("dh_get_step_dparams: bad argument"); return DH_ERR_INVALID; }
+    if ((int)c->step_dp.size() < 5 * n_steps) {
+        set_error("dh_get_step_dparams: the last dh_run_vjp kept %d steps (needs dh_options.want_dsched = 1)", (int)c->step_dp.size() / 5);
+        return DH_ERR_STATE;
+    }
+    for (int i = 0; i < 5 * n_steps; ++i) out[i] = c->step_dp[i];
+    return DH_OK;
+}
+
+// dL/dOmega_m and dL/dH0 through the step scalars of an ln-a schedule (initial state held fixed): central differences, in
+// fp64 on the host, of the closed-form host functions dh_schedule_lna and step_scalars -- no device work.
+int dh_chain_cosmology(const dh_cosmology* co, double a0, double a1, int n, const double* step_dparams, double* dOmega_m,
+                       double* dH0) {
+    if (!co || !step_dparams || n <= 0 || co->static_mode) { set_error("dh_chain_cosmology: bad argument"); return DH_ERR_INVALID; }
+    auto scalars = [&](const dh_cosmology& q, std::vector<StepScalars>& out) -> int {
+        std::vector<double> a(n + 1), dt(n);
+        DH_TRY(dh_schedule_lna(&q, a0, a1, n, a.data(), dt.data()));
+        out.resize(n);
+        for (int k = 0; k < n; ++k) out[k] = step_scalars(q, a[k], a[k + 1], dt[k], k == 0 ? 0.0 : dt[k - 1]);
+        return DH_OK;
+    };
+    double* outs[2] = {dOmega_m, dH0};
+    for (int which = 0; which < 2; ++which) {
+        if (!outs[which]) continue;
+        dh_cosmology p = *co, m = *co;
+        const double h = which == 0 ? 1e-5 : 1e-5 * co->H0;
+        if (which == 0) { p.Omega_m += h; m.Omega_m -= h; } else { p.H0 += h; m.H0 -= h; }
+        std::vector<StepScalars> sp, sm;
+        DH_TRY(scalars(p, sp)); DH_TRY(scalars(m, sm));
+        double acc = 0.0;
+        for (int k = 0; k < n; ++k) {
+            const double* d = step_dparams + (size_t)5 * k;        // (dgamma, dDtau, dkappa, dK, dA)
+            acc += (d[1] * (sp[k].dtau - sm[k].dtau) + d[2] * (sp[k].kappa - sm[k].kappa) + d[3] * (sp[k].K - sm[k].K) +
+                    d[4] * (sp[k].A - sm[k].A)) / (2.0 * h);
+        }
+        *outs[which] = acc;
+    }
+    return DH_OK;
 }
 
 // ---------------------------------------------------------------------------------------------- host variants ----
@@ -778,6 +843,7 @@ int dh_power_spectrum(dh_ctx* c, const float* field, double* power_out, double* 
     DH_CUDA(cudaMemcpyAsync(h.data(), c->ps_bins, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(cudaStreamSynchronize(c->stream));
     const double norm = c->box * c->box * c->box / ((double)c->n3 * (double)c->n3);
+    c->ps_count.assign(h.begin() + nb1, h.end());
     for (int b = 1; b < nb1; ++b) {
         power_out[b - 1] = h[nb1 + b] > 0 ? norm * h[b] / h[nb1 + b] : 0.0;
         if (count_out) count_out[b - 1] = h[nb1 + b];
@@ -789,15 +855,19 @@ int dh_power_spectrum_vjp(dh_ctx* c, const float* field, const double* power_bar
     if (!c || !field || !power_bar || !field_bar) { set_error("dh_power_spectrum_vjp: null argument"); return DH_ERR_INVALID; }
     DH_TRY(ps_scratch(c, "dh_power_spectrum_vjp"));
     const int nb1 = c->N / 2 + 1;
-    // mode counts per bin (a property of the grid): one pass of the forward kernel gives them
-    DH_CUDA(cudaMemsetAsync(c->ps_bins, 0, (size_t)2 * nb1 * sizeof(double), c->stream));
-    DH_TRY(own_power_spectrum(c, field, c->ps_bins));
-    std::vector<double> h(2 * nb1);
-    DH_CUDA(cudaMemcpyAsync(h.data(), c->ps_bins, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    DH_CUDA(cudaStreamSynchronize(c->stream));
+    // mode counts per bin are a property of the grid: one pass of the forward kernel gives them, once per context
+    if ((int)c->ps_count.size() != nb1) {
+        DH_CUDA(cudaMemsetAsync(c->ps_bins, 0, (size_t)2 * nb1 * sizeof(double), c->stream));
+        DH_TRY(own_power_spectrum(c, field, c->ps_bins));
+        std::vector<double> h(2 * nb1);
+        DH_CUDA(cudaMemcpyAsync(h.data(), c->ps_bins, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        DH_CUDA(cudaStreamSynchronize(c->stream));
+        c->ps_count.assign(h.begin() + nb1, h.end());
+    }
+    const std::vector<double>& cnt = c->ps_count;
     const double norm = c->box * c->box * c->box / ((double)c->n3 * (double)c->n3);
     std::vector<float> g(nb1, 0.f);
-    for (int b = 1; b < nb1; ++b) g[b] = h[nb1 + b] > 0 ? (float)(2.0 * norm * power_bar[b - 1] / h[nb1 + b]) : 0.f;
+    for (int b = 1; b < nb1; ++b) g[b] = cnt[b] > 0 ? (float)(2.0 * norm * power_bar[b - 1] / cnt[b]) : 0.f;
     float* gtab = reinterpret_cast<float*>(c->ps_bins + 2 * nb1);
     DH_CUDA(cudaMemcpyAsync(gtab, g.data(), nb1 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     DH_CUDA(cudaStreamSynchronize(c->stream));             // g is a local: the copy must finish before it goes away
@@ -833,20 +903,14 @@ int dh_subgrid_step_vjp(dh_ctx* c, float* const gas_in[5], const float* g0, cons
     DH_TRY(check_subgrid(c, gas_in, g0, g1, par, "dh_subgrid_step_vjp"));
     if (!cot_gas) { set_error("dh_subgrid_step_vjp: null cotangent"); return DH_ERR_INVALID; }
     for (int k = 0; k < 5; ++k) if (!cot_gas[k]) { set_error("dh_subgrid_step_vjp: null cotangent %d", k); return DH_ERR_INVALID; }
-    double* scal = nullptr;
-    DH_TRY(dev_alloc(c, (void**)&scal, 4 * sizeof(double)));
-    int rc = DH_OK;
+    if (!c->sg_scal) DH_TRY(dev_alloc(c, (void**)&c->sg_scal, 4 * sizeof(double)));
     double h[4] = {0, 0, 0, 0};
-    if (cudaMemsetAsync(scal, 0, 4 * sizeof(double), c->stream) != cudaSuccess) rc = DH_ERR_CUDA;
-    if (rc == DH_OK) rc = launch_subgrid_vjp(c, gas_in, g0, g1, *par, cot_gas, cot_z, scal);
-    if (rc == DH_OK && (cudaMemcpyAsync(h, scal, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
-                        cudaStreamSynchronize(c->stream) != cudaSuccess)) {
-        set_error("dh_subgrid_step_vjp: %s", cudaGetErrorString(cudaGetLastError()));
-        rc = DH_ERR_CUDA;
-    }
-    dev_free(c, scal, 4 * sizeof(double));
-    if (rc == DH_OK && dpar_out) for (int j = 0; j < 4; ++j) dpar_out[j] += h[j];
-    return rc;
+    DH_CUDA(cudaMemsetAsync(c->sg_scal, 0, 4 * sizeof(double), c->stream));
+    DH_TRY(launch_subgrid_vjp(c, gas_in, g0, g1, *par, cot_gas, cot_z, c->sg_scal));
+    DH_CUDA(cudaMemcpyAsync(h, c->sg_scal, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    if (dpar_out) for (int j = 0; j < 4; ++j) dpar_out[j] += h[j];
+    return DH_OK;
 }
 
 int dh_data_term(dh_ctx* c, int observable, float* const gas[5], const float* data, const float* noise_var, double scale,

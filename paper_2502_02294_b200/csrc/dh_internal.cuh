@@ -114,6 +114,11 @@ struct dh_ctx {
     float* cmax_log = nullptr;     // 3 * cmax_cap floats
     int cmax_cap = 0;
     int cmax_n = 0;
+    std::vector<double> ps_count;  // modes per bin (a property of the grid), filled by the first power-spectrum call
+    double* scal_log = nullptr;    // per-step copies of scal_dev (8 doubles each) of the last dh_run_vjp with want_dsched
+    int scal_log_cap = 0;
+    std::vector<double> step_dp;   // host: per step (dgamma, dDtau, dkappa, dK, dA) of the last dh_run_vjp with want_dsched
+    double* sg_scal = nullptr;     // 4 doubles: parameter cotangents of the sub-grid step
     double* ps_bins = nullptr;     // power spectrum: [2][N/2+1] doubles + (behind them) N/2+1 floats of the transpose's table
     double* scal_dev = nullptr;    // 8 doubles: (lam_b, kap_b, gamma_b, K_b, dtau_drift_b, A_b, spare, spare)
 
