@@ -635,6 +635,47 @@ def test_subgrid_step_and_its_transpose_match_oracle(api, torch_, O, W, IC):
     ctx.close()
 
 
+def test_config2_full_run_forward_and_gradient(api, torch_, O, W, IC):
+    """Config 2 in full (64^3 cells and particles, 100 ln-a steps to a = 0.33, gas overdensities up to ~7): protocol (ii),
+    every field within 1e-3 of the fp64 oracle at the end; CFL maxima within 1e-4; then the gradient of
+    sum (rho_gas - rho_target)^2 (target: seed 2002) through the checkpointed reverse pass (stride 10).  After 100 steps of a
+    piecewise-differentiable scheme the fp64 gradient itself moves by a few per cent when its inputs move by one fp32
+    rounding (measured here, reading R28), so the state cotangents are held to 1.5 x that; d gamma, a smooth global sum,
+    to the north-star 1e-3."""
+    cfg = W.CONFIGS[2]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.target_seed, cfg.rms_delta))
+
+    def oracle(gas_, part_):
+        g, p, cm, _ = O.run(P, gas_, part_, cfg.a0, a_s[1:], dt_s)
+        cot = np.zeros_like(g); cot[0] = 2.0 * (g[0] - target)
+        return (g, p, cm) + tuple(O.run_vjp(P, gas_, part_, cfg.a0, a_s[1:], dt_s, cot, np.zeros_like(p)))
+    g_ref, p_ref, cm_ref, rg, rp, rdp = oracle(gas, part)
+    prng = np.random.default_rng(7)
+    _, _, _, rg2, rp2, rdp2 = oracle(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)),
+                                     part.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(part.shape)))
+    sens_g, sens_p = PT.rel_l2(rg2, rg), PT.rel_l2(rp2, rp)
+    ctx = api.context_for(cfg)
+    sg = api.State(gas, part, cfg.a0)
+    ctx.dh_run(sg, a_s[1:], dt_s, cfg.checkpoint_stride or 10)
+    e = PT.field_err(sg.gas.cpu().numpy(), g_ref)
+    e.update(PT.part_err(sg.part.cpu().numpy(), p_ref, cfg.N))
+    assert max(e.values()) < TOL_RUN, e
+    assert np.max(np.abs(ctx.dh_get_cmax(cfg.n_steps) / cm_ref - 1)) < 1e-4
+    cg = torch_.empty_like(sg.gas)
+    ctx.dh_data_term(0, sg.gas, _gpu(torch_, target), None, 1.0, 1.0, cg, want_loss=False)
+    ct = api.Cot(cg, torch_.zeros_like(sg.part))
+    dp = ctx.dh_run_vjp(ct, ct)
+    eg, ep = PT.rel_l2(ct.gas.cpu().numpy(), rg), PT.rel_l2(ct.part.cpu().numpy(), rp)
+    print(f"config2 full run: fields {max(e.values()):.2e}; gradient gas {eg:.2e} (ref moves {sens_g:.2e}), particles "
+          f"{ep:.2e} ({sens_p:.2e}), dgamma {dp.dgamma / rdp[0] - 1:.2e} (ref moves {rdp2[0] / rdp[0] - 1:.2e})")
+    assert eg < max(TOL_GRAD, 1.5 * sens_g) and ep < max(TOL_GRAD, 1.5 * sens_p)
+    assert abs(dp.dgamma / rdp[0] - 1) < TOL_GRAD
+    ctx.close()
+
+
 def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
     """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
     ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
