@@ -255,6 +255,18 @@ int dh_subgrid_step(dh_ctx* ctx, float* const gas[5], const float* g0, const flo
 int dh_subgrid_step_vjp(dh_ctx* ctx, float* const gas_in[5], const float* g0, const float* g1,
                         const dh_subgrid_params* par, float* const cot_gas[5], const float* cot_z, double* dpar_out);
 
+/* ---- the whole chain with HOST buffers (the call of a field-level inference loop) ----
+ *   delta_init --dh_ic_zeldovich--> state --dh_run(n_steps, stride)--> final gas --dh_data_term--> L
+ * and back: dL/d delta_init through dh_run_vjp and dh_ic_zeldovich_vjp.  delta_init_host, data_host, noise_var_host (may be
+ * NULL = 1), grad_delta_host: HOST, N^3 floats each (pinned memory makes the copies asynchronous); only these meshes cross
+ * the bus (12 or 16 B/cell up, 4 B/cell down), the 44 B/cell state never leaves the device.  loss_out: HOST double (may be
+ * NULL).  dparams: accumulated as in dh_run_vjp (may be NULL).  Synchronises the stream.  Needs gravity_on and one
+ * particle per cell; observable, scale, weight as in dh_data_term; a0, vel_factor, e_tilde0 as in dh_ic_zeldovich. */
+int dh_value_and_grad_host(dh_ctx* ctx, const float* delta_init_host, const float* data_host, const float* noise_var_host,
+                           int observable, double scale, double weight, double a0, double vel_factor, double e_tilde0,
+                           const double* a_sched, const double* dt_sched, int n_steps, int checkpoint_stride,
+                           float* grad_delta_host, double* loss_out, dh_dparams* dparams);
+
 /* ---- cosmological-parameter gradients through the step scalars (sigma_8, Omega_m) --
  * Every step has its own Dtau, kappa, K, A (reading R15), so chaining to a cosmological parameter needs the cotangents
  * step by step, not their sums.  After a dh_run_vjp with dh_options.want_dsched = 1, dh_get_step_dparams copies them:

@@ -30,7 +30,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
            "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
-           "dh_chain_cosmology"]
+           "dh_chain_cosmology", "dh_value_and_grad_host"]
 
 
 class DhError(RuntimeError):
@@ -118,6 +118,9 @@ _lib.dh_subgrid_step.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POIN
                                  C.c_void_p, C.c_void_p]
 _lib.dh_subgrid_step_vjp.argtypes = [C.c_void_p, _P5, C.c_void_p, C.c_void_p, C.POINTER(dh_subgrid_params), _P5,
                                      C.c_void_p, _dp]
+_lib.dh_value_and_grad_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_double, _dp, _dp, C.c_int, C.c_int, C.c_void_p, _dp,
+                                        C.POINTER(dh_dparams)]
 _lib.dh_get_step_dparams.argtypes = [C.c_void_p, _dp, C.c_int]
 _lib.dh_chain_cosmology.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_int, _dp, _dp, _dp]
 _lib.dh_power_spectrum.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
@@ -359,6 +362,23 @@ class Context:
                                         _ptrs(cot_gas, 5, _P5), cot_z.data_ptr() if cot_z is not None else None,
                                         d.ctypes.data_as(_dp)), "dh_subgrid_step_vjp")
         return d
+
+    def dh_value_and_grad_host(self, delta_init: torch.Tensor, data: torch.Tensor, noise_var: torch.Tensor | None, observable,
+                               scale, weight, a0, vel_factor, e_tilde0, a_sched, dt_sched, checkpoint_stride,
+                               grad_out: torch.Tensor, dparams: dh_dparams | None = None):
+        """HOST (ideally pinned) fp32 tensors in, grad_out (host) filled; returns (loss, dparams)."""
+        for t in (delta_init, data, grad_out) + ((noise_var,) if noise_var is not None else ()):
+            assert not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+        a_s = np.ascontiguousarray(a_sched, dtype=np.float64); dt_s = np.ascontiguousarray(dt_sched, dtype=np.float64)
+        dparams = dparams if dparams is not None else dh_dparams()
+        loss = C.c_double(0.0)
+        _check(_lib.dh_value_and_grad_host(self._h, delta_init.data_ptr(), data.data_ptr(),
+                                           noise_var.data_ptr() if noise_var is not None else None, int(observable),
+                                           float(scale), float(weight), float(a0), float(vel_factor), float(e_tilde0),
+                                           a_s.ctypes.data_as(_dp), dt_s.ctypes.data_as(_dp), len(dt_s),
+                                           int(checkpoint_stride), grad_out.data_ptr(), C.byref(loss), C.byref(dparams)),
+               "dh_value_and_grad_host")
+        return loss.value, dparams
 
     def dh_get_step_dparams(self, n_steps: int) -> np.ndarray:
         """(n_steps, 5) = (dgamma, dDtau, dkappa, dK, dA) per step of the last dh_run_vjp (want_dsched = 1)."""

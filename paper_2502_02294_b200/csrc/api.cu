@@ -394,7 +394,7 @@ int dh_free(dh_ctx* c) {
     for (auto p : c->cot_tmp) cudaFree(p);
     for (auto p : c->part_tmp) cudaFree(p);
     cudaFree(c->cmax_step); cudaFree(c->cmax_log); cudaFree(c->scal_dev); cudaFree(c->ps_bins); cudaFree(c->sg_scal); cudaFree(c->scal_log);
-    cudaFree(c->hv_state); cudaFree(c->hv_cot);
+    cudaFree(c->hv_state); cudaFree(c->hv_cot); cudaFree(c->hv_mesh);
     for (auto& s : c->snaps) cudaFree(s.buf);
     for (auto& s : c->seg) cudaFree(s.buf);
     for (auto& t : c->tapes) cudaFree(t.buf);
@@ -751,6 +751,43 @@ int dh_run_vjp_host(dh_ctx* c, float* cot_gas_host, float* cot_part_host, dh_dpa
     DH_TRY(dh_run_vjp(c, &ct, &ct, dp));
     DH_CUDA(cudaMemcpyAsync(cot_gas_host, ct.gas[0], (size_t)5 * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (c->np > 0) DH_CUDA(cudaMemcpyAsync(cot_part_host, ct.part[0], (size_t)6 * c->np * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaStreamSynchronize(c->stream));
+    return DH_OK;
+}
+
+// The whole chain of field-level inference with host buffers: delta_init -> state -> n steps -> data term, and back.
+int dh_value_and_grad_host(dh_ctx* c, const float* delta_init_host, const float* data_host, const float* noise_var_host,
+                           int observable, double scale, double weight, double a0, double vel_factor, double e_tilde0,
+                           const double* a_sched, const double* dt_sched, int n_steps, int stride, float* grad_delta_host,
+                           double* loss_out, dh_dparams* dp) {
+    if (!c || !delta_init_host || !data_host || !a_sched || !dt_sched || !grad_delta_host || n_steps <= 0 || stride <= 0) {
+        set_error("dh_value_and_grad_host: bad argument (needs n_steps > 0 and a checkpoint stride > 0)");
+        return DH_ERR_INVALID;
+    }
+    DH_TRY(hv_ensure(c, &c->hv_state));
+    DH_TRY(hv_ensure(c, &c->hv_cot));
+    if (!c->hv_mesh) DH_TRY(dev_alloc(c, (void**)&c->hv_mesh, (size_t)3 * c->n3 * sizeof(float)));
+    float* delta_d = c->hv_mesh;
+    float* data_d = c->hv_mesh + c->n3;                    // becomes the gradient once the data term has read it
+    float* noise_d = noise_var_host ? c->hv_mesh + 2 * c->n3 : nullptr;
+    const size_t mesh_bytes = (size_t)c->n3 * sizeof(float);
+    DH_CUDA(cudaMemcpyAsync(delta_d, delta_init_host, mesh_bytes, cudaMemcpyHostToDevice, c->stream));
+    DH_CUDA(cudaMemcpyAsync(data_d, data_host, mesh_bytes, cudaMemcpyHostToDevice, c->stream));
+    if (noise_d) DH_CUDA(cudaMemcpyAsync(noise_d, noise_var_host, mesh_bytes, cudaMemcpyHostToDevice, c->stream));
+    dh_state st;
+    dh_cot ct;
+    for (int k = 0; k < 5; ++k) { st.gas[k] = c->hv_state + (size_t)k * c->n3; ct.gas[k] = c->hv_cot + (size_t)k * c->n3; }
+    for (int k = 0; k < 6; ++k) {
+        st.part[k] = c->hv_state + (size_t)5 * c->n3 + (size_t)k * c->np;
+        ct.part[k] = c->hv_cot + (size_t)5 * c->n3 + (size_t)k * c->np;
+    }
+    DH_TRY(dh_ic_zeldovich(c, delta_d, a0, vel_factor, e_tilde0, &st));
+    DH_TRY(dh_run(c, &st, a_sched, dt_sched, n_steps, stride));
+    DH_CUDA(cudaMemsetAsync(ct.part[0], 0, (size_t)6 * c->np * sizeof(float), c->stream));   // the loss does not see particles
+    DH_TRY(dh_data_term(c, observable, st.gas, data_d, noise_d, scale, weight, ct.gas, loss_out));
+    DH_TRY(dh_run_vjp(c, &ct, &ct, dp));
+    DH_TRY(dh_ic_zeldovich_vjp(c, delta_d, vel_factor, e_tilde0, &ct, data_d));
+    DH_CUDA(cudaMemcpyAsync(grad_delta_host, data_d, mesh_bytes, cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(cudaStreamSynchronize(c->stream));
     return DH_OK;
 }

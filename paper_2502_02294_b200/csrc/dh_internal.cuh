@@ -152,6 +152,7 @@ struct dh_ctx {
     // host-variant device buffers
     float* hv_state = nullptr;     // 5 N^3 + 6 N_p
     float* hv_cot = nullptr;
+    float* hv_mesh = nullptr;      // 3 N^3: delta_init, data (then the gradient), noise variance of dh_value_and_grad_host
 };
 
 namespace dh {

@@ -765,6 +765,34 @@ def test_run_source_priming_is_bit_identical(api, torch_, W, IC):
         assert outs[0][1] == outs[1][1] - (cfg.n_steps - 1)            # one launch fewer per step but the first
 
 
+def test_value_and_grad_host_matches_the_device_composition(api, torch_, W, IC):
+    """dh_value_and_grad_host (delta_init, data on the host -> loss, dL/d delta_init on the host) against the same chain
+    composed from the device calls: same loss; gradient equal up to the deposit's atomic order (reading R28 bounds)."""
+    cfg = W.scaled_config(0, 32, n_steps=6, a1=0.03)
+    delta = W.gaussian_field(cfg.N, cfg.box, 31, cfg.rms_delta).astype(np.float32)
+    data = (cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, 32, cfg.rms_delta))).astype(np.float32)
+    nv = (1.0 + np.random.default_rng(3).uniform(size=delta.shape)).astype(np.float32)
+    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg)
+    dd = _gpu(torch_, delta)
+    st = ctx.dh_ic_zeldovich(dd, cfg.a0, vf, e0)
+    ctx.dh_run(st, a_s[1:], dt_s, 4)
+    cg = torch_.empty_like(st.gas)
+    loss_dev = ctx.dh_data_term(0, st.gas, _gpu(torch_, data), _gpu(torch_, nv), 1.0, 0.5, cg)
+    ct = api.Cot(cg, torch_.zeros_like(st.part))
+    dp_dev = ctx.dh_run_vjp(ct, ct)
+    grad_dev = ctx.dh_ic_zeldovich_vjp(dd, vf, e0, ct).cpu().numpy()
+    hgrad = torch_.zeros(delta.shape).pin_memory()
+    loss, dp = ctx.dh_value_and_grad_host(torch_.from_numpy(delta).pin_memory(), torch_.from_numpy(data).pin_memory(),
+                                          torch_.from_numpy(nv).pin_memory(), 0, 1.0, 0.5, cfg.a0, vf, e0, a_s[1:], dt_s, 4,
+                                          hgrad)
+    assert abs(loss / loss_dev - 1) < 1e-5
+    assert PT.rel_l2_trimmed(hgrad.numpy(), grad_dev, frac=1e-2) < TOL_GRAD and PT.rel_l2(hgrad.numpy(), grad_dev) < 5e-3
+    assert abs(dp.dgamma / dp_dev.dgamma - 1) < 1e-3
+    ctx.close()
+
+
 def test_run_host_variant_matches_device_variant(api, torch_, W, IC):
     cfg = W.scaled_config(0, 32, n_steps=4, a1=0.02)
     delta, gas, part = IC.coupled_ic(W, cfg)
