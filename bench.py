@@ -271,7 +271,7 @@ def main():
     if delta_h is not None:
         # the state comes from delta on the device (dh_ic_zeldovich); timed on its own, outside the step loop
         delta_d = torch.from_numpy(delta_h).cuda()
-        vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+        vf, e0 = api.ic_factors_for(cfg)
         ctx.dh_ic_zeldovich(delta_d, cfg.a0, vf, e0)                    # warm-up
         ev_ic = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         torch.cuda.synchronize()

@@ -206,6 +206,13 @@ int dh_kick_drift(dh_ctx* ctx, float* const g[3], float* const part[6], double K
  * DH_ERR_INVALID.  Asynchronous on the context's stream. */
 int dh_ic_zeldovich(dh_ctx* ctx, const float* delta_init, double a0, double vel_factor, double e_tilde0,
                     dh_state* state_out);
+/* The two scalar arguments above from physical inputs (HOST only, fp64, no device work; readings R18, R19, R27):
+ *   *vel_factor = a0^2 H(a0) f(a0), f = dlnD/dlna the linear growth rate of the matter + curvature + Lambda background of
+ *                 `cosmo` (Einstein-de Sitter: H0 sqrt(a0));
+ *   *e_tilde0   = a0^2 k_B T0 / ((gamma - 1) mu m_p) in (km/s)^2, T0 in K, mu the mean molecular weight (0.59 ionised).
+ * Either output may be NULL.  Errors: DH_ERR_INVALID. */
+int dh_ic_factors(const dh_cosmology* cosmo, double a0, double T0, double gamma, double mu, double* vel_factor,
+                  double* e_tilde0);
 /* Transpose of the Jacobian of dh_ic_zeldovich at delta_init applied to cot_state (gas cotangents required, particle
  * cotangent pointers may be NULL = zero): grad_delta (DEVICE, N^3 floats) is OVERWRITTEN with dL/d delta_init.
  * Together with dh_run_vjp this is "gradient w.r.t. the initial density field" in device memory. */

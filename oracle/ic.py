@@ -86,14 +86,39 @@ def zeldovich_state_vjp(delta: np.ndarray, N: int, L: float, f_b: float, vel_fac
     return f_b * rho_b + displacement_T(psi_b, L)
 
 
-# ---- the same for a workloads.Config (tests and the CPU-baseline legs)
-def state_of(delta, cfg, W):
-    return zeldovich_state(delta, cfg.N, cfg.box, cfg.f_b, W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0())
+# ---- the two factors of the map (readings R18, R19, R27).  The oracle's own statement of them: the CUDA library has its
+# own (dh_ic_factors); the two are compared in tests/, never shared.
+K_BOLTZMANN = 1.380649e-23          # J / K (SI definition)
+M_PROTON = 1.67262192369e-27        # kg (CODATA 2018)
+MU_IONISED = 0.59                   # mean molecular weight of fully ionised primordial gas (R18)
+
+
+def thermal_energy_tilde(a0: float, T0: float, gamma: float, mu: float = MU_IONISED) -> float:
+    """e~_0 = a0^2 e(T0),  e(T) = k_B T / ((gamma - 1) mu m_p)  in (km/s)^2  (R18, R27)."""
+    e_si = K_BOLTZMANN * T0 / ((gamma - 1.0) * mu * M_PROTON)      # m^2 / s^2
+    return a0 * a0 * e_si * 1e-6
+
+
+def velocity_factor_eds(H0: float, a: float) -> float:
+    """w = a^2 H(a) f(a) psi.  Einstein-de Sitter: H = H0 a^-3/2, D = a so f = 1:  a^2 H f = H0 sqrt(a)  (R19)."""
+    return H0 * np.sqrt(a)
+
+
+def ic_factors(cfg):
+    """(vel_factor, e_tilde0) of a workloads.Config (EdS only, like the configs of BASELINE.json)."""
+    assert cfg.Omega_L == 0.0 and abs(cfg.Omega_m - 1.0) < 1e-15, "the oracle states the EdS factor only"
+    return velocity_factor_eds(cfg.H0, cfg.a0), thermal_energy_tilde(cfg.a0, cfg.T0, cfg.gamma)
+
+
+# ---- the same for a workloads.Config (tests and the CPU-baseline legs); W supplies the seeded field only
+def state_of(delta, cfg, W=None):
+    vf, e0 = ic_factors(cfg)
+    return zeldovich_state(delta, cfg.N, cfg.box, cfg.f_b, vf, e0)
 
 
 def state_vjp_of(delta, cfg, W, cot_gas, cot_part):
-    return zeldovich_state_vjp(delta, cfg.N, cfg.box, cfg.f_b, W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0(), cot_gas,
-                               cot_part)
+    vf, e0 = ic_factors(cfg)
+    return zeldovich_state_vjp(delta, cfg.N, cfg.box, cfg.f_b, vf, e0, cot_gas, cot_part)
 
 
 def coupled_ic(W, cfg, seed=None):

@@ -30,7 +30,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
            "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
-           "dh_chain_cosmology", "dh_value_and_grad_host"]
+           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors"]
 
 
 class DhError(RuntimeError):
@@ -126,6 +126,7 @@ _lib.dh_chain_cosmology.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_dou
 _lib.dh_power_spectrum.argtypes = [C.c_void_p, C.c_void_p, _dp, _dp]
 _lib.dh_power_spectrum_vjp.argtypes = [C.c_void_p, C.c_void_p, _dp, C.c_void_p]
 _lib.dh_ic_zeldovich_vjp.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.POINTER(dh_cot), C.c_void_p]
+_lib.dh_ic_factors.argtypes = [C.POINTER(dh_cosmology), C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
 
 
 def _check(rc, where):
@@ -444,6 +445,21 @@ def dh_step_scalars(a_i, a_next, dt, dt_prev, H0=100.0, Omega_m=1.0, Omega_b=0.1
     _check(_lib.dh_step_scalars(C.byref(co), float(a_i), float(a_next), float(dt), float(dt_prev),
                                 out.ctypes.data_as(_dp)), "dh_step_scalars")
     return dict(dtau=out[0], kappa=out[1], K=out[2], A=out[3])
+
+
+def dh_ic_factors(a0, T0, gamma, mu=0.59, H0=100.0, Omega_m=1.0, Omega_b=0.16, Omega_L=0.0):
+    """(vel_factor, e_tilde0) = (a0^2 H f, a0^2 e(T0)): the scalar arguments of dh_ic_zeldovich (host call)."""
+    co = dh_cosmology(H0, Omega_m, Omega_b, Omega_L, 0)
+    vf, e0 = C.c_double(0.0), C.c_double(0.0)
+    _check(_lib.dh_ic_factors(C.byref(co), float(a0), float(T0), float(gamma), float(mu), C.byref(vf), C.byref(e0)),
+           "dh_ic_factors")
+    return vf.value, e0.value
+
+
+def ic_factors_for(cfg):
+    """dh_ic_factors for a workloads.Config."""
+    return dh_ic_factors(cfg.a0, cfg.T0, cfg.gamma, H0=cfg.H0, Omega_m=cfg.Omega_m, Omega_b=cfg.Omega_b,
+                         Omega_L=cfg.Omega_L)
 
 
 def context_for(cfg, **kw) -> Context:

@@ -190,8 +190,12 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
             const int d = order[sidx];
             for (int k = 0; k < 5; ++k)
                 nxt[k] = sidx == 2 ? gas_out[k] : (tape ? tape->sw[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
-            DH_TRY(launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr,
-                                (sidx == 2 && prime_next) ? c->delta : nullptr));
+            const int rc = launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr,
+                                        (sidx == 2 && prime_next) ? c->delta : nullptr);
+            if (rc != DH_OK) {                         // join the side stream before reporting: callers see one stream
+                if (beside) cudaStreamWaitEvent(c->stream, c->ev_join, 0);
+                return rc;
+            }
             for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
         }
         if (beside) DH_CUDA(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
@@ -825,6 +829,41 @@ int dh_poisson(dh_ctx* c, const float* delta, double A, float* const g_out[3]) {
 int dh_poisson_vjp(dh_ctx* c, float* const g_bar[3], double A, float* delta_bar_out) {
     if (!c || !g_bar || !delta_bar_out || !c->plans) { set_error("dh_poisson_vjp: bad argument or gravity off"); return DH_ERR_INVALID; }
     return poisson_adjoint(c, g_bar, (float)A, delta_bar_out);
+}
+
+// The two scalar arguments of the Zel'dovich map from physical inputs (host only, fp64).  vel_factor = a^2 H(a) f(a) with
+// the linear growth rate f = dlnD/dlna of a matter + curvature + Lambda background, D ~ H int_0^a da'/(a'H)^3:
+//   f = dlnH/dlna + a / ((aE)^3 I),  E = H/H0,  I = int_0^a da'/(a'E)^3   (Simpson in s = sqrt(a'/a): smooth integrand);
+// e_tilde0 = a0^2 k_B T0 / ((gamma-1) mu m_p) in (km/s)^2 (readings R18, R27).
+int dh_ic_factors(const dh_cosmology* co, double a0, double T0, double gamma, double mu, double* vel_factor,
+                  double* e_tilde0) {
+    if (!co || !(a0 > 0) || !(gamma > 1.0) || !(mu > 0) || !(T0 >= 0) || !(co->Omega_m > 0)) {
+        set_error("dh_ic_factors: need a0 > 0, gamma > 1, mu > 0, T0 >= 0, Omega_m > 0");
+        return DH_ERR_INVALID;
+    }
+    const double Om = co->Omega_m, OL = co->Omega_L, Ok = 1.0 - Om - OL;
+    auto E2 = [&](double a) { return Om / (a * a * a) + Ok / (a * a) + OL; };
+    if (vel_factor) {
+        const int M = 4096;
+        double acc = 0.0;
+        for (int j = 0; j <= M; ++j) {
+            const double s = (double)j / M, ap = a0 * s * s;
+            // da' = 2 a0 s ds;  1/(a'E)^3 = (a'^2 E2)^-3/2 with a'^2 E2 = Om/a' + Ok + OL a'^2
+            const double q = j == 0 ? 0.0 : 2.0 * a0 * s / std::pow(Om / ap + Ok + OL * ap * ap, 1.5);
+            acc += ((j == 0 || j == M) ? 1.0 : ((j & 1) ? 4.0 : 2.0)) * q;
+        }
+        const double I = acc / (3.0 * M);
+        const double e2 = E2(a0), E = std::sqrt(e2);
+        const double dlnH = (-3.0 * Om / (a0 * a0 * a0) - 2.0 * Ok / (a0 * a0)) / (2.0 * e2);
+        const double aE = a0 * E;
+        const double f = dlnH + a0 / (aE * aE * aE * I);
+        *vel_factor = a0 * a0 * co->H0 * E * f;
+    }
+    if (e_tilde0) {
+        const double kB = 1.380649e-23, mp = 1.67262192369e-27;     // J/K (SI), kg (CODATA 2018)
+        *e_tilde0 = a0 * a0 * (kB * T0 / ((gamma - 1.0) * mu * mp)) * 1e-6;
+    }
+    return DH_OK;
 }
 
 static int check_ic(const dh_ctx* c, const float* delta_init, const char* who) {

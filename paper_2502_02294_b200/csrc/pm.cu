@@ -388,7 +388,7 @@ __global__ void __launch_bounds__(256) dot3_kernel(const float4* __restrict__ a0
                                                    const float4* __restrict__ a2, const float4* __restrict__ b0,
                                                    const float4* __restrict__ b1, const float4* __restrict__ b2,
                                                    int64_t n4, double scale, double* out) {
-    __shared__ float sm[64];
+    __shared__ double smd[32];
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int64_t stride = (int64_t)gridDim.x * blockDim.x;
     double acc = 0.0;
@@ -404,7 +404,6 @@ __global__ void __launch_bounds__(256) dot3_kernel(const float4* __restrict__ a0
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    double* smd = reinterpret_cast<double*>(sm);
     const int t = threadIdx.x;
     if ((t & 31) == 0) smd[t >> 5] = acc;
     __syncthreads();

@@ -116,12 +116,13 @@ __device__ __forceinline__ float limL_grad(float A, float B, float eps4, float& 
     const float t = A * B;
     const float s = copysignf(eps4, A);
     const float den = (A + B) + s;
-    const float rd = rcp_fast(den);
     const bool on = t > 0.f;
-    const float rd2 = rd * rd;
-    LA = on ? B * (B + s) * rd2 : 0.f;
-    LB = on ? A * (A + s) * rd2 : 0.f;
-    return on ? t * rd : 0.f;
+    // gate on the reciprocal and never square it: with AB > 0, |den| >= 4 eps and |B| / |den|, |B + s| / |den| <= 1,
+    // whereas 1/den^2 overflows fp32 for |den| < 5.4e-20 (wave tails decaying into a uniform region, lim_eps = 1e-20)
+    const float rd = on ? rcp_fast(den) : 0.f;
+    LA = (B * rd) * ((B + s) * rd);
+    LB = (A * rd) * ((A + s) * rd);
+    return t * rd;
 }
 
 // Marching-kernel forms of the limiter.  EPS = false drops the sign(A) 4 eps term of the denominator: for

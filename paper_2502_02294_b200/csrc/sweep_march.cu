@@ -450,8 +450,8 @@ int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const 
     const dim3 block = march_block(N);
     const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
     const bool eps = c->opt.lim_eps > 1e-18;
-    if (d == 1) march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out);
-    else march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out);
+    if (d == 1) DH_TRY(march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out));
+    else DH_TRY(march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out));
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }
@@ -464,8 +464,12 @@ int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, co
     const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
     const bool eps = c->opt.lim_eps > 1e-18;
     const bool lk = c->opt.want_dsched != 0;
-    if (d == 1) { if (lk) march_adj_dispatch<1, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); else march_adj_dispatch<1, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); }
-    else { if (lk) march_adj_dispatch<2, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); else march_adj_dispatch<2, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps); }
+    int rc;
+    if (d == 1) rc = lk ? march_adj_dispatch<1, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps)
+                        : march_adj_dispatch<1, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    else rc = lk ? march_adj_dispatch<2, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps)
+                 : march_adj_dispatch<2, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    DH_TRY(rc);
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }

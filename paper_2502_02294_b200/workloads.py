@@ -1,7 +1,9 @@
 """Seeded synthetic inputs shaped like the paper's workloads (BASELINE.json configs 0-4).
 
 This module is the ONE thing the CPU oracle's tests and the CUDA path's tests share.  It holds input
-recipes only (numpy on the host) -- none of the step's arithmetic, no CUDA, no oracle import:
+recipes only (numpy on the host) -- none of the method's arithmetic (the factors of the Zel'dovich map, a^2 H f and
+e~(T0), are computed by each side on its own: dh_ic_factors in the library, oracle/ic.py in the oracle), no CUDA, no
+oracle import:
   * a seeded Gaussian random field with P(k) = A k^-2 exp(-(k/k_c)^2), k_c = k_Nyq/2, rescaled to the stated rms
     (stand-in for the paper's Eisenstein-Hu + LPT initial conditions; reading R19 in DESIGN.md);
     -- the field is the input; the Zel'dovich map  delta -> (gas, particles)  is part of the method: the CUDA path does
@@ -15,9 +17,6 @@ from __future__ import annotations
 
 from dataclasses import dataclass, field
 import numpy as np
-
-KB_OVER_MP = 8.2544e-3   # (km/s)^2 / K
-MU = 0.59
 
 
 @dataclass
@@ -42,7 +41,8 @@ class Config:
     T0: float = 1.0e4
     checkpoint_stride: int = 0
     lim_eps: float = 1e-20
-    e_floor_rel: float = 1e-3      # e_floor = e_floor_rel * initial e~  (R17)
+    e_floor_cosmo: float = 2.1e-5  # option dh_options.e_floor of the cosmological configs, (km/s)^2: about 1e-3 of the
+                                   # initial e~ (R17); a stated input, given identically to both sides
     extra: dict = field(default_factory=dict)
 
     @property
@@ -53,12 +53,8 @@ class Config:
     def f_b(self):
         return self.Omega_b / self.Omega_m
 
-    def e_tilde0(self):
-        """a0^2 e(T0): initial thermal energy per unit mass in tilde variables (R18, R27)."""
-        return self.a0 ** 2 * KB_OVER_MP * self.T0 / ((self.gamma - 1.0) * MU)
-
     def e_floor(self):
-        return 1e-12 if self.static_mode else self.e_floor_rel * self.e_tilde0()
+        return 1e-12 if self.static_mode else self.e_floor_cosmo
 
 
 CONFIGS = {
@@ -117,12 +113,6 @@ def gaussian_field(N: int, L: float, seed: int, rms: float) -> np.ndarray:
     d -= d.mean()
     d *= rms / np.sqrt(np.mean(d * d))
     return d
-
-
-def velocity_factor(cfg: Config, a: float) -> float:
-    """w = a^2 H(a) f(a) psi; EdS: H0 sqrt(a)."""
-    assert cfg.Omega_L == 0.0 and abs(cfg.Omega_m - 1.0) < 1e-15, "only EdS ICs are provided"
-    return cfg.H0 * np.sqrt(a)
 
 
 # ------------------------------------------------------------------ hydro ICs ------

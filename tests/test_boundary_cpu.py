@@ -87,3 +87,44 @@ def test_package_imports_without_cuda_and_has_no_fallback():
         from paper_2502_02294_b200 import api
         with pytest.raises(RuntimeError, match="no CPU fallback"):
             api.Context(32, 10.0, 1.4)
+
+
+def test_ic_factors_against_textbook_values(lib, IC):
+    """dh_ic_factors (the library's own statement of readings R18, R19, R27) and the oracle's (oracle/ic.py), each against
+    numbers neither computes: e(10^4 K) = 209.9 (km/s)^2 for gamma = 5/3, mu = 0.59, the sound speed of
+    ionised gas at 10^4 K (15.3 km/s), a^2 H f = H0 sqrt(a) in Einstein-de Sitter, and the growth rate of flat LambdaCDM,
+    f = dlnD/dlna from the growth ODE integrated in the test (and Omega_m(a)^0.55 to 1 %, Linder's fit), f -> 1 early."""
+    dp = C.POINTER(C.c_double)
+    vf, e0 = C.c_double(0), C.c_double(0)
+    eds = Cosmo(100.0, 1.0, 0.16, 0.0, 0)
+    assert lib.dh_ic_factors(C.byref(eds), C.c_double(1.0), C.c_double(1e4), C.c_double(5.0 / 3.0), C.c_double(0.59),
+                             C.byref(vf), C.byref(e0)) == 0
+    for e in (e0.value, IC.thermal_energy_tilde(1.0, 1e4, 5.0 / 3.0)):
+        assert abs(e - 209.9) < 0.05
+        assert abs(np.sqrt(5.0 / 3.0 * 2.0 / 3.0 * e) - 15.3) < 0.05
+    assert abs(e0.value / IC.thermal_energy_tilde(1.0, 1e4, 5.0 / 3.0) - 1) < 1e-14
+    for a in (0.01, 0.1, 0.5):
+        lib.dh_ic_factors(C.byref(eds), C.c_double(a), C.c_double(1e4), C.c_double(1.4), C.c_double(0.59), C.byref(vf), C.byref(e0))
+        assert abs(vf.value / (100.0 * np.sqrt(a)) - 1) < 1e-12
+        assert abs(IC.velocity_factor_eds(100.0, a) / (100.0 * np.sqrt(a)) - 1) < 1e-15
+        assert abs(e0.value / (a * a * IC.thermal_energy_tilde(1.0, 1e4, 1.4)) - 1) < 1e-14       # e~ = a^2 e
+    # flat LambdaCDM: the growth equation D'' + (2 + dlnH/dlna) D' = 1.5 Omega_m(a) D in x = ln a, integrated here
+    from scipy.integrate import solve_ivp
+    Om, OL = 0.31, 0.69
+
+    def rhs(x, y):
+        a = np.exp(x)
+        E2 = Om / a ** 3 + OL
+        return [y[1], -(2.0 - 1.5 * Om / a ** 3 / E2) * y[1] + 1.5 * Om / a ** 3 / E2 * y[0]]
+    sol = solve_ivp(rhs, [np.log(1e-4), 0.0], [1e-4, 1e-4], rtol=1e-10, atol=1e-14, dense_output=True)
+    lcdm = Cosmo(70.0, Om, 0.049, OL, 0)
+    for a in (0.01, 0.3, 0.5, 1.0):
+        lib.dh_ic_factors(C.byref(lcdm), C.c_double(a), C.c_double(0.0), C.c_double(1.4), C.c_double(0.59), C.byref(vf), None)
+        E = np.sqrt(Om / a ** 3 + OL)
+        f = vf.value / (a * a * 70.0 * E)
+        D, dD = sol.sol(np.log(a))
+        assert abs(f / (dD / D) - 1) < 1e-6, (a, f, dD / D)
+        assert abs(f / (Om / a ** 3 / E ** 2) ** 0.55 - 1) < 1e-2, (a, f)
+        if a == 0.01:
+            assert abs(f - 1) < 1e-5
+    assert lib.dh_ic_factors(C.byref(eds), C.c_double(-1.0), C.c_double(1e4), C.c_double(1.4), C.c_double(0.59), C.byref(vf), None) == -1

@@ -310,7 +310,7 @@ def test_config4_full_size_properties(api, torch_, W):
     N = cfg.N
     delta = torch_.from_numpy(W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)).cuda()
     ctx = api.context_for(cfg)
-    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+    vf, e0 = api.ic_factors_for(cfg)
     st0 = ctx.dh_ic_zeldovich(delta, cfg.a0, vf, e0)
     assert abs(float(st0.gas[0].double().mean()) / cfg.f_b - 1) < 1e-6            # delta has zero mean
     src = ctx.dh_deposit(st0.gas[0], st0.part[:3].contiguous())
@@ -493,7 +493,7 @@ def test_config0_gradient_of_final_density_norm(api, torch_, O, W, IC):
         ct = api.Cot(cg, torch_.zeros_like(sg.part))
         dp = ctx.dh_run_vjp(ct, ct)
         # the chain to the initial density field on the device as well (dh_ic_zeldovich_vjp)
-        gd = ctx.dh_ic_zeldovich_vjp(_gpu(torch_, delta), W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0(), ct)
+        gd = ctx.dh_ic_zeldovich_vjp(_gpu(torch_, delta), *api.ic_factors_for(cfg), ct)
         results.append((ct.gas.cpu().numpy(), ct.part.cpu().numpy(), dp.as_dict(), gd.cpu().numpy()))
     for (gg, gp, dp, gd) in results:
         eg, ep = PT.rel_l2(gg, rg), PT.rel_l2(gp, rp)
@@ -519,8 +519,10 @@ def test_ic_map_and_its_transpose_match_oracle(api, torch_, W, IC, N):
     (both maps are smooth: no gates, no floor)."""
     cfg = W.scaled_config(0, N, rms_delta=0.05)
     delta = W.gaussian_field(N, cfg.box, 77 + N, cfg.rms_delta).astype(np.float32)
-    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
-    g_ref, p_ref = IC.zeldovich_state(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf, e0)
+    vf, e0 = api.ic_factors_for(cfg)                 # the library's own a^2 H f and e~(T0) ...
+    vf_o, e0_o = IC.ic_factors(cfg)                  # ... against the oracle's own statement of them (readings R18, R19)
+    assert abs(vf / vf_o - 1) < 1e-12 and abs(e0 / e0_o - 1) < 1e-12
+    g_ref, p_ref = IC.zeldovich_state(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf_o, e0_o)
     ctx = api.context_for(cfg)
     dd = _gpu(torch_, delta)
     st = ctx.dh_ic_zeldovich(dd, cfg.a0, vf, e0)
@@ -531,7 +533,7 @@ def test_ic_map_and_its_transpose_match_oracle(api, torch_, W, IC, N):
     rng = np.random.default_rng(N)
     cg = rng.standard_normal(g_ref.shape).astype(np.float32)
     cp = rng.standard_normal(p_ref.shape).astype(np.float32)
-    ref = IC.zeldovich_state_vjp(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf, e0, cg, cp)
+    ref = IC.zeldovich_state_vjp(delta.astype(np.float64), N, cfg.box, cfg.f_b, vf_o, e0_o, cg, cp)
     got = ctx.dh_ic_zeldovich_vjp(dd, vf, e0, api.Cot(cg, cp)).cpu().numpy()
     assert PT.rel_l2(got, ref) < 1e-5, PT.rel_l2(got, ref)
     # the state it makes is the state the step accepts: one step runs and stays finite
@@ -557,7 +559,7 @@ def test_data_term_matches_oracle(api, torch_, W, IC, observable):
     cfg = W.scaled_config(0, N, rms_delta=0.05)
     _, gas, _ = IC.coupled_ic(W, cfg)
     rng = np.random.default_rng(observable)
-    scale = 1.0 if observable == 0 else 1.0 / cfg.e_tilde0()
+    scale = 1.0 if observable == 0 else 1.0 / api.ic_factors_for(cfg)[1]
     data = rng.standard_normal((N, N, N)).astype(np.float32)
     nv = (1.0 + rng.uniform(size=(N, N, N))).astype(np.float32)
     L_ref, cot_ref = IC.data_term(gas, data, nv, scale, 0.5, observable)
@@ -599,11 +601,11 @@ def test_subgrid_step_and_its_transpose_match_oracle(api, torch_, O, W, IC):
     N = 64
     cfg = W.scaled_config(0, N, rms_delta=0.3)
     _, gas, part = IC.coupled_ic(W, cfg)
-    gas[1:4] *= 0.1; gas[4] = gas[0] * cfg.e_tilde0() * (1 + 0.3 * np.sin(np.arange(N))[None, None, :]) \
+    gas[1:4] *= 0.1; gas[4] = gas[0] * api.ic_factors_for(cfg)[1] * (1 + 0.3 * np.sin(np.arange(N))[None, None, :]) \
         + 0.5 * np.sum(gas[1:4].astype(np.float64) ** 2, axis=0).astype(np.float32) / gas[0]      # moderate Mach number
     rng = np.random.default_rng(11)
     g0 = rng.gumbel(size=(N, N, N)).astype(np.float32); g1 = rng.gumbel(size=(N, N, N)).astype(np.float32)
-    e0 = cfg.e_tilde0()
+    e0 = api.ic_factors_for(cfg)[1]
     T0 = 1e4
     par = dict(rho_mean=cfg.f_b, t_per_e=T0 / e0, T_c=1.2e4, delta_c=0.2, Pi0=0.3, e_inject=3.0 * e0, a_width=0.25,
                b_width=2e3, tau=0.1)
@@ -772,7 +774,7 @@ def test_value_and_grad_host_matches_the_device_composition(api, torch_, W, IC):
     delta = W.gaussian_field(cfg.N, cfg.box, 31, cfg.rms_delta).astype(np.float32)
     data = (cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, 32, cfg.rms_delta))).astype(np.float32)
     nv = (1.0 + np.random.default_rng(3).uniform(size=delta.shape)).astype(np.float32)
-    vf, e0 = W.velocity_factor(cfg, cfg.a0), cfg.e_tilde0()
+    vf, e0 = api.ic_factors_for(cfg)
     a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
     ctx = api.context_for(cfg)
     dd = _gpu(torch_, delta)

@@ -267,6 +267,7 @@ def test_cold_gas_tracks_dark_matter_in_linear_regime(O, W, IC):
     N = 16
     cfg = W.scaled_config(0, N, n_steps=16, a1=0.04, rms_delta=2e-3)
     cfg.T0 = 1.0     # cold: negligible pressure
+    cfg.e_floor_cosmo = 2.1e-9
     delta, gas, part = IC.coupled_ic(W, cfg, seed=21)
     P = O.make_params(cfg.N, cfg.box, cfg.gamma, e_floor=cfg.e_floor())
     a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
