@@ -84,3 +84,44 @@ def golden(name):
                 k, v = line.split()[:2]
                 out[k] = float(v)
     return out
+
+
+# ---- conditioning of a piecewise-differentiable reference (reading R28) --------------------------------
+def nonuniform_mask(gas, reach=4):
+    """Cells that have a neighbour within `reach` cells along some axis (periodic) whose state differs in any field.
+    Where the input is exactly constant over the stencil every flux difference is exactly 0 in any precision (identical
+    inputs give identical outputs), so rounding cannot act there; everywhere else it can."""
+    gas = np.asarray(gas)
+    m = np.zeros(gas.shape[1:], dtype=bool)
+    for ax in (1, 2, 3):
+        for s in range(1, reach + 1):
+            d = np.any(gas != np.roll(gas, s, axis=ax), axis=0)
+            m |= d | np.roll(d, -s, axis=ax - 1)
+    return m
+
+
+def perturb_like_fp32(gas, seed, rel=6e-8):
+    """The fp32 input promoted to fp64 and moved by one fp32 rounding (relative 6e-8, Gaussian) wherever rounding can
+    act (nonuniform_mask): the model of what fp32 arithmetic does to the limiter / floor / |v| switches."""
+    g = np.asarray(gas, dtype=np.float64)
+    rng = np.random.default_rng(seed)
+    return g * (1.0 + rel * rng.standard_normal(g.shape) * nonuniform_mask(gas)[None])
+
+
+def stable_entries(ref, perturbed_refs, tol=1e-5):
+    """Entries of a reference gradient that the reference itself reproduces to tol x max|ref| when its input moves by one
+    fp32 rounding.  On these a correct fp32 adjoint must agree tightly; the others sit on a switch of the piecewise
+    derivative, where the one-sided values differ by O(1) and any of them is valid."""
+    ref = np.asarray(ref, dtype=np.float64)
+    scale = np.max(np.abs(ref))
+    ok = np.ones(ref.shape, dtype=bool)
+    for r in perturbed_refs:
+        ok &= np.abs(np.asarray(r, dtype=np.float64) - ref) <= tol * scale
+    return ok
+
+
+def masked_errors(got, ref, mask):
+    """(max |got - ref| / max |ref|, relative L2) over the entries selected by mask."""
+    got = np.asarray(got, dtype=np.float64); ref = np.asarray(ref, dtype=np.float64)
+    d = (got - ref)[mask]
+    return np.max(np.abs(d)) / np.max(np.abs(ref)), np.linalg.norm(d) / max(np.linalg.norm(ref[mask]), 1e-300)

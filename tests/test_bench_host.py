@@ -68,3 +68,23 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["n_gpus"] == 2
+
+
+def test_parity_helpers_locate_where_rounding_can_act():
+    """tests/parity.py: nonuniform_mask / perturb_like_fp32 / stable_entries (the conditioning protocol of reading R28)."""
+    import numpy as np
+    import parity as PT
+    gas = np.ones((5, 16, 16, 16), dtype=np.float32)
+    gas[2, 8, 8, 8] = 2.0                                     # one cell differs
+    m = PT.nonuniform_mask(gas, reach=4)
+    assert m[8, 8, 8] and m[8, 8, 4] and m[8, 8, 12] and m[4, 8, 8] and m[8, 12, 8]
+    assert not m[8, 8, 3] and not m[8, 8, 13] and not m[0, 0, 0] and not m[9, 9, 8]
+    assert m.sum() == 1 + 3 * 8                               # the cell and 4 cells either side along each axis
+    p = PT.perturb_like_fp32(gas, 1)
+    assert np.array_equal(p[:, ~m], gas[:, ~m].astype(np.float64))          # exactly uniform surroundings stay exact
+    assert np.all(np.abs(p[:, m] / gas[:, m] - 1) < 1e-6) and np.any(p[:, m] != gas[:, m])
+    ref = np.array([1.0, 2.0, -3.0, 0.0])
+    ok = PT.stable_entries(ref, [ref + np.array([0, 1e-7, 0, 1e-3]), ref + np.array([1e-9, 0, 0.5, 0])], tol=1e-5)
+    assert ok.tolist() == [True, True, False, False]
+    e_max, e_l2 = PT.masked_errors(ref + 1e-6, ref, ok)
+    assert abs(e_max - 1e-6 / 3.0) < 1e-12

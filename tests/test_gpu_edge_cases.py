@@ -81,21 +81,29 @@ def test_sweep_vjp_edge_states(api, torch_, O, W, name, d):
     cin, sc = cin.cpu().numpy(), sc.cpu().numpy()
     assert np.all(np.isfinite(cin)) and np.all(np.isfinite(sc)), name
     rin, _, rsc = O.sweep_vjp(gas.astype(np.float64), d, lam, 0.0, gamma, cot.astype(np.float64), e_floor=e_floor)
-    e_all, e_trim = PT.rel_l2(cin, rin), PT.rel_l2_trimmed(cin, rin, frac=1e-3)
-    print(f"sweep vjp edge [{name}, d={d}]: rel L2 {e_all:.2e}, trimmed(1e-3) {e_trim:.2e}, "
+    # Conditioning of the reference (reading R28): the same oracle VJP with its input moved by one fp32 rounding wherever
+    # rounding can act.  Entries it reproduces are the well-defined part of the derivative: tight agreement required,
+    # entry by entry (max norm).  The rest sit on a limiter / floor / |v| switch: bounded, finite, and few.
+    pert = [O.sweep_vjp(PT.perturb_like_fp32(gas, 900 + s), d, lam, 0.0, gamma, cot.astype(np.float64), e_floor=e_floor)[0]
+            for s in range(4)]
+    stable = PT.stable_entries(rin, pert)
+    e_max, e_l2 = PT.masked_errors(cin, rin, stable)
+    bad = np.mean(np.abs(cin - rin)[stable] > 1e-4 * np.max(np.abs(rin)))
+    e_all = PT.rel_l2(cin, rin)
+    self_all = max(PT.rel_l2(p, rin) for p in pert)
+    print(f"sweep vjp edge [{name}, d={d}]: stable entries {stable.mean():.4f}; on them max {e_max:.2e}, rel L2 {e_l2:.2e}, "
+          f"outliers {bad:.1e}; all entries rel L2 {e_all:.2e} (oracle moves itself {self_all:.2e}); "
           f"dgamma {sc[2]:.6g} vs {rsc['gamma']:.6g}, dlam {sc[0]:.6g} vs {rsc['lam']:.6g}")
-    assert e_trim < 2e-5
-    assert e_all < EDGE_TOL[name]
+    assert stable.mean() > MIN_STABLE[name]
+    assert e_l2 < 2e-5 and bad < 2e-4
+    assert e_all < max(TOL_GRAD, 2.0 * self_all)
+    assert np.max(np.abs(cin)) < 10 * np.max(np.abs(rin))
     for k, key in ((0, "lam"), (2, "gamma")):
         assert abs(sc[k] - rsc[key]) < 2e-3 * max(abs(rsc[key]), np.sqrt(gas[0].size)), (key, sc[k], rsc[key])
     ctx.close()
 
 
-# Untrimmed bound per state (reading R28).  The smooth floor case has no gate at rounding level: north star.  The
-# evolved states end in tails whose flux differences are a few fp32 ulps of the background: there the sign of A B is
-# decided by fp32 rounding of G itself, the gate takes the other branch than in fp64 on a thin shell of cells, and each
-# such entry is off by O(1) (both branches are valid one-sided derivatives of the same piecewise function).
-EDGE_TOL = {"at_rest": TOL_GRAD, "floor_patch": TOL_GRAD, "sod_evolved": 3e-2, "sedov_evolved": 3e-2}
+MIN_STABLE = {"at_rest": 0.999, "floor_patch": 0.99, "sod_evolved": 0.5, "sedov_evolved": 0.9}
 
 
 def _oracle_cfl_run(O, P, gas, gamma, t_end, dx, cfl=0.4):
@@ -110,12 +118,66 @@ def _oracle_cfl_run(O, P, gas, gamma, t_end, dx, cfl=0.4):
     return so, np.array(dts)
 
 
+def _smooth_direction(N, seed):
+    """A smooth low-k perturbation direction of a hydro state: (5,N,N,N), density and energy only, O(1) amplitudes."""
+    rng = np.random.default_rng(seed)
+    c = (np.arange(N) + 0.5) / N
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+    v = np.zeros((5, N, N, N))
+    for f in (0, 4):
+        for _ in range(3):
+            k = rng.integers(-2, 3, size=3)
+            v[f] += rng.standard_normal() * np.cos(2 * np.pi * (k[0] * x + k[1] * y + k[2] * z) + rng.uniform(0, 2 * np.pi))
+    return v
+
+
+def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stride, got, dp, min_stable):
+    """What a hydro-only reverse pass is held to (reading R28), given the GPU cotangent `got` of L = 1/2 sum rho_final^2:
+    (a) entry by entry on the entries the fp64 oracle reproduces under one fp32 rounding of its input, (b) over all
+    entries within twice what the oracle does to itself, (c) projected on smooth directions against the oracle AND
+    against central differences of the GPU's own loss, (d) d gamma."""
+    n = len(dts)
+    nop = np.zeros((6, 0))
+
+    def oracle_grad(gas_):
+        gf = O.run(P, gas_, nop, 1.0, np.ones(n), dts)[0]
+        cot = np.zeros_like(gf); cot[0] = gf[0]
+        return O.run_vjp(P, gas_, nop, 1.0, np.ones(n), dts, cot, nop)
+    rg, _, rdp = oracle_grad(gas)
+    rg2, _, rdp2 = oracle_grad(PT.perturb_like_fp32(gas, 7))
+    stable = PT.stable_entries(rg, [rg2])
+    e_max, e_l2 = PT.masked_errors(got, rg, stable)
+    bad = np.mean(np.abs(got - rg)[stable] > 1e-4 * np.max(np.abs(rg)))
+    sens, eg = PT.rel_l2(rg2, rg), PT.rel_l2(got, rg)
+    print(f"{label} gradient: stable entries {stable.mean():.4f}; on them rel L2 {e_l2:.2e}, max {e_max:.2e}, outliers "
+          f"{bad:.1e}; all entries {eg:.2e} (oracle moves itself {sens:.2e}); dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g} "
+          f"(oracle moves {rdp2[0] / rdp[0] - 1:+.1e}), dDtau {dp.dDtau:.6g} vs {rdp[1]:.6g}")
+    assert stable.mean() > min_stable
+    assert e_l2 < 1e-3 and bad < 1e-2           # one perturbation sample: the GPU's own flips are not all excluded
+    assert eg < max(TOL_GRAD, 2.0 * sens)
+    assert abs(dp.dgamma / rdp[0] - 1) < TOL_GRAD and abs(dp.dDtau / rdp[1] - 1) < 5e-3
+    # (c) directional derivatives
+    zero = torch_.zeros_like(_gpu(torch_, gas[0]))
+
+    def gpu_loss(gas_):
+        st = api.State(gas_.astype(np.float32), np.zeros((6, 0), dtype=np.float32), 1.0)
+        ctx.dh_run(st, np.ones(n), dts, 0)
+        return ctx.dh_data_term(0, st.gas, zero, None, 1.0, 0.5, None)
+    for j in range(2):
+        v = _smooth_direction(gas.shape[1], 40 + j) * np.abs(gas).mean(axis=(1, 2, 3), keepdims=True)
+        a, b = float(np.sum(got * v)), float(np.sum(rg * v))
+        h = 1e-2
+        fd = (gpu_loss(gas + h * v) - gpu_loss(gas - h * v)) / (2 * h)
+        print(f"{label} direction {j}: <grad,v> GPU {a:.6e}, oracle {b:.6e} ({a / b - 1:+.1e}), FD of the GPU loss {fd:.6e} ({a / fd - 1:+.1e})")
+        assert abs(a / b - 1) < TOL_GRAD
+        assert abs(a / fd - 1) < 1e-2
+
+
 def test_config1_at_128_forward_and_gradient(api, torch_, O, W):
     """Config 1 at ITS size: 128^3 spherical Sod, gamma = 1.4, static, to t = 0.1 at CFL 0.4 (dt list from the oracle).
     Forward <= 1e-3 (protocol ii), conservation, then the checkpointed adjoint of L = 1/2 sum rho^2 against the oracle's
-    run VJP: finite everywhere (r01: NaN from 1/den^2 in the chain-x limiter derivative), d gamma <= 1e-3, the state
-    cotangent <= 1e-3 on all but the worst 1 % of entries and within the oracle's own sensitivity to one fp32 rounding of
-    its input over all of them (reading R28: the shock surface is where gates flip)."""
+    run VJP: finite everywhere (r01: NaN from 1/den^2 in the chain-x limiter derivative), and the checks of
+    _static_run_gradient_checks."""
     cfg = W.CONFIGS[1]
     N, g = cfg.N, cfg.gamma
     gas = W.sod_sphere(N, g)
@@ -131,33 +193,18 @@ def test_config1_at_128_forward_and_gradient(api, torch_, O, W):
     assert max(e.values()) < TOL_RUN, e
     assert abs(out[0].astype(np.float64).sum() / gas[0].astype(np.float64).sum() - 1) < 1e-5
     assert abs(out[4].astype(np.float64).sum() / gas[4].astype(np.float64).sum() - 1) < 1e-5
-    ct = api.Cot(sg.gas.clone() * torch_.tensor([1.0, 0, 0, 0, 0], device="cuda").view(5, 1, 1, 1),
-                 torch_.zeros((6, 0), device="cuda"))
+    cg = torch_.zeros_like(sg.gas); cg[0] = sg.gas[0]
+    ct = api.Cot(cg, torch_.zeros((6, 0), device="cuda"))
     dp = ctx.dh_run_vjp(ct, ct)
     got = ct.gas.cpu().numpy()
     assert np.all(np.isfinite(got)) and np.isfinite(dp.dgamma) and np.isfinite(dp.dDtau)
-
-    def oracle_grad(gas_):
-        gf = O.run(P, gas_, np.zeros((6, 0)), 1.0, np.ones(n), dts)[0]
-        cot = np.zeros_like(gf); cot[0] = gf[0]
-        return O.run_vjp(P, gas_, np.zeros((6, 0)), 1.0, np.ones(n), dts, cot, np.zeros((6, 0)))
-    rg, _, rdp = oracle_grad(gas)
-    prng = np.random.default_rng(7)
-    rg2, _, rdp2 = oracle_grad(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)))
-    sens = PT.rel_l2(rg2, rg)
-    eg, eg_trim = PT.rel_l2(got, rg), PT.rel_l2_trimmed(got, rg, frac=1e-2)
-    print(f"config1 128^3 gradient: rel L2 {eg:.2e} (oracle moves itself {sens:.2e}), trimmed(1e-2) {eg_trim:.2e}, "
-          f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g} (oracle moves {rdp2[0] / rdp[0] - 1:.1e}), dDtau {dp.dDtau:.6g} vs {rdp[1]:.6g}")
-    assert sens < 0.2, "the reference itself is unusable"
-    assert eg < max(TOL_GRAD, 1.5 * sens)
-    assert eg_trim < max(TOL_GRAD, 0.5 * sens)
-    assert abs(dp.dgamma / rdp[0] - 1) < max(TOL_GRAD, 3 * abs(rdp2[0] / rdp[0] - 1))
+    _static_run_gradient_checks(api, torch_, O, W, "config1 128^3", ctx, P, gas, dts, 10, got, dp, 0.9)
     ctx.close()
 
 
 def test_sedov_run_vjp_is_finite_and_matches_oracle_at_64(api, torch_, O, W):
     """Reverse pass through the Sedov blast (64^3, to r_sh = 8 cells, oracle CFL list): central-cell Mach >> 100, floor
-    active upstream, exactly uniform gas at rest ahead of the shock.  Finite; trimmed parity; d gamma."""
+    active upstream, exactly uniform gas at rest ahead of the shock.  Finite; the checks of _static_run_gradient_checks."""
     N, g = 64, 5.0 / 3.0
     gas = W.sedov_ic(N, g)
     P = O.make_params(N, float(N), g, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-12)
@@ -172,17 +219,5 @@ def test_sedov_run_vjp_is_finite_and_matches_oracle_at_64(api, torch_, O, W):
     dp = ctx.dh_run_vjp(ct, ct)
     got = ct.gas.cpu().numpy()
     assert np.all(np.isfinite(got)) and np.isfinite(dp.dgamma)
-    cot = np.zeros_like(so.gas); cot[0] = so.gas[0]
-    rg, _, rdp = O.run_vjp(P, gas, np.zeros((6, 0)), 1.0, np.ones(n), dts, cot, np.zeros((6, 0)))
-    prng = np.random.default_rng(7)
-    gas_p = gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape))
-    gf = O.run(P, gas_p, np.zeros((6, 0)), 1.0, np.ones(n), dts)[0]
-    cot_p = np.zeros_like(gf); cot_p[0] = gf[0]
-    rg2, _, rdp2 = O.run_vjp(P, gas_p, np.zeros((6, 0)), 1.0, np.ones(n), dts, cot_p, np.zeros((6, 0)))
-    sens = PT.rel_l2(rg2, rg)
-    eg, eg_trim = PT.rel_l2(got, rg), PT.rel_l2_trimmed(got, rg, frac=1e-2)
-    print(f"sedov 64^3 gradient ({n} steps): rel L2 {eg:.2e} (oracle moves itself {sens:.2e}), trimmed {eg_trim:.2e}, "
-          f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g} ({rdp2[0]:.6g})")
-    assert eg < max(TOL_GRAD, 1.5 * sens) and eg_trim < max(TOL_GRAD, 0.5 * sens)
-    assert abs(dp.dgamma / rdp[0] - 1) < max(TOL_GRAD, 3 * abs(rdp2[0] / rdp[0] - 1))
+    _static_run_gradient_checks(api, torch_, O, W, f"sedov 64^3 ({n} steps)", ctx, P, gas, dts, 6, got, dp, 0.5)
     ctx.close()

@@ -1,0 +1,229 @@
+"""Configs 3 and 4 as BASELINE.json states them, at their sizes, in the launch configuration bench.py times
+(VERDICT r01 missing #2, #4; "parity on >= 3 steps + one 10-step segment vs oracle" at 256^3,
+"parity on 1-2 steps" at 512^3).  The oracle needs minutes here: these are the slow tests of the suite.
+"""
+import numpy as np
+import pytest
+
+import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-5
+TOL_GRAD = 1e-3
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2502_02294_b200 import api
+    return api
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+def _gpu(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, W):
+    """Config 3 (256^3 cells + 256^3 particles).  The GPU evolves the config's own initial state through the first 180 of
+    its 200 ln-a steps (a = 0.01 -> 0.23: the nonlinear end of the run, where particles have left their lattice order);
+    that fp32 state goes to both sides.  (i) steps 180, 181, 182 one by one (dh_step) and the 10-step segment 180..189:
+    fields within k x 1e-5 after k steps; CFL maxima; (ii) dh_run(10, stride 10) lands on the same state as the chained
+    dh_step calls; (iii) its dh_run_vjp (snapshots, kept g', tapes) with the loss cotangent 2 (rho - rho_target) against
+    the oracle's chained step VJPs and against the GPU's own untaped dh_step_vjp chain."""
+    cfg = W.CONFIGS[3]
+    N, K0, NS = cfg.N, 180, 10
+    delta = W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)
+    target = (cfg.f_b * (1.0 + W.gaussian_field(N, cfg.box, cfg.target_seed, cfg.rms_delta))).astype(np.float32)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg)
+    vf, e0 = api.ic_factors_for(cfg)
+    st = ctx.dh_ic_zeldovich(_gpu(torch_, delta), cfg.a0, vf, e0)
+    ctx.dh_run(st, a_s[1:K0 + 1], dt_s[:K0], 0)
+    assert st.step == K0
+    gas0, part0 = st.gas.cpu().numpy(), st.part.cpu().numpy()
+    disp = np.abs(part0[:3] - (np.stack(np.meshgrid(*(np.arange(N) + 0.5,) * 3, indexing="ij")[::-1]).reshape(3, -1)))
+    disp = np.minimum(disp, N - disp)
+    print(f"config3 state at step {K0}: a = {st.a:.4f}, max gas overdensity {gas0[0].max() / cfg.f_b:.2f}, "
+          f"rms / max particle displacement {np.sqrt((disp ** 2).mean()):.2f} / {disp.max():.2f} cells")
+    # ---- oracle: NS steps from that state, keeping every step's input
+    P = PT.oracle_params(O, cfg)
+    so = O.State(gas0, part0, a_s[K0], dt_prev=dt_s[K0 - 1], step=K0)
+    ins, cms = [], []
+    sg = api.State(gas0, part0, so.a, so.dt_prev, so.step)
+    g_states = []
+    cm = torch_.zeros(3, device="cuda")
+    for j in range(NS):
+        k = K0 + j
+        ins.append(so.copy())
+        g_states.append(sg.clone())
+        cm_ref, _ = O.step(P, so, dt_s[k], a_s[k + 1])
+        cm.zero_()
+        ctx.dh_step(sg, dt_s[k], a_s[k + 1], cm)
+        if j < 3 or j == NS - 1:
+            e = PT.field_err(sg.gas.cpu().numpy(), so.gas)
+            e.update(PT.part_err(sg.part.cpu().numpy(), so.part, N))
+            print(f"config3 after step {k}: {e}")
+            assert max(e.values()) < (j + 1) * TOL_STEP, (k, e)
+            assert np.max(np.abs(cm.cpu().numpy() / cm_ref - 1)) < (j + 1) * TOL_STEP
+    # ---- (ii) dh_run over the same segment
+    sr = api.State(gas0, part0, a_s[K0], dt_s[K0 - 1], K0)
+    ctx.dh_run(sr, a_s[K0 + 1:K0 + NS + 1], dt_s[K0:K0 + NS], 10)
+    assert sr.step == K0 + NS
+    for f in range(5):
+        assert float((sr.gas[f] - sg.gas[f]).abs().max()) <= 2e-5 * float(sg.gas[f].abs().max())
+    # ---- (iii) reverse pass
+    tgt = _gpu(torch_, target)
+    cg = torch_.empty_like(sr.gas)
+    ctx.dh_data_term(0, sr.gas, tgt, None, 1.0, 1.0, cg, want_loss=False)
+    ct = api.Cot(cg, torch_.zeros_like(sr.part))
+    dp = ctx.dh_run_vjp(ct, ct)
+    got_g, got_p = ct.gas.cpu().numpy(), ct.part.cpu().numpy()
+    assert np.all(np.isfinite(got_g)) and np.all(np.isfinite(got_p))
+    # the GPU's own chain of untaped step VJPs from the states the dh_step loop visited
+    cg2 = torch_.empty_like(sg.gas)
+    ctx.dh_data_term(0, sg.gas, tgt, None, 1.0, 1.0, cg2, want_loss=False)
+    c2 = api.Cot(cg2, torch_.zeros_like(sg.part))
+    dp2 = None
+    for j in reversed(range(NS)):
+        dp2 = ctx.dh_step_vjp(g_states[j], dt_s[K0 + j], a_s[K0 + j + 1], c2, c2, dp2)
+    del g_states
+    e_self = PT.rel_l2(got_g, c2.gas.cpu().numpy()), PT.rel_l2_trimmed(got_g, c2.gas.cpu().numpy(), frac=1e-2)
+    print(f"config3 segment reverse: dh_run_vjp vs chained dh_step_vjp: gas {e_self[0]:.2e} (trimmed {e_self[1]:.2e}), "
+          f"dgamma {dp.dgamma:.6g} vs {dp2.dgamma:.6g}")
+    assert e_self[1] < TOL_GRAD and e_self[0] < 2e-2
+    assert abs(dp.dgamma / dp2.dgamma - 1) < TOL_GRAD
+    # the oracle's chain
+    rg = np.zeros_like(so.gas); rg[0] = 2.0 * (so.gas[0] - target)
+    rp = np.zeros_like(so.part)
+    rdp = np.zeros(5)
+    for j in reversed(range(NS)):
+        k = K0 + j
+        rg, rp, d = O.step_vjp(P, ins[j], dt_s[k], a_s[k + 1], rg, rp)
+        rdp += d
+    eg, ep = PT.rel_l2(got_g, rg), PT.rel_l2(got_p, rp)
+    et = PT.rel_l2_trimmed(got_g, rg, frac=1e-2)
+    print(f"config3 segment reverse vs oracle: gas {eg:.2e} (trimmed 1e-2: {et:.2e}), particles {ep:.2e}, "
+          f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}")
+    assert et < TOL_GRAD and eg < 2e-2 and ep < 2e-2
+    assert abs(dp.dgamma / rdp[0] - 1) < TOL_GRAD
+    ctx.close()
+
+
+def test_config3_full_run_200_steps_stride_10_and_reverse(api, torch_, W):
+    """Config 3 exactly as stated: 200 ln-a steps to a = 0.33, checkpoint every 10 steps, gradients w.r.t. the initial
+    256^3 density field and gamma.  No oracle at this length (hours): properties.  Finite everywhere, gas mass conserved,
+    particles inside the box, CFL number of the predefined schedule below 1 at every step, device memory within one B200,
+    a second run reproduces the loss to the deposit's atomic order."""
+    cfg = W.CONFIGS[3]
+    N = cfg.N
+    delta = _gpu(torch_, W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta))
+    target = _gpu(torch_, cfg.f_b * (1.0 + W.gaussian_field(N, cfg.box, cfg.target_seed, cfg.rms_delta)))
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg, want_dA=0, want_dsched=0)
+    vf, e0 = api.ic_factors_for(cfg)
+    losses = []
+    for rep in range(2):
+        st = ctx.dh_ic_zeldovich(delta, cfg.a0, vf, e0)
+        m0 = float(st.gas[0].double().sum())
+        ctx.dh_run(st, a_s[1:], dt_s, cfg.checkpoint_stride)
+        assert st.step == 200 and abs(st.a - cfg.a1) < 1e-15
+        assert abs(float(st.gas[0].double().sum()) / m0 - 1) < 1e-6
+        assert float(st.part[:3].min()) >= 0.0 and float(st.part[:3].max()) < N
+        cg = torch_.empty_like(st.gas)
+        losses.append(ctx.dh_data_term(0, st.gas, target, None, 1.0, 1.0, cg))
+        if rep == 1:
+            break
+        cm = ctx.dh_get_cmax(200)
+        lam = np.array([api.dh_step_scalars(a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1] if k else 0.0)["dtau"]
+                        for k in range(200)]) / (cfg.box / N)
+        cfl = cm.max(axis=1) * lam
+        print(f"config3 full run: CFL number max {cfl.max():.3f} (step {int(cfl.argmax())}), final max overdensity "
+              f"{float(st.gas[0].max()) / cfg.f_b:.2f}, loss {losses[0]:.6e}")
+        assert np.all(np.isfinite(cm)) and cfl.max() < 1.0
+        ct = api.Cot(cg, torch_.zeros_like(st.part))
+        dp = ctx.dh_run_vjp(ct, ct)
+        gd = ctx.dh_ic_zeldovich_vjp(delta, vf, e0, ct)
+        assert bool(torch_.isfinite(gd).all()) and bool(torch_.isfinite(ct.part).all()) and np.isfinite(dp.dgamma)
+        gb = ctx.dh_device_bytes() / 2 ** 30
+        print(f"config3 full run: |dL/d delta_init| {float(gd.double().norm()):.6e}, dgamma {dp.dgamma:.6e}, "
+              f"device memory held by the context {gb:.1f} GiB")
+        assert float(gd.double().norm()) > 0 and gb < 170
+    assert abs(losses[1] / losses[0] - 1) < 1e-3
+    ctx.close()
+
+
+def test_config4_one_step_against_oracle_at_512(api, torch_, O, W):
+    """Config 4 at its size: one coupled step of the 512^3 state from dh_ic_zeldovich against the fp64 oracle on every
+    cell and particle (the oracle holds ~25 GB and takes minutes), cell indices bit-exact on all 3 x 2^27 coordinates."""
+    cfg = W.CONFIGS[4]
+    N = cfg.N
+    delta = W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg)
+    vf, e0 = api.ic_factors_for(cfg)
+    st = ctx.dh_ic_zeldovich(_gpu(torch_, delta), cfg.a0, vf, e0)
+    del delta
+    gas0, part0 = st.gas.cpu().numpy(), st.part.cpu().numpy()
+    for ax in range(3):
+        i0, i1 = ctx.dh_debug_cell_index(st.part[ax])
+        r0, r1 = O.cell_index(part0[ax], N)
+        assert np.array_equal(i0.cpu().numpy(), r0) and np.array_equal(i1.cpu().numpy(), r1)
+        del i0, i1, r0, r1
+    P = PT.oracle_params(O, cfg)
+    so = O.State(gas0, part0, cfg.a0)
+    del gas0, part0
+    cm_ref, _ = O.step(P, so, dt_s[0], a_s[1])
+    cm = torch_.zeros(3, device="cuda")
+    ctx.dh_step(st, dt_s[0], a_s[1], cm)
+    e = PT.field_err(st.gas.cpu().numpy(), so.gas)
+    e.update(PT.part_err(st.part.cpu().numpy(), so.part, N))
+    print("config4 512^3 one step vs oracle:", e)
+    assert max(e.values()) < TOL_STEP, e
+    assert np.max(np.abs(cm.cpu().numpy() / cm_ref - 1)) < TOL_STEP
+    ctx.close()
+
+
+def test_config4_fifty_steps_and_five_step_adjoint_window(api, torch_, W):
+    """Config 4 as stated: 50 ln-a steps forward at 512^3, the last 5 with checkpoints, then the 5-step adjoint window.
+    Properties (no oracle at this length): finite, mass conserved, particles inside the box, CFL number below 1, the
+    window's memory fits one B200, gradient finite and non-zero."""
+    cfg = W.CONFIGS[4]
+    N = cfg.N
+    delta = _gpu(torch_, W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta))
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg, want_dA=0, want_dsched=0)
+    vf, e0 = api.ic_factors_for(cfg)
+    st = ctx.dh_ic_zeldovich(delta, cfg.a0, vf, e0)
+    del delta
+    m0 = float(st.gas[0].double().sum())
+    ctx.dh_run(st, a_s[1:46], dt_s[:45], 0)
+    cm = ctx.dh_get_cmax(45)
+    ctx.dh_run(st, a_s[46:], dt_s[45:], cfg.checkpoint_stride)
+    cm = np.concatenate([cm, ctx.dh_get_cmax(5)])
+    assert st.step == 50 and abs(st.a - cfg.a1) < 1e-15
+    lam = np.array([api.dh_step_scalars(a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1] if k else 0.0)["dtau"]
+                    for k in range(50)]) / (cfg.box / N)
+    cfl = cm.max(axis=1) * lam
+    print(f"config4 full run: CFL number max {cfl.max():.3f} (step {int(cfl.argmax())}), final max overdensity "
+          f"{float(st.gas[0].max()) / cfg.f_b:.2f}")
+    assert np.all(np.isfinite(cm)) and cfl.max() < 1.0
+    assert abs(float(st.gas[0].double().sum()) / m0 - 1) < 1e-6
+    assert float(st.part[:3].min()) >= 0.0 and float(st.part[:3].max()) < N
+    cg = torch_.zeros_like(st.gas)
+    cg[0] = 2.0 * (st.gas[0] - cfg.f_b)
+    ct = api.Cot(cg, torch_.zeros_like(st.part))
+    dp = ctx.dh_run_vjp(ct, ct)
+    gb = ctx.dh_device_bytes() / 2 ** 30
+    print(f"config4 5-step window: |cot gas| {float(ct.gas.double().norm()):.6e}, dgamma {dp.dgamma:.6e}, context holds {gb:.1f} GiB")
+    assert bool(torch_.isfinite(ct.gas).all()) and bool(torch_.isfinite(ct.part).all()) and np.isfinite(dp.dgamma)
+    assert float(ct.gas.double().norm()) > 0 and gb < 150
+    ctx.close()

@@ -1,0 +1,179 @@
+"""The paper's own gradient check on the CUDA path (PAPER.md:294 Fig. 6, :312: "automatic derivatives ... compared with
+those calculated with finite differences"), i.e. evidence for the GPU gradient that does not come from the oracle
+(VERDICT r01 missing #5, weak #2), and the per-step late-time checks of ADVICE r01.
+
+Directional derivatives <dL/d delta_init, v> of the whole chain delta_init -> state -> n steps -> loss along smooth
+low-k directions v against central differences of the loss the LIBRARY returns (fp64 sum over fp32 fields), at three
+step sizes.  The loss is continuous and piecewise smooth (reading R28): finite differences average over the gate flips
+the pointwise gradient comparison is sensitive to, so this is the check that says whether the gradient is USEFUL.
+"""
+import numpy as np
+import pytest
+
+import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2502_02294_b200 import api
+    return api
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+def _gpu(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+class Chain:
+    """delta_init -> loss and dL/d delta_init, d/d gamma through the library's device calls."""
+
+    def __init__(self, api, torch, W, cfg, target, stride, gamma=None):
+        self.api, self.torch, self.cfg, self.stride = api, torch, cfg, stride
+        self.ctx = api.context_for(cfg, **({} if gamma is None else {"gamma": gamma}))
+        self.vf, self.e0 = api.ic_factors_for(cfg)            # reading R20: the initial state does not move with gamma
+        self.a_s, self.dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+        self.target = _gpu(torch, target)
+
+    def loss(self, delta, want_grad=False):
+        torch, ctx = self.torch, self.ctx
+        dd = _gpu(torch, delta)
+        st = ctx.dh_ic_zeldovich(dd, self.cfg.a0, self.vf, self.e0)
+        ctx.dh_run(st, self.a_s[1:], self.dt_s, self.stride if want_grad else 0)
+        if not want_grad:
+            return ctx.dh_data_term(0, st.gas, self.target, None, 1.0, 1.0, None)
+        cg = torch.empty_like(st.gas)
+        L = ctx.dh_data_term(0, st.gas, self.target, None, 1.0, 1.0, cg)
+        ct = self.api.Cot(cg, torch.zeros_like(st.part))
+        dp = ctx.dh_run_vjp(ct, ct)
+        g = ctx.dh_ic_zeldovich_vjp(dd, self.vf, self.e0, ct)
+        return L, g.double().cpu().numpy(), dp
+
+    def close(self):
+        self.ctx.close()
+
+
+def fd_table(chain, delta, dirs, hs):
+    """[(direction index, h, central difference of the loss)]"""
+    out = []
+    for j, v in enumerate(dirs):
+        for h in hs:
+            lp = chain.loss((delta + h * v).astype(np.float32))
+            lm = chain.loss((delta - h * v).astype(np.float32))
+            out.append((j, h, (lp - lm) / (2 * h)))
+    return out
+
+
+@pytest.mark.parametrize("which", [0, 2])
+def test_gpu_gradient_against_finite_differences_of_the_gpu_loss(api, torch_, O, W, IC, which):
+    """Configs 0 and 2 in full (20 steps to a = 0.1 at 32^3; 100 steps to a = 0.33 at 64^3), loss sum (rho - rho_t)^2.
+    <grad, v> from dh_run_vjp + dh_ic_zeldovich_vjp against central differences of the GPU loss for h = 0.1, 0.03, 0.01
+    (v has the rms of delta_init itself), and d/d gamma against a central difference over two more contexts."""
+    cfg = W.CONFIGS[which]
+    delta = W.gaussian_field(cfg.N, cfg.box, cfg.seed, cfg.rms_delta)
+    target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.target_seed or cfg.seed + 1000, cfg.rms_delta))
+    dirs = [W.gaussian_field(cfg.N, cfg.box, 9000 + j, cfg.rms_delta) for j in range(2)]
+    ch = Chain(api, torch_, W, cfg, target, 10)
+    L, g, dp = ch.loss(delta.astype(np.float32), want_grad=True)
+    assert np.isfinite(L) and np.all(np.isfinite(g))
+    # the same chain is deterministic up to the deposit's atomic order: the loss repeats to ~1e-7
+    L2 = ch.loss(delta.astype(np.float32))
+    assert abs(L2 / L - 1) < 1e-5
+    hs = (0.1, 0.03, 0.01)
+    worst = 0.0
+    for j, h, fd in fd_table(ch, delta, dirs, hs):
+        ad = float(np.sum(g * dirs[j]))
+        print(f"config{which} dir {j} h {h}: <grad,v> {ad:.6e}  FD {fd:.6e}  ratio-1 {ad / fd - 1:+.2e}")
+        if h == 0.01:
+            worst = max(worst, abs(ad / fd - 1))
+    ch.close()
+    assert worst < FD_TOL[which], worst
+    # d/d gamma
+    hg = 1e-3
+    lp = Chain(api, torch_, W, cfg, target, 10, gamma=cfg.gamma + hg)
+    lm = Chain(api, torch_, W, cfg, target, 10, gamma=cfg.gamma - hg)
+    fdg = (lp.loss(delta.astype(np.float32)) - lm.loss(delta.astype(np.float32))) / (2 * hg)
+    lp.close(); lm.close()
+    print(f"config{which} dgamma {dp.dgamma:.6e}  FD {fdg:.6e}  ratio-1 {dp.dgamma / fdg - 1:+.2e}")
+    assert abs(dp.dgamma / fdg - 1) < FD_TOL_GAMMA[which]
+
+
+# Measured on B200 (reading R28): config 0 agrees to ~1e-4, config 2 (100 steps, overdensities ~7) to ~1e-3 --
+# directional derivatives meet the north-star 1e-3 where the pointwise comparison cannot.
+FD_TOL = {0: 2e-3, 2: 1e-2}
+FD_TOL_GAMMA = {0: 5e-3, 2: 2e-2}
+
+
+def test_config0_directional_derivative_matches_the_oracle(api, torch_, O, W, IC):
+    """<grad, v> of config 0's chain: GPU against the fp64 oracle (run VJP + Zel'dovich transpose) -- the gate flips that
+    move individual entries by O(1) (R28) average out in a projection on a smooth direction."""
+    cfg = W.CONFIGS[0]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.seed + 1000, cfg.rms_delta))
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    g_ref, p_ref, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
+    cot = np.zeros_like(g_ref); cot[0] = 2.0 * (g_ref[0] - target)
+    rg, rp, rdp = O.run_vjp(P, gas, part, cfg.a0, a_s[1:], dt_s, cot, np.zeros_like(p_ref))
+    gd_ref = IC.state_vjp_of(delta, cfg, W, rg, rp)
+    ch = Chain(api, torch_, W, cfg, target, 10)
+    L, g, dp = ch.loss(delta.astype(np.float32), want_grad=True)
+    ch.close()
+    L_ref = float(np.sum((g_ref[0] - target) ** 2))
+    assert abs(L / L_ref - 1) < 1e-4
+    for j in range(3):
+        v = W.gaussian_field(cfg.N, cfg.box, 9000 + j, cfg.rms_delta)
+        a, b = float(np.sum(g * v)), float(np.sum(gd_ref * v))
+        print(f"config0 dir {j}: GPU {a:.6e} oracle {b:.6e} ratio-1 {a / b - 1:+.2e}")
+        assert abs(a / b - 1) < 1e-3
+    assert abs(dp.dgamma / rdp[0] - 1) < 1e-3
+
+
+@pytest.mark.parametrize("k", [50, 90, 99])
+def test_config2_late_step_vjp_matches_oracle(api, torch_, O, W, IC, k):
+    """chaos-independent late-time checks.  Config 2's GPU state after k steps (a up to 0.33, gas
+    overdensities ~7, particles displaced by several cells) goes to BOTH sides; one step and its VJP with a random
+    cotangent: fields <= 1e-5, cotangents <= 1e-3 everywhere and <= 2e-5 on all but the worst 0.1 % of entries."""
+    cfg = W.CONFIGS[2]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    ctx = api.context_for(cfg)
+    sg = api.State(gas, part, cfg.a0)
+    ctx.dh_run(sg, a_s[1:k + 1], dt_s[:k], 0)
+    gas_k, part_k = sg.gas.cpu().numpy(), sg.part.cpu().numpy()
+    so = O.State(gas_k, part_k, a_s[k], dt_prev=dt_s[k - 1], step=k)
+    s_in = so.copy()
+    cm_ref, _ = O.step(P, so, dt_s[k], a_s[k + 1])
+    cm = torch_.zeros(3, device="cuda")
+    s1 = sg.clone()
+    ctx.dh_step(s1, dt_s[k], a_s[k + 1], cm)
+    e = PT.field_err(s1.gas.cpu().numpy(), so.gas)
+    e.update(PT.part_err(s1.part.cpu().numpy(), so.part, cfg.N))
+    assert max(e.values()) < 1e-5, e
+    assert np.max(np.abs(cm.cpu().numpy() / cm_ref - 1)) < 1e-5
+    rng = np.random.default_rng(k)
+    cg = rng.standard_normal(gas.shape).astype(np.float32)
+    cp = rng.standard_normal(part.shape).astype(np.float32)
+    rg, rp, rdp = O.step_vjp(P, s_in, dt_s[k], a_s[k + 1], cg, cp)
+    co = api.Cot(cg, cp)
+    dp = ctx.dh_step_vjp(sg, dt_s[k], a_s[k + 1], co, co)
+    eg, ep = PT.rel_l2(co.gas.cpu().numpy(), rg), PT.rel_l2(co.part.cpu().numpy(), rp)
+    et = PT.rel_l2_trimmed(co.gas.cpu().numpy(), rg, frac=1e-3)
+    rho = gas_k[0] / cfg.f_b
+    print(f"config2 step {k} (max gas overdensity {rho.max():.2f}): fields {max(e.values()):.1e}; VJP gas {eg:.2e} "
+          f"(trimmed {et:.2e}), particles {ep:.2e}, dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}")
+    assert eg < 1e-3 and ep < 1e-3 and et < 2e-5
+    got = np.array([dp.dgamma, dp.dDtau, dp.dkappa, dp.dK, dp.dA])
+    scale = np.abs(rdp) + 1e-3 * np.max(np.abs(rdp))
+    assert np.all(np.abs(got - rdp) < 2e-3 * scale), (got, rdp)
+    ctx.close()

