@@ -127,27 +127,36 @@ __device__ __forceinline__ float limL_grad(float A, float B, float eps4, float& 
 
 // Marching-kernel forms of the limiter.  EPS = false drops the sign(A) 4 eps term of the denominator: for
 // 4 eps <= 4e-18 it changes L by at most 2 eps in absolute value (L = AB/(A+B) <= min(|A|,|B|)), far below one fp32
-// rounding of any flux the scheme produces; launchers pick EPS = true whenever lim_eps > 1e-18.
+// rounding of any flux the scheme produces; the forward launcher picks EPS = true whenever lim_eps > 1e-18.
 // The gate AB > 0 is applied to the reciprocal, so value and partials all vanish with one select.
+// With AB > 0 the signs of A, B and A + B agree, so  A + B + sign(A) 4 eps = sign(A) (|A + B| + 4 eps):  the epsilon
+// costs one FADD with free |.| modifiers instead of a sign transfer.
 template <bool EPS>
 __device__ __forceinline__ float limM(float A, float B, float eps4) {
     const float t = A * B;
-    float den = A + B;
-    if (EPS) den += copysignf(eps4, A);
-    const float r = t > 0.f ? rcp_fast(den) : 0.f;
+    if (EPS) {
+        const float r = t > 0.f ? rcp_fast(fabsf(A + B) + eps4) : 0.f;
+        return A * (fabsf(B) * r);
+    }
+    const float r = t > 0.f ? rcp_fast(A + B) : 0.f;
     return t * r;
 }
-// value and partials: with w = 1/den (0 when gated off), L = A B w, L_A = B (B + s) w^2, L_B = A (A + s) w^2
-template <bool EPS>
+// value and partials: with w = 1/|den| (0 when gated off), L = A |B| w, L_A = |B| (|B| + 4 eps) w^2, L_B likewise.
+// EPS = 2 ("denominator only", the adjoint's choice for 0 < lim_eps <= 1e-18): 4 eps stays in the denominator but not in
+// the two numerators.  Dropping it everywhere (EPS = 0) is harmless for the VALUE (|dL| <= 2 eps) but not for the
+// partials: where a wave tail decays into a background that is exactly zero (transverse momentum ahead of a shock)
+// |A|, |B| fall below 4 eps over ~10 cells and B^2/(A+B)^2 stays O(1) while the true partial B (B+s)/(A+B+s)^2 -> 0.
+// With 4 eps in the denominator only, the partials are wrong by at most 0.25 and only where |A| + |B| ~ 4 eps (a range of
+// one decade, less than a cell of such a tail), for one instruction per limiter.
+template <int EPS>
 __device__ __forceinline__ float limM_grad(float A, float B, float eps4, float& LA, float& LB) {
     const float t = A * B;
-    const float s = EPS ? copysignf(eps4, A) : 0.f;
-    const float den = (A + B) + s;
+    const float den = EPS ? fabsf(A + B) + eps4 : fabsf(A + B);
     const float r = t > 0.f ? rcp_fast(den) : 0.f;
-    const float wA = A * r, wB = B * r;
-    if (EPS) {
-        LA = wB * ((B + s) * r);
-        LB = wA * ((A + s) * r);
+    const float wA = fabsf(A) * r, wB = fabsf(B) * r;
+    if (EPS == 1) {
+        LA = wB * ((fabsf(B) + eps4) * r);
+        LB = wA * ((fabsf(A) + eps4) * r);
     } else {
         LA = wB * wB;
         LB = wA * wA;

@@ -108,6 +108,10 @@ constexpr int PF_ADJ = 2;
 #ifndef DH_ADJ_BLOCKS
 #define DH_ADJ_BLOCKS 3
 #endif
+#ifndef DH_ADJ_UNROLL
+#define DH_ADJ_UNROLL 2
+#endif
+constexpr int ADJ_UNROLL = DH_ADJ_UNROLL;
 constexpr int ADJ_BLOCKS = DH_ADJ_BLOCKS;        // adjoint: stages i-4 .. i are re-read, i+1 .. i+2 in flight, one spare
 
 // block = (BX lanes along x, BY pencils); grid = (N / BX, N / BY, segments along the sweep axis)
@@ -174,7 +178,7 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
 
 // ------------------------------------------------------------------------------------------------- adjoint ----
 // LK = false drops the cotangents of lam and kap (dh_options.want_dsched = 0): gamma_b only.
-template <bool HAS_G, bool EPS, bool LK>
+template <bool HAS_G, int EPS, bool LK>
 struct AdjPipe {
     // forward recompute
     float u1[5], g1, G1[5], D2[5];         // u_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
@@ -301,7 +305,7 @@ struct AdjPipe {
     }
 };
 
-template <int DIR, bool HAS_G, bool EPS, bool LK>
+template <int DIR, bool HAS_G, int EPS, bool LK>
 __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 in, const float* __restrict__ gfield,
                                                                           Ptr5 cot_out, MPtr5 cot_in,
                                                                           float* __restrict__ gbar, double* scal,
@@ -347,7 +351,7 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
     AdjPipe<HAS_G, EPS, LK> pipe;
     pipe.init();
     float lacc = 0.f, kacc = 0.f, gacc = 0.f;
-#pragma unroll 1
+#pragma unroll ADJ_UNROLL
     for (int i = 0; i < niter; ++i) {
         if (i + PF_ADJ < niter) issue(i + PF_ADJ);
         cp_async_commit();
@@ -416,31 +420,35 @@ static int march_segment(int N, int tuned, int halo) {
 template <int DIR>
 static int march_fwd_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const MPtr5& pout,
                               float* cmax, const SweepConst& sc, int S, bool eps, float* delta_out) {
+    const size_t sm = (size_t)RING * (g ? 6 : 5) * block.x * block.y * sizeof(float);
     if (g) {
-        const size_t sm = (size_t)RING * 6 * block.x * block.y * sizeof(float);
         if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
         else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
     } else {
-        const size_t sm = (size_t)RING * 5 * block.x * block.y * sizeof(float);
         if (eps) MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
         else MARCH_LAUNCH((sweep_march_fwd_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S, delta_out);
     }
     return DH_OK;
 }
 
+template <int DIR, bool LK, bool HAS_G, int EPS>
+static int march_adj_launch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const Ptr5& pco,
+                            const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S) {
+    const size_t sm = (size_t)RING * (HAS_G ? 11 : 10) * block.x * block.y * sizeof(float);
+    MARCH_LAUNCH((sweep_march_adj_kernel<DIR, HAS_G, EPS, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+    return DH_OK;
+}
+
+// eps_mode: 1 = sign(A) 4 eps in denominator and numerators (lim_eps > 1e-18), 2 = denominator only, 0 = lim_eps == 0
 template <int DIR, bool LK>
 static int march_adj_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr5& pin, const float* g, const Ptr5& pco,
-                              const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S, bool eps) {
-    if (g) {
-        const size_t sm = (size_t)RING * 11 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, true, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, true, false, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-    } else {
-        const size_t sm = (size_t)RING * 10 * block.x * block.y * sizeof(float);
-        if (eps) MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, true, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-        else MARCH_LAUNCH((sweep_march_adj_kernel<DIR, false, false, LK>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
-    }
-    return DH_OK;
+                              const MPtr5& pci, float* gbar, double* scal, const SweepConst& sc, int S, int eps_mode) {
+#define DH_ADJ_CASE(G_, E_) return march_adj_launch<DIR, LK, G_, E_>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S)
+    if (g) { if (eps_mode == 1) DH_ADJ_CASE(true, 1); if (eps_mode == 2) DH_ADJ_CASE(true, 2); DH_ADJ_CASE(true, 0); }
+    if (eps_mode == 1) DH_ADJ_CASE(false, 1);
+    if (eps_mode == 2) DH_ADJ_CASE(false, 2);
+    DH_ADJ_CASE(false, 0);
+#undef DH_ADJ_CASE
 }
 
 int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
@@ -462,7 +470,7 @@ int launch_sweep_march_vjp(dh_ctx* c, int d, const Ptr5& pin, const float* g, co
     const int S = march_segment(N, c->tune_march_s_adj, 4);
     const dim3 block = march_block(N);
     const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
-    const bool eps = c->opt.lim_eps > 1e-18;
+    const int eps = c->opt.lim_eps > 1e-18 ? 1 : (c->opt.lim_eps > 0.0 ? 2 : 0);
     const bool lk = c->opt.want_dsched != 0;
     int rc;
     if (d == 1) rc = lk ? march_adj_dispatch<1, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps)
