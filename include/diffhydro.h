@@ -3,8 +3,9 @@
  * One coupled time step of the relaxing-TVD finite-volume Euler solver and the dark-matter particle-mesh gravity
  * solver of Horowitz & Lukic, arXiv 2502.02294 (section 2.2 Eq. 2-3, section 2.3 Eq. 4-20), and that
  * step's reverse-mode adjoint (section 2.3.5, :198-220), as hand-written CUDA kernels for sm_100a.
- * cuFFT is used for the 3-D real transforms only.  There is no CPU fallback: dh_init fails with DH_ERR_NO_DEVICE
- * when no sm_100 device is present.
+ * The Poisson solve runs on the library's own 1-D FFT passes with the Green multiply fused into the z pass (grids
+ * whose side is a power of two); other sides fall back to cuFFT for the 3-D real transforms only.  There is no CPU
+ * fallback: dh_init fails with DH_ERR_NO_DEVICE when no sm_100 device is present.
  *
  * Conventions
  *   - Every entry point returns int: DH_OK (0) or a negative DH_ERR_* code; dh_last_error() gives a thread-local
@@ -90,7 +91,9 @@ typedef struct {
 /* ---- the four calls of the north star (+ dh_run_vjp, which consumes dh_run's checkpoints) ------------------- */
 
 /* Create a context for an N^3 grid in a periodic box of side `box` (h^-1 Mpc) with adiabatic index gamma.
- * Builds the cuFFT R2C/C2R plans and scratch meshes.  grid_n must be a multiple of 4, 8 <= grid_n <= 1024.
+ * Allocates the scratch meshes (and, for a side that is not a power of two, the cuFFT R2C/C2R plans; a power-of-two
+ * side makes them only when dh_tune("own_fft", 0) asks for the cuFFT route).  grid_n must be a multiple of 32,
+ * 32 <= grid_n <= 1024 (a warp's 32 lanes are 32 consecutive x in every mesh kernel).
  * Errors: DH_ERR_INVALID, DH_ERR_NO_DEVICE, DH_ERR_CUFFT, DH_ERR_OOM. */
 int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmology* cosmo, const dh_options* opt);
 int dh_free(dh_ctx* ctx);
@@ -165,7 +168,12 @@ int dh_sync(dh_ctx* ctx);
  *   "gstore": 0 makes a checkpointed dh_run NOT keep every step's g' (3 N^3 floats per step of the run) for
  *           dh_run_vjp, which then repeats deposit + Poisson solve in the segment re-run (default 1, same fallback).
  *   "own_fft": 0 routes the Poisson solve through cuFFT (1 R2C + multiply kernel + 3 C2R) instead of the library's own
- *           FFT passes fused with the Green multiply (default 1 when grid_n is a power of two).
+ *           FFT passes fused with the Green multiply (default 1 when grid_n is a power of two); the cuFFT plans are
+ *           made by this call when they do not exist yet (DH_ERR_CUFFT / DH_ERR_OOM);
+ *   "overlap": 0 keeps the particle update of a step on the caller's stream, before the sweeps, instead of forking it
+ *           onto the context's side stream beside them (default 1);
+ *   "prime": 0 makes every step of dh_run initialise its own Poisson source instead of letting the previous step's last
+ *           sweep write it (default 1; bit-identical either way).
  * Unknown key: DH_ERR_INVALID. */
 int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of

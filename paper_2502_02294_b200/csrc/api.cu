@@ -279,6 +279,35 @@ static int harvest_scalars(dh_ctx* c, dh_dparams* dp) {
     return DH_OK;
 }
 
+// cuFFT R2C / C2R plans sharing one work area, on the context's stream; made on first need.
+static int ensure_cufft_plans(dh_ctx* c) {
+    if (c->plans) return DH_OK;
+    const int n = c->N;
+    size_t w1 = 0, w2 = 0;
+    if (cufftCreate(&c->plan_r2c) != CUFFT_SUCCESS) { set_error("cufftCreate failed"); return DH_ERR_CUFFT; }
+    if (cufftCreate(&c->plan_c2r) != CUFFT_SUCCESS) {
+        cufftDestroy(c->plan_r2c);
+        set_error("cufftCreate failed"); return DH_ERR_CUFFT;
+    }
+    c->plans = true;
+    cufftSetAutoAllocation(c->plan_r2c, 0);
+    cufftSetAutoAllocation(c->plan_c2r, 0);
+    if (cufftMakePlan3d(c->plan_r2c, n, n, n, CUFFT_R2C, &w1) != CUFFT_SUCCESS ||
+        cufftMakePlan3d(c->plan_c2r, n, n, n, CUFFT_C2R, &w2) != CUFFT_SUCCESS) {
+        set_error("cufftMakePlan3d(%d^3) failed", n); return DH_ERR_CUFFT;
+    }
+    c->fft_work_bytes = w1 > w2 ? w1 : w2;
+    if (c->fft_work_bytes > 0) {
+        DH_TRY(dev_alloc(c, &c->fft_work, c->fft_work_bytes));
+        cufftSetWorkArea(c->plan_r2c, c->fft_work);
+        cufftSetWorkArea(c->plan_c2r, c->fft_work);
+    }
+    if (cufftSetStream(c->plan_r2c, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_c2r, c->stream) != CUFFT_SUCCESS) {
+        set_error("cufftSetStream failed"); return DH_ERR_CUFFT;
+    }
+    return DH_OK;
+}
+
 static int check_state(const dh_ctx* c, const float* const gas[5], const float* const part[6]) {
     for (int k = 0; k < 5; ++k) if (!gas[k]) { set_error("null gas pointer %d", k); return DH_ERR_INVALID; }
     if (c->np > 0) for (int k = 0; k < 6; ++k) if (!part[k]) { set_error("null particle pointer %d", k); return DH_ERR_INVALID; }
@@ -341,27 +370,9 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
         for (int i = 0; i < 4; ++i)
             if ((rc = dev_alloc(c, (void**)&c->spec[i], nspec * sizeof(float2))) != DH_OK) return fail(rc);
         if ((rc = alloc_fields(c, c->gp, 3, c->n3)) != DH_OK) return fail(rc);
-        // cuFFT plans share one work area
-        size_t w1 = 0, w2 = 0;
-        if (cufftCreate(&c->plan_r2c) != CUFFT_SUCCESS || cufftCreate(&c->plan_c2r) != CUFFT_SUCCESS) {
-            set_error("cufftCreate failed"); return fail(DH_ERR_CUFFT);
-        }
-        c->plans = true;
-        cufftSetAutoAllocation(c->plan_r2c, 0);
-        cufftSetAutoAllocation(c->plan_c2r, 0);
-        if (cufftMakePlan3d(c->plan_r2c, grid_n, grid_n, grid_n, CUFFT_R2C, &w1) != CUFFT_SUCCESS ||
-            cufftMakePlan3d(c->plan_c2r, grid_n, grid_n, grid_n, CUFFT_C2R, &w2) != CUFFT_SUCCESS) {
-            set_error("cufftMakePlan3d(%d^3) failed", grid_n); return fail(DH_ERR_CUFFT);
-        }
-        c->fft_work_bytes = w1 > w2 ? w1 : w2;
-        if (c->fft_work_bytes > 0) {
-            if ((rc = dev_alloc(c, &c->fft_work, c->fft_work_bytes)) != DH_OK) return fail(rc);
-            cufftSetWorkArea(c->plan_r2c, c->fft_work);
-            cufftSetWorkArea(c->plan_c2r, c->fft_work);
-        }
-        if (cufftSetStream(c->plan_r2c, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_c2r, c->stream) != CUFFT_SUCCESS) {
-            set_error("cufftSetStream failed"); return fail(DH_ERR_CUFFT);
-        }
+        // cuFFT plans (transforms only) are needed by the route for sides that are not a power of two; a power-of-two side
+        // makes them only when dh_tune("own_fft", 0) asks for that route (at 512^3 their work area is ~0.5 GB)
+        if (!own_fft_supported(grid_n) && (rc = ensure_cufft_plans(c)) != DH_OK) return fail(rc);
         if (own_fft_supported(grid_n)) {
             if ((rc = own_fft_init(c)) != DH_OK) return fail(rc);
             c->own_fft = true;
@@ -454,7 +465,10 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
     else if (!strcmp(key, "tape")) c->tune_tape = value;
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
-    else if (!strcmp(key, "own_fft")) c->tune_own_fft = value;
+    else if (!strcmp(key, "own_fft")) {
+        if (!value && c->opt.gravity_on) DH_TRY(ensure_cufft_plans(c));
+        c->tune_own_fft = value;
+    }
     else if (!strcmp(key, "overlap")) c->tune_overlap = value;
     else if (!strcmp(key, "prime")) c->tune_prime = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
@@ -822,12 +836,12 @@ int dh_deposit(dh_ctx* c, const float* rho_gas, float* const pos[3], float* delt
 }
 
 int dh_poisson(dh_ctx* c, const float* delta, double A, float* const g_out[3]) {
-    if (!c || !delta || !g_out || !c->plans) { set_error("dh_poisson: bad argument or gravity off"); return DH_ERR_INVALID; }
+    if (!c || !delta || !g_out || !c->opt.gravity_on) { set_error("dh_poisson: bad argument or gravity off"); return DH_ERR_INVALID; }
     return poisson_forward(c, delta, (float)A, g_out);
 }
 
 int dh_poisson_vjp(dh_ctx* c, float* const g_bar[3], double A, float* delta_bar_out) {
-    if (!c || !g_bar || !delta_bar_out || !c->plans) { set_error("dh_poisson_vjp: bad argument or gravity off"); return DH_ERR_INVALID; }
+    if (!c || !g_bar || !delta_bar_out || !c->opt.gravity_on) { set_error("dh_poisson_vjp: bad argument or gravity off"); return DH_ERR_INVALID; }
     return poisson_adjoint(c, g_bar, (float)A, delta_bar_out);
 }
 

@@ -146,7 +146,7 @@ def _smooth_direction(N, seed):
 STATIC_STABLE_L2, STATIC_STABLE_OUTLIERS = 2e-2, 1e-1      # provisional: tightened to ~3x the B200 measurement
 
 
-def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stride, got, dp, min_stable, max_sens):
+def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stride, got, dp, min_stable, max_sens, n_pert=1):
     """What a hydro-only reverse pass is held to (reading R28), given the GPU cotangent `got` of L = 1/2 sum rho_final^2:
     (a) entry by entry on the entries the fp64 oracle reproduces under one fp32 rounding of its input, (b) over all
     entries within twice what the oracle does to itself, (c) projected on smooth directions against the oracle AND
@@ -163,9 +163,15 @@ def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stri
     # 1e-16 of the background) reaches cells that are still EXACTLY uniform in fp32, where every limiter argument is 0 and
     # the gate is off by convention (R26); moving the whole input by one fp32 rounding puts the oracle's gates in those
     # cells on the other branch too
-    prng = np.random.default_rng(7)
-    rg2, _, rdp2 = oracle_grad(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)))
-    stable = PT.stable_entries(rg, [rg2], tol=1e-4)
+    # (n_pert independent copies: an entry counts as well defined only if every copy reproduces it -- one copy leaves the
+    # gates it did not happen to flip among the "stable" entries, and in the Sedov blast a few hundred such entries next to
+    # the central cell carry gradient values 1e3 times the typical one)
+    pert = []
+    for s in range(n_pert):
+        prng = np.random.default_rng(7 + s)
+        pert.append(oracle_grad(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape))))
+    rg2, _, rdp2 = pert[0]
+    stable = PT.stable_entries(rg, [q[0] for q in pert], tol=1e-4)
     e_max, e_l2 = PT.masked_errors(got, rg, stable)
     bad = np.mean(np.abs(got - rg)[stable] > 1e-3 * np.max(np.abs(rg)))
     sens, eg = PT.rel_l2(rg2, rg), PT.rel_l2(got, rg)
@@ -240,5 +246,5 @@ def test_sedov_run_vjp_is_finite_and_matches_oracle_at_64(api, torch_, O, W):
     dp = ctx.dh_run_vjp(ct, ct)
     got = ct.gas.cpu().numpy()
     assert np.all(np.isfinite(got)) and np.isfinite(dp.dgamma)
-    _static_run_gradient_checks(api, torch_, O, W, f"sedov 64^3 ({n} steps)", ctx, P, gas, dts, 6, got, dp, 0.3, 0.5)
+    _static_run_gradient_checks(api, torch_, O, W, f"sedov 64^3 ({n} steps)", ctx, P, gas, dts, 6, got, dp, 0.3, 0.5, n_pert=6)
     ctx.close()
