@@ -62,6 +62,12 @@ typedef struct {
     int32_t want_dsched;          /* 1: the sweep adjoints also accumulate the cotangents of Dtau and kappa (dparams.dDtau,
                                    * dparams.dkappa: needed for cosmological-parameter gradients); 0: they are skipped (about
                                    * 6 % of the adjoint sweeps' arithmetic) and both fields come back as NaN */
+    int32_t dual_energy;          /* 1: dual-energy formalism (readings R33-R36 of DESIGN.md): a sixth mesh field
+                                   * q = a^2 rho_b e (dh_state.eint) is advanced by the internal-energy equation whose source
+                                   * S_e = -p div U the paper prints at :101, and replaces eps - |m|^2/(2 rho) in the pressure
+                                   * and the freezing speed wherever the thermal energy is less than dual_eta of the total.
+                                   * The five conserved fields keep their equations.  0: single energy (the paper's runs) */
+    double dual_eta;              /* thermal fraction below which q is used (customary: 1e-3) */
 } dh_options;
 
 /* State of the simulation.  gas/part: caller-owned DEVICE pointers (N^3 and N_p floats each).
@@ -72,12 +78,14 @@ typedef struct {
     double a;        /* scale factor of this state (1 in static mode) */
     double dt_prev;  /* cosmic-time length of the previous step; 0 before the first step (reading R15) */
     int64_t step;    /* step counter; step mod 6 selects the Strang order (reading R9) */
+    float* eint;     /* dual_energy = 1 only: caller-owned DEVICE pointer, N^3 floats, q = a^2 rho_b e; else ignored (NULL) */
 } dh_state;
 
 /* Cotangent of a state: same 11 arrays, caller-owned DEVICE pointers. */
 typedef struct {
     float* gas[5];
     float* part[6];
+    float* eint;     /* dual_energy = 1 only: cotangent of dh_state.eint; else ignored (NULL) */
 } dh_cot;
 
 /* Gradients w.r.t. the scalars of the scheme, ACCUMULATED (+=) by the VJP calls (host struct, fp64).
@@ -134,7 +142,8 @@ int dh_reserve(dh_ctx* ctx, int n_steps, int checkpoint_stride);
 
 /* ---- host-buffer variants (end-to-end path: host <-> device copies inside the call) ------------------------- */
 
-/* gas_host: 5 N^3 floats, part_host: 6 N_p floats (HOST, pinned or pageable), updated in place with the final state.
+/* gas_host: 5 N^3 floats (6 N^3 with dual_energy: q last), part_host: 6 N_p floats (HOST, pinned or pageable), updated in
+ * place with the final state.
  * a, dt_prev, step: host scalars of the state, updated. */
 int dh_run_host(dh_ctx* ctx, float* gas_host, float* part_host, double* a, double* dt_prev, int64_t* step,
                 const double* a_sched, const double* dt_sched, int n_steps, int checkpoint_stride);
@@ -194,6 +203,11 @@ int dh_sweep(dh_ctx* ctx, int d, float* const gas_in[5], const float* g, double 
  * scal_bar: DEVICE double[3] += (lam_bar, kap_bar, gamma_bar). */
 int dh_sweep_vjp(dh_ctx* ctx, int d, float* const gas_in[5], const float* g, double lam, double kap,
                  float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar);
+/* The same two calls for a context with dual_energy = 1: six fields (rho, m_x, m_y, m_z, eps, q) in and out. */
+int dh_sweep_de(dh_ctx* ctx, int d, float* const gas_in[6], const float* g, double lam, double kap,
+                float* const gas_out[6], float* cmax_out);
+int dh_sweep_de_vjp(dh_ctx* ctx, int d, float* const gas_in[6], const float* g, double lam, double kap,
+                    float* const cot_out[6], float* const cot_in[6], float* g_bar, double* scal_bar);
 /* delta_tot = [gas_sources_gravity] rho_gas - rho_bar + m_p CIC(pos) (rho_gas may be NULL). */
 int dh_deposit(dh_ctx* ctx, const float* rho_gas, float* const pos[3], float* delta_out);
 /* g'_d (3 meshes) from delta (delta is not modified). */

@@ -30,7 +30,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
            "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
-           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors"]
+           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors", "dh_sweep_de", "dh_sweep_de_vjp"]
 
 
 class DhError(RuntimeError):
@@ -48,16 +48,17 @@ class dh_cosmology(C.Structure):
 class dh_options(C.Structure):
     _fields_ = [("n_part_side", C.c_int32), ("gravity_on", C.c_int32), ("hydro_on", C.c_int32),
                 ("gas_sources_gravity", C.c_int32), ("e_floor", C.c_double), ("lim_eps", C.c_double),
-                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32), ("want_dsched", C.c_int32)]
+                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32), ("want_dsched", C.c_int32),
+                ("dual_energy", C.c_int32), ("dual_eta", C.c_double)]
 
 
 class dh_state(C.Structure):
     _fields_ = [("gas", C.c_void_p * 5), ("part", C.c_void_p * 6), ("a", C.c_double), ("dt_prev", C.c_double),
-                ("step", C.c_int64)]
+                ("step", C.c_int64), ("eint", C.c_void_p)]
 
 
 class dh_cot(C.Structure):
-    _fields_ = [("gas", C.c_void_p * 5), ("part", C.c_void_p * 6)]
+    _fields_ = [("gas", C.c_void_p * 5), ("part", C.c_void_p * 6), ("eint", C.c_void_p)]
 
 
 class dh_subgrid_params(C.Structure):
@@ -108,6 +109,9 @@ _P6 = C.c_void_p * 6
 _lib.dh_sweep.argtypes = [C.c_void_p, C.c_int, _P5, C.c_void_p, C.c_double, C.c_double, _P5, C.c_void_p]
 _lib.dh_sweep_vjp.argtypes = [C.c_void_p, C.c_int, _P5, C.c_void_p, C.c_double, C.c_double, _P5, _P5, C.c_void_p,
                               C.c_void_p]
+_lib.dh_sweep_de.argtypes = [C.c_void_p, C.c_int, _P6, C.c_void_p, C.c_double, C.c_double, _P6, C.c_void_p]
+_lib.dh_sweep_de_vjp.argtypes = [C.c_void_p, C.c_int, _P6, C.c_void_p, C.c_double, C.c_double, _P6, _P6, C.c_void_p,
+                                 C.c_void_p]
 _lib.dh_deposit.argtypes = [C.c_void_p, C.c_void_p, _P3, C.c_void_p]
 _lib.dh_poisson.argtypes = [C.c_void_p, C.c_void_p, C.c_double, _P3]
 _lib.dh_poisson_vjp.argtypes = [C.c_void_p, _P3, C.c_double, C.c_void_p]
@@ -135,15 +139,16 @@ def _check(rc, where):
 
 
 def _ptrs(t: torch.Tensor, n: int, arr_type):
-    """Pointers to the n leading slices of a contiguous fp32 CUDA tensor of shape (n, ...)."""
-    assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.shape[0] == n, (t.shape, t.dtype)
+    """Pointers to the n leading slices of a contiguous fp32 CUDA tensor of shape (>= n, ...)."""
+    assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.shape[0] >= n, (t.shape, t.dtype)
     stride = t[0].numel() * 4
     base = t.data_ptr()
     return arr_type(*[base + i * stride for i in range(n)])
 
 
 class State:
-    """Device state: gas (5,N,N,N) and part (6,N_p) fp32 CUDA tensors (caller-owned) + host scalars."""
+    """Device state: gas (5,N,N,N) -- (6,N,N,N) with dual energy, the sixth field is q = a^2 rho e (dh_state.eint) -- and
+    part (6,N_p) fp32 CUDA tensors (caller-owned) + host scalars."""
 
     def __init__(self, gas, part, a, dt_prev=0.0, step=0, device="cuda"):
         self.gas = torch.as_tensor(np.asarray(gas, dtype=np.float32) if not torch.is_tensor(gas) else gas,
@@ -155,6 +160,8 @@ class State:
     def c_struct(self) -> dh_state:
         s = dh_state()
         s.gas = _ptrs(self.gas, 5, _P5)
+        if self.gas.shape[0] == 6:
+            s.eint = self.gas[5].data_ptr()
         if self.part.shape[1] > 0:
             s.part = _ptrs(self.part, 6, _P6)
         s.a, s.dt_prev, s.step = self.a, self.dt_prev, self.step
@@ -172,6 +179,8 @@ class Cot:
     def c_struct(self) -> dh_cot:
         s = dh_cot()
         s.gas = _ptrs(self.gas, 5, _P5)
+        if self.gas.shape[0] == 6:
+            s.eint = self.gas[5].data_ptr()
         if self.part.shape[1] > 0:
             s.part = _ptrs(self.part, 6, _P6)
         return s
@@ -182,16 +191,18 @@ class Context:
 
     def __init__(self, N, box, gamma, n_part_side=None, H0=100.0, Omega_m=1.0, Omega_b=0.16, Omega_L=0.0, static_mode=0,
                  gravity_on=1, hydro_on=1, gas_sources_gravity=1, e_floor=1e-12, lim_eps=1e-20, want_dA=1, want_dsched=1,
-                 stream: torch.cuda.Stream | None = None):
+                 dual_energy=0, dual_eta=1e-3, stream: torch.cuda.Stream | None = None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2502_02294_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
         self.N = int(N)
+        self.nc = 6 if dual_energy else 5
         self.nps = self.N if n_part_side is None else int(n_part_side)
         self.np = self.nps ** 3
         self.cosmo = dh_cosmology(H0, Omega_m, Omega_b, Omega_L, int(static_mode))
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         self.opt = dh_options(self.nps, int(gravity_on), int(hydro_on), int(gas_sources_gravity), float(e_floor),
-                              float(lim_eps), C.c_void_p(self.stream.cuda_stream), int(want_dA), int(want_dsched))
+                              float(lim_eps), C.c_void_p(self.stream.cuda_stream), int(want_dA), int(want_dsched),
+                              int(dual_energy), float(dual_eta))
         self._h = C.c_void_p()
         _check(_lib.dh_init(C.byref(self._h), self.N, float(box), float(gamma), C.byref(self.cosmo), C.byref(self.opt)),
                "dh_init")
@@ -311,6 +322,23 @@ class Context:
                                  gb.data_ptr() if gb is not None else None, sc.data_ptr()), "dh_sweep_vjp")
         return cot_in, gb, sc
 
+    def dh_sweep_de(self, d, gas_in: torch.Tensor, g: torch.Tensor | None, lam, kap, cmax: torch.Tensor | None = None):
+        """The dual-energy sweep on a (6,N,N,N) state (needs a context with dual_energy=1)."""
+        out = torch.empty_like(gas_in)
+        _check(_lib.dh_sweep_de(self._h, int(d), _ptrs(gas_in, 6, _P6), g.data_ptr() if g is not None else None,
+                                float(lam), float(kap), _ptrs(out, 6, _P6),
+                                cmax.data_ptr() if cmax is not None else None), "dh_sweep_de")
+        return out
+
+    def dh_sweep_de_vjp(self, d, gas_in, g, lam, kap, cot_out):
+        cot_in = torch.empty_like(gas_in)
+        gb = torch.zeros_like(g) if g is not None else None
+        sc = torch.zeros(3, dtype=torch.float64, device=gas_in.device)
+        _check(_lib.dh_sweep_de_vjp(self._h, int(d), _ptrs(gas_in, 6, _P6), g.data_ptr() if g is not None else None,
+                                    float(lam), float(kap), _ptrs(cot_out, 6, _P6), _ptrs(cot_in, 6, _P6),
+                                    gb.data_ptr() if gb is not None else None, sc.data_ptr()), "dh_sweep_de_vjp")
+        return cot_in, gb, sc
+
     def dh_deposit(self, rho_gas: torch.Tensor | None, pos: torch.Tensor):
         out = torch.empty((self.N,) * 3, dtype=torch.float32, device=pos.device)
         _check(_lib.dh_deposit(self._h, rho_gas.data_ptr() if rho_gas is not None else None, _ptrs(pos, 3, _P3),
@@ -335,7 +363,7 @@ class Context:
         """delta_init (N,N,N) fp32 CUDA tensor -> a new State (tensors allocated here, filled by the library)."""
         assert delta_init.is_cuda and delta_init.dtype == torch.float32 and delta_init.is_contiguous()
         n3 = self.N ** 3
-        st = State(torch.empty((5, self.N, self.N, self.N), dtype=torch.float32, device=delta_init.device),
+        st = State(torch.empty((self.nc, self.N, self.N, self.N), dtype=torch.float32, device=delta_init.device),
                    torch.empty((6, n3), dtype=torch.float32, device=delta_init.device), a0)
         cs = st.c_struct()
         _check(_lib.dh_ic_zeldovich(self._h, delta_init.data_ptr(), float(a0), float(vel_factor), float(e_tilde0),

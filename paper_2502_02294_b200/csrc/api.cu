@@ -54,6 +54,13 @@ StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, doub
     return s;
 }
 
+// The gas arrays of a state / cotangent as one list of c->nc pointers (the sixth is q with dual energy).
+struct G6 {
+    float* p[6];
+    G6(const dh_state& s) { for (int k = 0; k < 5; ++k) p[k] = s.gas[k]; p[5] = s.eint; }
+    G6(const dh_cot& s) { for (int k = 0; k < 5; ++k) p[k] = s.gas[k]; p[5] = s.eint; }
+};
+
 static int alloc_fields(dh_ctx* c, float** arr, int n, size_t count) {
     for (int i = 0; i < n; ++i) DH_TRY(dev_alloc(c, (void**)&arr[i], count * sizeof(float)));
     return DH_OK;
@@ -62,24 +69,25 @@ static int alloc_fields(dh_ctx* c, float** arr, int n, size_t count) {
 static int ensure_adjoint_scratch(dh_ctx* c) {
     if (c->adj_alloc) return DH_OK;
     if (c->opt.hydro_on) {
-        DH_TRY(alloc_fields(c, c->sw_in[0], 5, c->n3));
-        DH_TRY(alloc_fields(c, c->sw_in[1], 5, c->n3));
-        DH_TRY(alloc_fields(c, c->cot_tmp, 5, c->n3));
+        DH_TRY(alloc_fields(c, c->sw_in[0], c->nc, c->n3));
+        DH_TRY(alloc_fields(c, c->sw_in[1], c->nc, c->n3));
+        DH_TRY(alloc_fields(c, c->cot_tmp, c->nc, c->n3));
     }
     if (c->opt.gravity_on) DH_TRY(alloc_fields(c, c->gpb, 3, c->n3));
     c->adj_alloc = true;
     return DH_OK;
 }
 
-static size_t state_floats(const dh_ctx* c) { return (size_t)(5 * c->n3 + 6 * c->np); }
+static size_t state_floats(const dh_ctx* c) { return (size_t)(c->nc * c->n3 + 6 * c->np); }
 
 static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st) {
     if (!s.buf) DH_TRY(dev_alloc(c, (void**)&s.buf, state_floats(c) * sizeof(float)));
     Prof prof(c, PROF_COPY);
-    for (int k = 0; k < 5; ++k)
-        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)k * c->n3, st->gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    const G6 g(*st);
+    for (int k = 0; k < c->nc; ++k)
+        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)k * c->n3, g.p[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     for (int k = 0; k < 6 && c->np > 0; ++k)
-        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)5 * c->n3 + (size_t)k * c->np, st->part[k], c->np * sizeof(float),
+        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)c->nc * c->n3 + (size_t)k * c->np, st->part[k], c->np * sizeof(float),
                                 cudaMemcpyDeviceToDevice, c->stream));
     s.a = st->a; s.dt_prev = st->dt_prev; s.step = st->step;
     return DH_OK;
@@ -87,14 +95,15 @@ static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st) {
 
 static void snapshot_view(const dh_ctx* c, const Snapshot& s, dh_state* st) {
     for (int k = 0; k < 5; ++k) st->gas[k] = s.buf + (size_t)k * c->n3;
-    for (int k = 0; k < 6; ++k) st->part[k] = s.buf + (size_t)5 * c->n3 + (size_t)k * c->np;
+    st->eint = c->nc == 6 ? s.buf + (size_t)5 * c->n3 : nullptr;
+    for (int k = 0; k < 6; ++k) st->part[k] = s.buf + (size_t)c->nc * c->n3 + (size_t)k * c->np;
     st->a = s.a; st->dt_prev = s.dt_prev; st->step = s.step;
 }
 
 static void tape_view(const dh_ctx* c, StepTape& t) {
     for (int d = 0; d < 3; ++d) t.gp[d] = t.buf + (size_t)d * c->n3;
     for (int i = 0; i < 2; ++i)
-        for (int k = 0; k < 5; ++k) t.sw[i][k] = t.buf + (size_t)(3 + 5 * i + k) * c->n3;
+        for (int k = 0; k < c->nc; ++k) t.sw[i][k] = t.buf + (size_t)(3 + c->nc * i + k) * c->n3;
 }
 
 // Tapes for the steps of one segment.  All or nothing: if the device cannot hold them the reverse pass falls back to
@@ -102,7 +111,7 @@ static void tape_view(const dh_ctx* c, StepTape& t) {
 static bool ensure_tapes(dh_ctx* c, int in_seg) {
     if (!c->tune_tape) return false;
     if ((int)c->tapes.size() < in_seg) c->tapes.resize(in_seg);
-    const size_t bytes = (size_t)13 * c->n3 * sizeof(float);
+    const size_t bytes = (size_t)(3 + 2 * c->nc) * c->n3 * sizeof(float);
     for (int i = 0; i < in_seg; ++i) {
         if (c->tapes[i].buf) continue;
         if (dev_alloc(c, (void**)&c->tapes[i].buf, bytes) != DH_OK) {
@@ -142,7 +151,7 @@ static void free_snaps(dh_ctx* c, std::vector<Snapshot>& v) {
 }
 
 // S1 + S2: delta_tot and g' from the state's gas density and particle positions.
-static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6], float A, float* const gp[3],
+static int compute_gravity(dh_ctx* c, float* const* gas, float* const part[6], float A, float* const gp[3],
                            bool delta_primed = false) {
     DH_TRY(launch_deposit(c, gas[0], part[0], part[1], part[2], c->delta, delta_primed));
     DH_TRY(poisson_forward(c, c->delta, A, gp));
@@ -155,7 +164,7 @@ static int compute_gravity(dh_ctx* c, float* const gas[5], float* const part[6],
 // scratch.  gp_keep: where g' of this step goes (the run's per-step g' store); gp_ready: it already holds g' of this
 // step, so deposit and Poisson solve are skipped.  part_out == nullptr skips the particle update, last_sweep == false stops after sweep 2 (the reverse pass
 // needs nothing more of a segment's last step).
-static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], float* const gas_out[5],
+static int step_arrays(dh_ctx* c, float* const* gas, float* const part[6], float* const* gas_out,
                        float* const part_out[6], const StepScalars& s, int64_t step, float* cmax3, StepTape* tape,
                        bool last_sweep, float* const* gp_keep = nullptr, bool gp_ready = false,
                        bool delta_primed = false, bool prime_next = false) {
@@ -183,12 +192,13 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
         const float lam = (float)(s.dtau / c->dx), kap = (float)s.kappa;
-        float* cur[5]; float* nxt[5];
-        for (int k = 0; k < 5; ++k) cur[k] = gas[k];
+        const int nc = c->nc;
+        float* cur[6]; float* nxt[6];
+        for (int k = 0; k < nc; ++k) cur[k] = gas[k];
         for (int sidx = 0; sidx < 3; ++sidx) {
             if (sidx == 2 && !last_sweep) break;
             const int d = order[sidx];
-            for (int k = 0; k < 5; ++k)
+            for (int k = 0; k < nc; ++k)
                 nxt[k] = sidx == 2 ? gas_out[k] : (tape ? tape->sw[sidx][k] : (sidx == 0 ? c->gas_tmp[k] : c->gas_tmp2[k]));
             const int rc = launch_sweep(c, d, cur, grav ? gp[d] : nullptr, lam, kap, nxt, cmax3 ? cmax3 + sidx : nullptr,
                                         (sidx == 2 && prime_next) ? c->delta : nullptr);
@@ -196,11 +206,11 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
                 if (beside) cudaStreamWaitEvent(c->stream, c->ev_join, 0);
                 return rc;
             }
-            for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
+            for (int k = 0; k < nc; ++k) cur[k] = nxt[k];
         }
         if (beside) DH_CUDA(cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     } else if (gas_out[0] != gas[0]) {
-        for (int k = 0; k < 5; ++k)
+        for (int k = 0; k < c->nc; ++k)
             DH_CUDA(cudaMemcpyAsync(gas_out[k], gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     }
     return DH_OK;
@@ -208,8 +218,8 @@ static int step_arrays(dh_ctx* c, float* const gas[5], float* const part[6], flo
 
 // The step VJP.  tape == nullptr: g' and the inputs of sweeps 2 and 3 are recomputed from the step's input state
 // into the context's scratch first; otherwise they are taken from the tape the reverse pass recorded.
-static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_in[6], const StepScalars& s, int64_t step,
-                           float* const cot_gas_out[5], float* const cot_part_out[6], float* const cot_gas_in[5],
+static int step_vjp_arrays(dh_ctx* c, float* const* gas_in, float* const part_in[6], const StepScalars& s, int64_t step,
+                           float* const* cot_gas_out, float* const cot_part_out[6], float* const* cot_gas_in,
                            float* const cot_part_in[6], StepTape* tape, float* const* gp_kept = nullptr) {
     DH_TRY(ensure_adjoint_scratch(c));
     const bool grav = c->opt.gravity_on != 0;
@@ -217,7 +227,7 @@ static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_
     StepTape local;
     if (!tape) {
         for (int d = 0; d < 3; ++d) local.gp[d] = c->gp[d];
-        for (int i = 0; i < 2; ++i) for (int k = 0; k < 5; ++k) local.sw[i][k] = c->sw_in[i][k];
+        for (int i = 0; i < 2; ++i) for (int k = 0; k < c->nc; ++k) local.sw[i][k] = c->sw_in[i][k];
         DH_TRY(step_arrays(c, gas_in, part_in, gas_in, nullptr, s, step, nullptr, &local, false, gp_kept, gp_kept != nullptr));
         tape = &local;
     }
@@ -225,21 +235,22 @@ static int step_vjp_arrays(dh_ctx* c, float* const gas_in[5], float* const part_
     // ---- S4 reversed
     if (c->opt.hydro_on) {
         const int* order = STRANG[((step % 6) + 6) % 6];
-        float* cur[5]; float* nxt[5];
-        for (int k = 0; k < 5; ++k) cur[k] = cot_gas_out[k];
+        const int nc = c->nc;
+        float* cur[6]; float* nxt[6];
+        for (int k = 0; k < nc; ++k) cur[k] = cot_gas_out[k];
         for (int sidx = 2; sidx >= 0; --sidx) {
             const int d = order[sidx];
             float* const* src = (sidx == 0) ? gas_in : tape->sw[sidx - 1];
             // the last adjoint sweep writes the caller's cot_gas_in; the others alternate between the two scratch sets
-            if (sidx == 0) for (int k = 0; k < 5; ++k) nxt[k] = cot_gas_in[k];
-            else if (sidx == 2) for (int k = 0; k < 5; ++k) nxt[k] = c->cot_tmp[k];
-            else for (int k = 0; k < 5; ++k) nxt[k] = c->gas_tmp[k];
+            if (sidx == 0) for (int k = 0; k < nc; ++k) nxt[k] = cot_gas_in[k];
+            else if (sidx == 2) for (int k = 0; k < nc; ++k) nxt[k] = c->cot_tmp[k];
+            else for (int k = 0; k < nc; ++k) nxt[k] = c->gas_tmp[k];
             DH_TRY(launch_sweep_vjp(c, d, src, grav ? gp[d] : nullptr, lam, kap, cur, nxt, grav ? c->gpb[d] : nullptr,
                                     c->scal_dev));
-            for (int k = 0; k < 5; ++k) cur[k] = nxt[k];
+            for (int k = 0; k < nc; ++k) cur[k] = nxt[k];
         }
     } else {
-        for (int k = 0; k < 5; ++k)
+        for (int k = 0; k < c->nc; ++k)
             if (cot_gas_in[k] != cot_gas_out[k])
                 DH_CUDA(cudaMemcpyAsync(cot_gas_in[k], cot_gas_out[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
         if (grav) for (int d = 0; d < 3; ++d) DH_TRY(launch_fill(c, c->gpb[d], c->n3, 0.f));
@@ -308,8 +319,9 @@ static int ensure_cufft_plans(dh_ctx* c) {
     return DH_OK;
 }
 
-static int check_state(const dh_ctx* c, const float* const gas[5], const float* const part[6]) {
+static int check_state(const dh_ctx* c, const float* const gas[5], const float* const part[6], const float* eint) {
     for (int k = 0; k < 5; ++k) if (!gas[k]) { set_error("null gas pointer %d", k); return DH_ERR_INVALID; }
+    if (c->nc == 6 && !eint) { set_error("dual_energy = 1 needs the eint pointer of the state / cotangent"); return DH_ERR_INVALID; }
     if (c->np > 0) for (int k = 0; k < 6; ++k) if (!part[k]) { set_error("null particle pointer %d", k); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -327,6 +339,10 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
     *out = nullptr;
     if (grid_n < 32 || grid_n > 1024 || grid_n % 32 != 0) {
         set_error("dh_init: grid_n must be a multiple of 32 in [32, 1024], got %d", grid_n);
+        return DH_ERR_INVALID;
+    }
+    if (opt->dual_energy && !(opt->dual_eta >= 0.0)) {
+        set_error("dh_init: dual_energy needs dual_eta >= 0 (customary 1e-3)");
         return DH_ERR_INVALID;
     }
     if (!(box > 0) || !(gamma > 1.0) || !(opt->e_floor > 0) || opt->n_part_side < 0) {
@@ -355,6 +371,7 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
     c->np = (int64_t)c->nps * c->nps * c->nps;
     c->box = box; c->gamma = gamma; c->dx = box / grid_n;
     c->cosmo = *cosmo; c->opt = *opt;
+    c->nc = opt->dual_energy ? 6 : 5;
     c->f_b = cosmo->Omega_m > 0 ? cosmo->Omega_b / cosmo->Omega_m : 0.0;
     c->m_p = c->np > 0 ? (1.0 - c->f_b) * (double)c->n3 / (double)c->np : 0.0;
     c->rho_bar = (c->np > 0 ? 1.0 - c->f_b : 0.0) + (opt->gas_sources_gravity ? c->f_b : 0.0);
@@ -378,8 +395,8 @@ int dh_init(dh_ctx** out, int grid_n, double box, double gamma, const dh_cosmolo
             c->own_fft = true;
         }
     }
-    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp, 5, c->n3)) != DH_OK) return fail(rc);
-    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp2, 5, c->n3)) != DH_OK) return fail(rc);
+    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp, c->nc, c->n3)) != DH_OK) return fail(rc);
+    if (opt->hydro_on && (rc = alloc_fields(c, c->gas_tmp2, c->nc, c->n3)) != DH_OK) return fail(rc);
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
@@ -471,6 +488,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     }
     else if (!strcmp(key, "overlap")) c->tune_overlap = value;
     else if (!strcmp(key, "prime")) c->tune_prime = value;
+    else if (!strcmp(key, "run_gather")) c->tune_run_gather = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -514,11 +532,12 @@ int dh_schedule_lna(const dh_cosmology* co, double a0, double a1, int n, double*
 
 int dh_step(dh_ctx* c, dh_state* st, double dt, double a, float* cfl_cmax_out) {
     if (!c || !st) { set_error("dh_step: null argument"); return DH_ERR_INVALID; }
-    DH_TRY(check_state(c, st->gas, st->part));
+    DH_TRY(check_state(c, st->gas, st->part, st->eint));
     const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
     float* cm = cfl_cmax_out ? cfl_cmax_out : c->cmax_step;
     DH_CUDA(cudaMemsetAsync(cm, 0, 3 * sizeof(float), c->stream));
-    DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, cm, nullptr, true));
+    const G6 g(*st);
+    DH_TRY(step_arrays(c, g.p, st->part, g.p, st->part, s, st->step, cm, nullptr, true));
     st->a = c->cosmo.static_mode ? 1.0 : a;
     st->dt_prev = dt;
     st->step += 1;
@@ -527,18 +546,18 @@ int dh_step(dh_ctx* c, dh_state* st, double dt, double a, float* cfl_cmax_out) {
 
 int dh_step_vjp(dh_ctx* c, const dh_state* st, double dt, double a, const dh_cot* cot_out, dh_cot* cot_in, dh_dparams* dp) {
     if (!c || !st || !cot_out || !cot_in) { set_error("dh_step_vjp: null argument"); return DH_ERR_INVALID; }
-    DH_TRY(check_state(c, st->gas, st->part));
-    DH_TRY(check_state(c, cot_out->gas, cot_out->part));
-    DH_TRY(check_state(c, cot_in->gas, cot_in->part));
+    DH_TRY(check_state(c, st->gas, st->part, st->eint));
+    DH_TRY(check_state(c, cot_out->gas, cot_out->part, cot_out->eint));
+    DH_TRY(check_state(c, cot_in->gas, cot_in->part, cot_in->eint));
     const StepScalars s = step_scalars(c->cosmo, st->a, a, dt, st->dt_prev);
-    DH_TRY(step_vjp_arrays(c, st->gas, st->part, s, st->step, cot_out->gas, cot_out->part, cot_in->gas, cot_in->part,
-                           nullptr));
+    const G6 g(*st), co(*cot_out), ci(*cot_in);
+    DH_TRY(step_vjp_arrays(c, g.p, st->part, s, st->step, co.p, cot_out->part, ci.p, cot_in->part, nullptr));
     return harvest_scalars(c, dp);
 }
 
 int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sched, int n_steps, int stride) {
     if (!c || !st || !a_sched || !dt_sched || n_steps < 0) { set_error("dh_run: bad argument"); return DH_ERR_INVALID; }
-    DH_TRY(check_state(c, st->gas, st->part));
+    DH_TRY(check_state(c, st->gas, st->part, st->eint));
     if (n_steps > c->cmax_cap) {
         dev_free(c, c->cmax_log, (size_t)3 * c->cmax_cap * sizeof(float));
         c->cmax_log = nullptr; c->cmax_cap = 0;
@@ -557,8 +576,9 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     for (int k = 0; k < n_steps; ++k) {
         if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
-        const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && !c->tune_yz_chain && c->tune_prime;
-        DH_TRY(step_arrays(c, st->gas, st->part, st->gas, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
+        const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && !c->tune_yz_chain && c->tune_prime && c->nc == 5;
+        const G6 g(*st);
+        DH_TRY(step_arrays(c, g.p, st->part, g.p, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
                            c->run_gstore ? c->gstore[k].gp : nullptr, false, can_prime && k > 0,
                            can_prime && k + 1 < n_steps));
         st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
@@ -616,14 +636,15 @@ int dh_get_cmax(dh_ctx* c, float* out, int n) {
 int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dparams* dp) {
     if (!c || !cot_final || !cot_initial) { set_error("dh_run_vjp: null argument"); return DH_ERR_INVALID; }
     if (!c->run_valid) { set_error("dh_run_vjp: no checkpointed dh_run to differentiate"); return DH_ERR_STATE; }
-    DH_TRY(check_state(c, cot_final->gas, cot_final->part));
-    DH_TRY(check_state(c, cot_initial->gas, cot_initial->part));
+    DH_TRY(check_state(c, cot_final->gas, cot_final->part, cot_final->eint));
+    DH_TRY(check_state(c, cot_initial->gas, cot_initial->part, cot_initial->eint));
     const int n = c->run_n, stride = c->run_stride;
     const int nseg = (n + stride - 1) / stride;
     // cot_initial doubles as the running cotangent
-    for (int k = 0; k < 5; ++k)
-        if (cot_initial->gas[k] != cot_final->gas[k])
-            DH_CUDA(cudaMemcpyAsync(cot_initial->gas[k], cot_final->gas[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    const G6 cf(*cot_final), cini(*cot_initial);
+    for (int k = 0; k < c->nc; ++k)
+        if (cini.p[k] != cf.p[k])
+            DH_CUDA(cudaMemcpyAsync(cini.p[k], cf.p[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     for (int k = 0; k < 6 && c->np > 0; ++k)
         if (cot_initial->part[k] != cot_final->part[k])
             DH_CUDA(cudaMemcpyAsync(cot_initial->part[k], cot_final->part[k], c->np * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
@@ -652,14 +673,16 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
             StepTape* tape = taped ? &c->tapes[k - k0] : nullptr;
             float* const* gk = c->run_gstore ? c->gstore[k].gp : nullptr;
+            const G6 gin(in);
             if (last) {
-                DH_TRY(step_arrays(c, in.gas, in.part, in.gas, nullptr, s, in.step, nullptr, tape, false, gk, gk != nullptr));
+                DH_TRY(step_arrays(c, gin.p, in.part, gin.p, nullptr, s, in.step, nullptr, tape, false, gk, gk != nullptr));
             } else {
                 Snapshot& nx = c->seg[k - k0 + 1];
                 if (!nx.buf) DH_TRY(dev_alloc(c, (void**)&nx.buf, state_floats(c) * sizeof(float)));
                 dh_state out;
                 snapshot_view(c, nx, &out);
-                DH_TRY(step_arrays(c, in.gas, in.part, out.gas, out.part, s, in.step, nullptr, tape, true, gk, gk != nullptr));
+                const G6 gout(out);
+                DH_TRY(step_arrays(c, gin.p, in.part, gout.p, out.part, s, in.step, nullptr, tape, true, gk, gk != nullptr));
                 nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
                 nx.dt_prev = c->run_dt[k];
                 nx.step = in.step + 1;
@@ -670,7 +693,8 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             dh_state in;
             snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
-            DH_TRY(step_vjp_arrays(c, in.gas, in.part, s, in.step, cot_initial->gas, cot_initial->part, cot_initial->gas,
+            const G6 gin(in);
+            DH_TRY(step_vjp_arrays(c, gin.p, in.part, s, in.step, cini.p, cot_initial->part, cini.p,
                                    cot_initial->part, taped ? &c->tapes[k - k0] : nullptr,
                                    c->run_gstore ? c->gstore[k].gp : nullptr));
             if (per_step) {
@@ -746,12 +770,13 @@ int dh_run_host(dh_ctx* c, float* gas_host, float* part_host, double* a, double*
     DH_TRY(hv_ensure(c, &c->hv_state));
     dh_state st;
     for (int k = 0; k < 5; ++k) st.gas[k] = c->hv_state + (size_t)k * c->n3;
-    for (int k = 0; k < 6; ++k) st.part[k] = c->hv_state + (size_t)5 * c->n3 + (size_t)k * c->np;
+    st.eint = c->nc == 6 ? c->hv_state + (size_t)5 * c->n3 : nullptr;
+    for (int k = 0; k < 6; ++k) st.part[k] = c->hv_state + (size_t)c->nc * c->n3 + (size_t)k * c->np;
     st.a = *a; st.dt_prev = *dt_prev; st.step = *step;
-    DH_CUDA(cudaMemcpyAsync(st.gas[0], gas_host, (size_t)5 * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    DH_CUDA(cudaMemcpyAsync(st.gas[0], gas_host, (size_t)c->nc * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     if (c->np > 0) DH_CUDA(cudaMemcpyAsync(st.part[0], part_host, (size_t)6 * c->np * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     DH_TRY(dh_run(c, &st, a_sched, dt_sched, n_steps, stride));
-    DH_CUDA(cudaMemcpyAsync(gas_host, st.gas[0], (size_t)5 * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaMemcpyAsync(gas_host, st.gas[0], (size_t)c->nc * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (c->np > 0) DH_CUDA(cudaMemcpyAsync(part_host, st.part[0], (size_t)6 * c->np * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(cudaStreamSynchronize(c->stream));
     *a = st.a; *dt_prev = st.dt_prev; *step = st.step;
@@ -763,11 +788,12 @@ int dh_run_vjp_host(dh_ctx* c, float* cot_gas_host, float* cot_part_host, dh_dpa
     DH_TRY(hv_ensure(c, &c->hv_cot));
     dh_cot ct;
     for (int k = 0; k < 5; ++k) ct.gas[k] = c->hv_cot + (size_t)k * c->n3;
-    for (int k = 0; k < 6; ++k) ct.part[k] = c->hv_cot + (size_t)5 * c->n3 + (size_t)k * c->np;
-    DH_CUDA(cudaMemcpyAsync(ct.gas[0], cot_gas_host, (size_t)5 * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    ct.eint = c->nc == 6 ? c->hv_cot + (size_t)5 * c->n3 : nullptr;
+    for (int k = 0; k < 6; ++k) ct.part[k] = c->hv_cot + (size_t)c->nc * c->n3 + (size_t)k * c->np;
+    DH_CUDA(cudaMemcpyAsync(ct.gas[0], cot_gas_host, (size_t)c->nc * c->n3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     if (c->np > 0) DH_CUDA(cudaMemcpyAsync(ct.part[0], cot_part_host, (size_t)6 * c->np * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     DH_TRY(dh_run_vjp(c, &ct, &ct, dp));
-    DH_CUDA(cudaMemcpyAsync(cot_gas_host, ct.gas[0], (size_t)5 * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(cudaMemcpyAsync(cot_gas_host, ct.gas[0], (size_t)c->nc * c->n3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (c->np > 0) DH_CUDA(cudaMemcpyAsync(cot_part_host, ct.part[0], (size_t)6 * c->np * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(cudaStreamSynchronize(c->stream));
     return DH_OK;
@@ -795,13 +821,16 @@ int dh_value_and_grad_host(dh_ctx* c, const float* delta_init_host, const float*
     dh_state st;
     dh_cot ct;
     for (int k = 0; k < 5; ++k) { st.gas[k] = c->hv_state + (size_t)k * c->n3; ct.gas[k] = c->hv_cot + (size_t)k * c->n3; }
+    st.eint = c->nc == 6 ? c->hv_state + (size_t)5 * c->n3 : nullptr;
+    ct.eint = c->nc == 6 ? c->hv_cot + (size_t)5 * c->n3 : nullptr;
     for (int k = 0; k < 6; ++k) {
-        st.part[k] = c->hv_state + (size_t)5 * c->n3 + (size_t)k * c->np;
-        ct.part[k] = c->hv_cot + (size_t)5 * c->n3 + (size_t)k * c->np;
+        st.part[k] = c->hv_state + (size_t)c->nc * c->n3 + (size_t)k * c->np;
+        ct.part[k] = c->hv_cot + (size_t)c->nc * c->n3 + (size_t)k * c->np;
     }
     DH_TRY(dh_ic_zeldovich(c, delta_d, a0, vel_factor, e_tilde0, &st));
     DH_TRY(dh_run(c, &st, a_sched, dt_sched, n_steps, stride));
     DH_CUDA(cudaMemsetAsync(ct.part[0], 0, (size_t)6 * c->np * sizeof(float), c->stream));   // the loss does not see particles
+    if (ct.eint) DH_CUDA(cudaMemsetAsync(ct.eint, 0, (size_t)c->n3 * sizeof(float), c->stream));   // nor q
     DH_TRY(dh_data_term(c, observable, st.gas, data_d, noise_d, scale, weight, ct.gas, loss_out));
     DH_TRY(dh_run_vjp(c, &ct, &ct, dp));
     DH_TRY(dh_ic_zeldovich_vjp(c, delta_d, vel_factor, e_tilde0, &ct, data_d));
@@ -819,7 +848,24 @@ int dh_debug_cell_index(dh_ctx* c, const float* x_dev, int64_t n, int32_t* i0_de
 int dh_sweep(dh_ctx* c, int d, float* const gas_in[5], const float* g, double lam, double kap, float* const gas_out[5],
              float* cmax_out) {
     if (!c || d < 0 || d > 2 || !gas_in || !gas_out) { set_error("dh_sweep: bad argument"); return DH_ERR_INVALID; }
+    if (c->nc != 5) { set_error("dh_sweep: this context has dual_energy = 1, call dh_sweep_de"); return DH_ERR_INVALID; }
     return launch_sweep(c, d, gas_in, g, (float)lam, (float)kap, gas_out, cmax_out);
+}
+
+int dh_sweep_de(dh_ctx* c, int d, float* const gas_in[6], const float* g, double lam, double kap, float* const gas_out[6],
+                float* cmax_out) {
+    if (!c || d < 0 || d > 2 || !gas_in || !gas_out) { set_error("dh_sweep_de: bad argument"); return DH_ERR_INVALID; }
+    if (c->nc != 6) { set_error("dh_sweep_de: needs a context with dual_energy = 1"); return DH_ERR_INVALID; }
+    return launch_sweep(c, d, gas_in, g, (float)lam, (float)kap, gas_out, cmax_out);
+}
+
+int dh_sweep_de_vjp(dh_ctx* c, int d, float* const gas_in[6], const float* g, double lam, double kap,
+                    float* const cot_out[6], float* const cot_in[6], float* g_bar, double* scal_bar) {
+    if (!c || d < 0 || d > 2 || !gas_in || !cot_out || !cot_in || !scal_bar || (g && !g_bar)) {
+        set_error("dh_sweep_de_vjp: bad argument"); return DH_ERR_INVALID;
+    }
+    if (c->nc != 6) { set_error("dh_sweep_de_vjp: needs a context with dual_energy = 1"); return DH_ERR_INVALID; }
+    return launch_sweep_vjp(c, d, gas_in, g, (float)lam, (float)kap, cot_out, cot_in, g_bar, scal_bar);
 }
 
 int dh_sweep_vjp(dh_ctx* c, int d, float* const gas_in[5], const float* g, double lam, double kap,
@@ -827,6 +873,7 @@ int dh_sweep_vjp(dh_ctx* c, int d, float* const gas_in[5], const float* g, doubl
     if (!c || d < 0 || d > 2 || !gas_in || !cot_out || !cot_in || !scal_bar || (g && !g_bar)) {
         set_error("dh_sweep_vjp: bad argument"); return DH_ERR_INVALID;
     }
+    if (c->nc != 5) { set_error("dh_sweep_vjp: this context has dual_energy = 1, call dh_sweep_de_vjp"); return DH_ERR_INVALID; }
     return launch_sweep_vjp(c, d, gas_in, g, (float)lam, (float)kap, cot_out, cot_in, g_bar, scal_bar);
 }
 
@@ -892,9 +939,13 @@ static int check_ic(const dh_ctx* c, const float* delta_init, const char* who) {
 int dh_ic_zeldovich(dh_ctx* c, const float* delta_init, double a0, double vel_factor, double e_tilde0, dh_state* out) {
     DH_TRY(check_ic(c, delta_init, "dh_ic_zeldovich"));
     if (!out) { set_error("dh_ic_zeldovich: null state"); return DH_ERR_INVALID; }
-    DH_TRY(check_state(c, out->gas, out->part));
+    DH_TRY(check_state(c, out->gas, out->part, out->eint));
     DH_TRY(poisson_forward(c, delta_init, 1.f, c->gp));                    // psi = grad^-1 of -delta: the A = 1 solve
     DH_TRY(launch_ic_state(c, delta_init, c->gp, out->gas, out->part, (float)vel_factor, (float)e_tilde0));
+    if (c->nc == 6) {                                                      // q = rho e~_0 (reading R33)
+        DH_TRY(launch_fill(c, out->eint, c->n3, 0.f));
+        DH_TRY(launch_axpy(c, out->gas[0], out->eint, (float)e_tilde0));
+    }
     out->a = a0; out->dt_prev = 0.0; out->step = 0;
     return DH_OK;
 }
@@ -906,7 +957,13 @@ int dh_ic_zeldovich_vjp(dh_ctx* c, const float* delta_init, double vel_factor, d
     for (int k = 0; k < 5; ++k) if (!cot_state->gas[k]) { set_error("dh_ic_zeldovich_vjp: null gas cotangent %d", k); return DH_ERR_INVALID; }
     DH_TRY(ensure_adjoint_scratch(c));
     DH_TRY(poisson_forward(c, delta_init, 1.f, c->gp));
-    DH_TRY(launch_ic_state_vjp(c, delta_init, c->gp, cot_state->gas, cot_state->part, grad_delta, c->gpb,
+    const float* cg[5] = {cot_state->gas[0], cot_state->gas[1], cot_state->gas[2], cot_state->gas[3], cot_state->gas[4]};
+    if (c->nc == 6 && cot_state->eint) {                                   // q = rho e~_0: rho_b += e~_0 q_b, in scratch
+        DH_CUDA(cudaMemcpyAsync(c->delta, cot_state->gas[0], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+        DH_TRY(launch_axpy(c, cot_state->eint, c->delta, (float)e_tilde0));
+        cg[0] = c->delta;                                                  // consumed before the Poisson adjoint reuses it
+    }
+    DH_TRY(launch_ic_state_vjp(c, delta_init, c->gp, cg, cot_state->part, grad_delta, c->gpb,
                                (float)vel_factor, (float)e_tilde0));
     DH_TRY(poisson_adjoint(c, c->gpb, 1.f, c->delta));
     DH_TRY(launch_axpy(c, c->delta, grad_delta, 1.f));

@@ -59,9 +59,9 @@ struct Snapshot {
 // What the VJP of one step needs besides the step's input state: g' of the start-of-step state and the inputs of
 // sweeps 2 and 3.  Kept per step of a segment by the reverse pass when memory allows (13 N^3 floats), else recomputed.
 struct StepTape {
-    float* buf = nullptr;   // 13 N^3 floats: g'_x, g'_y, g'_z, sweep-2 input (5), sweep-3 input (5)
+    float* buf = nullptr;   // (3 + 2 nc) N^3 floats: g'_x, g'_y, g'_z, sweep-2 input (nc), sweep-3 input (nc)
     float* gp[3] = {nullptr, nullptr, nullptr};
-    float* sw[2][5] = {};
+    float* sw[2][6] = {};
 };
 
 // g' of one step of a checkpointed run, kept from the forward pass for the reverse pass.
@@ -74,6 +74,7 @@ struct GravStore {
 
 struct dh_ctx {
     int N = 0;
+    int nc = 5;                    // gas fields per cell: 5, or 6 with dh_options.dual_energy (the sixth is q = a^2 rho e)
     int64_t n3 = 0, np = 0;
     int nps = 0;
     double box = 0, gamma = 0, dx = 0;
@@ -95,6 +96,7 @@ struct dh_ctx {
     int tune_prime = 1;                               // 0: every step of dh_run initialises its Poisson source itself
     int tune_overlap = 1;                             // 0: kick_drift on the main stream, after which the sweeps start
     int tune_yz_chain = 0;                            // 1: y/z sweeps through the chain kernels of sweep.cu
+    int tune_run_gather = 0;                          // 1: particle gathers take the upper-x cloud values from the next lane
 
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans = false;
@@ -108,8 +110,8 @@ struct dh_ctx {
     float* delta = nullptr;        // N^3 real (Poisson source / delta_bar)
     float2* spec[4] = {nullptr, nullptr, nullptr, nullptr};   // half spectra: [0] delta^, [1..3] g^_d
     float* gp[3] = {nullptr, nullptr, nullptr};               // g'_d
-    float* gas_tmp[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // output of sweep 1
-    float* gas_tmp2[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // output of sweep 2 (sweep 3 writes the state)
+    float* gas_tmp[6] = {};        // output of sweep 1
+    float* gas_tmp2[6] = {};       // output of sweep 2 (sweep 3 writes the state)
     float* cmax_step = nullptr;    // 3 floats (device) for dh_step when the caller passes NULL
     float* cmax_log = nullptr;     // 3 * cmax_cap floats
     int cmax_cap = 0;
@@ -123,9 +125,9 @@ struct dh_ctx {
     double* scal_dev = nullptr;    // 8 doubles: (lam_b, kap_b, gamma_b, K_b, dtau_drift_b, A_b, spare, spare)
 
     // adjoint scratch (allocated on first use)
-    float* sw_in[2][5] = {};       // inputs of sweeps 2 and 3
+    float* sw_in[2][6] = {};       // inputs of sweeps 2 and 3
     float* gpb[3] = {nullptr, nullptr, nullptr};   // cotangent of g'
-    float* cot_tmp[5] = {};        // cotangent ping-pong
+    float* cot_tmp[6] = {};        // cotangent ping-pong
     float* part_tmp[6] = {};       // particle scratch for the recompute
     bool adj_alloc = false;
 
@@ -183,10 +185,11 @@ StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, doub
 
 // ---- kernels (sweep.cu) ----
 // delta_out (may be NULL; not with tune_yz_chain): also write delta = [gas] rho' - rho_bar, the next step's Poisson source
-int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
+// (with dh_options.dual_energy the arrays hold six pointers and the calls go to the kernels of sweep_de.cu)
+int launch_sweep(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap, float* const* out,
                  float* cmax, float* delta_out = nullptr);
-int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap,
-                     float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar);
+int launch_sweep_vjp(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap,
+                     float* const* cot_out, float* const* cot_in, float* g_bar, double* scal_bar);
 // ---- kernels (pm.cu) ----
 // primed: delta already holds [gas] rho_gas - rho_bar (written by the previous step's last sweep): deposit only
 int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float* y, const float* z, float* delta,

@@ -176,6 +176,31 @@ __device__ __forceinline__ void gather_issue(const float* __restrict__ m, const 
 #pragma unroll
     for (int j = 0; j < 4; ++j) { v.lo[j] = __ldg(m + q.lo[j]); v.hi[j] = __ldg(m + q.hi[j]); }
 }
+// The same batch with half the full-width requests: lane l's upper-x cell is lane l+1's lower-x cell whenever the two
+// particles sit in the same pair of rows one cell apart (`pass`, the run test of deposit_kernel), so the upper-x value
+// comes from the neighbour's register by shuffle and only the lanes that break the run load it themselves.  All lanes of
+// the warp must call this (the shuffles are warp-wide); dead lanes pass live = false.
+__device__ __forceinline__ bool gather_run(const Cic8& q, bool live) {
+    const int lane = threadIdx.x & 31;
+    const int row = live ? q.row : -7;
+    const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
+    const int i0x_next = __shfl_down_sync(0xffffffffu, q.i0x, 1);
+    return live && lane < 31 && row_next == row && i0x_next == q.i1x;
+}
+__device__ __forceinline__ void gather_issue_run(const float* __restrict__ m, const Cic8& q, bool live, bool pass, Gath8& v) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        v.lo[j] = live ? __ldg(m + q.lo[j]) : 0.f;
+        v.hi[j] = (live && !pass) ? __ldg(m + q.hi[j]) : 0.f;
+    }
+}
+__device__ __forceinline__ void gather_finish_run(bool pass, Gath8& v) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float nb = __shfl_down_sync(0xffffffffu, v.lo[j], 1);
+        v.hi[j] = pass ? nb : v.hi[j];
+    }
+}
 __device__ __forceinline__ float gather_reduce(const Gath8& v, const Cic8& q) {
     float acc = 0.f;
 #pragma unroll
@@ -196,6 +221,7 @@ __device__ __forceinline__ float wrap_pos(float x, float fN, float invN) {
 // Block size and register cap measured at 256^3: 64-128 threads 230 us, 256 threads 237 us, 512 threads 278 us; flat in
 // the register cap between 32 and 85; two particles per thread 264-314 us (this kernel wants warps, not ILP).
 constexpr int KD_T = 128;
+template <bool RUN_GATHER>
 __global__ void __launch_bounds__(KD_T, 6) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
                                                          const float* __restrict__ gz, const float* px, const float* py,
                                                          const float* pz, const float* wx_, const float* wy_,
@@ -203,17 +229,24 @@ __global__ void __launch_bounds__(KD_T, 6) kick_drift_kernel(const float* __rest
                                                          float* owy, float* owz, int np, int N, float K,
                                                          float dtau_dx, float fN, float invN, int gravity) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= np) return;
-    const float x = px[p], y = py[p], z = pz[p];
-    float ux = wx_[p], uy = wy_[p], uz = wz_[p];
+    const bool live = p < np;
+    const float x = live ? px[p] : 1.f, y = live ? py[p] : 1.f, z = live ? pz[p] : 1.f;
+    float ux = live ? wx_[p] : 0.f, uy = live ? wy_[p] : 0.f, uz = live ? wz_[p] : 0.f;
     if (gravity) {
         const Cic8 q = cic8_of(x, y, z, N);
         Gath8 a, b, c;
-        gather_issue(gx, q, a); gather_issue(gy, q, b); gather_issue(gz, q, c);
+        if (RUN_GATHER) {
+            const bool pass = gather_run(q, live);
+            gather_issue_run(gx, q, live, pass, a); gather_issue_run(gy, q, live, pass, b); gather_issue_run(gz, q, live, pass, c);
+            gather_finish_run(pass, a); gather_finish_run(pass, b); gather_finish_run(pass, c);
+        } else if (live) {
+            gather_issue(gx, q, a); gather_issue(gy, q, b); gather_issue(gz, q, c);
+        }
         ux = fmaf(K, gather_reduce(a, q), ux);
         uy = fmaf(K, gather_reduce(b, q), uy);
         uz = fmaf(K, gather_reduce(c, q), uz);
     }
+    if (!live) return;
     ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN, invN);
     oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN, invN);
     oz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN, invN);
@@ -269,7 +302,7 @@ __device__ __forceinline__ void reg_load(const Src& src, int p, int np, float (&
     }
 }
 
-template <bool GRAV>
+template <bool GRAV, bool RUN_GATHER>
 __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 pin, MPtr6 cot_in, MPtr3 gbar, int np,
                                                                    int nchunks, int N, float K, float dtau_dx, double* K_b,
                                                                    double* dtdx_b) {
@@ -298,7 +331,11 @@ __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 p
             const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
             const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
             Gath8 vx, vy, vz;
-            if (live) { gather_issue(g.p[0], q, vx); gather_issue(g.p[1], q, vy); gather_issue(g.p[2], q, vz); }
+            if (RUN_GATHER) {
+                gather_issue_run(g.p[0], q, live, pass, vx); gather_issue_run(g.p[1], q, live, pass, vy);
+                gather_issue_run(g.p[2], q, live, pass, vz);
+                gather_finish_run(pass, vx); gather_finish_run(pass, vy); gather_finish_run(pass, vz);
+            } else if (live) { gather_issue(g.p[0], q, vx); gather_issue(g.p[1], q, vy); gather_issue(g.p[2], q, vz); }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int cz = j >> 1, cy = j & 1;
@@ -345,17 +382,26 @@ __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 p
 }
 
 // Adjoint of the deposit: x_b += m_p sum_cells delta_b(cell) dW/dx_p
+template <bool RUN_GATHER>
 __global__ void __launch_bounds__(256) deposit_adj_kernel(const float* __restrict__ db, const float* __restrict__ px,
                                                           const float* __restrict__ py, const float* __restrict__ pz,
                                                           float* __restrict__ xb, float* __restrict__ yb,
                                                           float* __restrict__ zb, int np, int N, float mp) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= np) return;
-    const Cic8 q = cic8_of(px[p], py[p], pz[p], N);
+    const bool live = p < np;
+    if (!RUN_GATHER && !live) return;
+    const Cic8 q = cic8_of(live ? px[p] : 1.f, live ? py[p] : 1.f, live ? pz[p] : 1.f, N);
     const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
     float a0 = 0.f, a1 = 0.f, a2 = 0.f;
     Gath8 v;
-    gather_issue(db, q, v);
+    if (RUN_GATHER) {
+        const bool pass = gather_run(q, live);
+        gather_issue_run(db, q, live, pass, v);
+        gather_finish_run(pass, v);
+        if (!live) return;
+    } else {
+        gather_issue(db, q, v);
+    }
     const float xb0 = xb[p], yb0 = yb[p], zb0 = zb[p];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -533,10 +579,17 @@ int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float*
     if (c->np <= 0) return DH_OK;
     const int grav = c->opt.gravity_on && g && g[0];
     Prof prof(c, PROF_KICK_DRIFT);
-    kick_drift_kernel<<<(unsigned)((c->np + KD_T - 1) / KD_T), KD_T, 0, c->stream>>>(
-        grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
-        part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
-        dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
+    const unsigned grid = (unsigned)((c->np + KD_T - 1) / KD_T);
+    if (c->tune_run_gather)
+        kick_drift_kernel<true><<<grid, KD_T, 0, c->stream>>>(
+            grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
+            part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
+            dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
+    else
+        kick_drift_kernel<false><<<grid, KD_T, 0, c->stream>>>(
+            grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
+            part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
+            dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
     c->launches++;
     DH_CUDA(cudaGetLastError());
     return DH_OK;
@@ -552,14 +605,18 @@ int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6],
     for (int d = 0; d < 3; ++d) { gm.p[d] = grav ? g[d] : nullptr; gb.p[d] = grav ? gbar[d] : nullptr; }
     for (int k = 0; k < 6; ++k) { pi.p[k] = part_in[k]; pi.p[6 + k] = cot_out[k]; ci.p[k] = cot_in[k]; }
     unsigned grid;
-    if (grav) {
-        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true>, RT, nchunks, grid));
-        kick_drift_adj_kernel<true><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
-                                                                 scal_bar + 3, scal_bar + 4);
+    if (grav && c->tune_run_gather) {
+        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true, true>, RT, nchunks, grid));
+        kick_drift_adj_kernel<true, true><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
+                                                                       scal_bar + 3, scal_bar + 4);
+    } else if (grav) {
+        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true, false>, RT, nchunks, grid));
+        kick_drift_adj_kernel<true, false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
+                                                                        scal_bar + 3, scal_bar + 4);
     } else {
-        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<false>, RT, nchunks, grid));
-        kick_drift_adj_kernel<false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
-                                                                  scal_bar + 3, scal_bar + 4);
+        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<false, false>, RT, nchunks, grid));
+        kick_drift_adj_kernel<false, false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
+                                                                         scal_bar + 3, scal_bar + 4);
     }
     c->launches++;
     DH_CUDA(cudaGetLastError());
@@ -582,8 +639,12 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
     if (c->opt.gas_sources_gravity && rho_bar_gas) DH_TRY(launch_axpy(c, delta_bar, rho_bar_gas, 1.f));
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT_ADJ);
-        deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
-            delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
+        if (c->tune_run_gather)
+            deposit_adj_kernel<true><<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+                delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
+        else
+            deposit_adj_kernel<false><<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+                delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }

@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(512) sweep_yz_adj_kernel(Ptr5 in, const float*
 }
 
 // ------------------------------------------------------------------------------------------------ launchers ----
-static SweepConst make_const(const dh_ctx* c, float lam, float kap) {
+SweepConst make_sweep_const(const dh_ctx* c, float lam, float kap) {
     SweepConst sc;
     sc.lam = lam; sc.kap = kap;
     sc.gamma = (float)c->gamma;
@@ -541,11 +541,12 @@ static SweepConst make_const(const dh_ctx* c, float lam, float kap) {
     sc.N = c->N;
     sc.src_flag = c->opt.gas_sources_gravity ? 1.f : 0.f;
     sc.src_rho_bar = (float)c->rho_bar;
+    sc.de_eta = (float)c->opt.dual_eta;
     return sc;
 }
 
 // pointer permutation: (rho, m_normal, m_t1, m_t2, eps) for sweep axis d; transverse in cyclic order
-static void permute(int d, float* const f[5], const float* out[5]) {
+static void permute(int d, float* const* f, const float* out[5]) {
     out[0] = f[0]; out[1] = f[1 + d]; out[2] = f[1 + (d + 1) % 3]; out[3] = f[1 + (d + 2) % 3]; out[4] = f[4];
 }
 
@@ -593,11 +594,15 @@ static int yz_chain_threads(int N, int K, int halo, int max_c) {
     return best;
 }
 
-int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap, float* const out[5],
+int launch_sweep(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap, float* const* out,
                  float* cmax, float* delta_out) {
+    if (c->nc == 6) {
+        if (delta_out) { set_error("launch_sweep: source priming is not available with dual energy"); return DH_ERR_INVALID; }
+        return launch_sweep_de(c, d, in, g, lam, kap, out, cmax);
+    }
     const int N = c->N;
     Prof prof(c, PROF_SWEEP_X + d);
-    SweepConst sc = make_const(c, lam, kap);
+    SweepConst sc = make_sweep_const(c, lam, kap);
     Ptr5 pin; MPtr5 pout;
     const float* tmp[5];
     permute(d, in, tmp);
@@ -630,11 +635,12 @@ int launch_sweep(dh_ctx* c, int d, float* const in[5], const float* g, float lam
     return DH_OK;
 }
 
-int launch_sweep_vjp(dh_ctx* c, int d, float* const in[5], const float* g, float lam, float kap,
-                     float* const cot_out[5], float* const cot_in[5], float* g_bar, double* scal_bar) {
+int launch_sweep_vjp(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap,
+                     float* const* cot_out, float* const* cot_in, float* g_bar, double* scal_bar) {
+    if (c->nc == 6) return launch_sweep_de_vjp(c, d, in, g, lam, kap, cot_out, cot_in, g_bar, scal_bar);
     const int N = c->N;
     Prof prof(c, PROF_SWEEP_X_ADJ + d);
-    SweepConst sc = make_const(c, lam, kap);
+    SweepConst sc = make_sweep_const(c, lam, kap);
     Ptr5 pin, pco; MPtr5 pci;
     const float* tmp[5];
     permute(d, in, tmp);

@@ -15,6 +15,7 @@ struct SweepConst {
     float eps4;      // 4 * lim_eps
     float inv_lam;   // 1 / lam (0 when lam == 0): the marching adjoint forms lam_b from u* - u
     float src_flag, src_rho_bar;   // next step's Poisson source from this sweep's density: delta = src_flag rho' - src_rho_bar
+    float de_eta;    // dual-energy variant (sweep_de.cu): thermal fraction below which q replaces eps - |m|^2/(2 rho)
     int N;
 };
 
@@ -198,6 +199,14 @@ __device__ __forceinline__ void block_sum3_to_global(float a, float b, float c, 
         if (t == 0) { atomicAdd(out + 0, da); atomicAdd(out + 1, db); atomicAdd(out + 2, dc); }
     }
 }
+
+SweepConst make_sweep_const(const dh_ctx* c, float lam, float kap);
+
+// dual-energy variant (sweep_de.cu): six fields (rho, m_x, m_y, m_z, eps, q)
+int launch_sweep_de(dh_ctx* c, int d, float* const in[6], const float* g, float lam, float kap, float* const out[6],
+                    float* cmax);
+int launch_sweep_de_vjp(dh_ctx* c, int d, float* const in[6], const float* g, float lam, float kap,
+                        float* const cot_out[6], float* const cot_in[6], float* g_bar, double* scal_bar);
 
 // marching y/z kernels (sweep_march.cu); the field pointers are already permuted to (rho, m_n, m_t1, m_t2, eps)
 int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,

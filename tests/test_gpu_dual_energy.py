@@ -1,0 +1,316 @@
+"""Dual-energy variant (readings R33-R36) on the GPU against oracle/dual_energy.py:
+the six-field sweep and its transpose on all three axes with both branches of the selection active, a hydro-only run and
+its reverse pass, the coupled run, the initial-condition map's sixth field, finite differences of the GPU's own loss, what
+the formalism is for (a Mach-1000 flow in fp32), and the measurement VERDICT r01 asks for: the thermal energy of config 2
+at a = 0.33 in fp32 with and without it."""
+import numpy as np
+import pytest
+
+import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-5
+TOL_GRAD = 1e-3
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2502_02294_b200 import api
+    return api
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+@pytest.fixture(scope="module")
+def DE():
+    from oracle import dual_energy
+    return dual_energy
+
+
+def _gpu(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _state6(W, N, seed, mach=2.5, amp=0.3):
+    """Smooth random state whose thermal fraction straddles its own median (so eta = median splits the cells), with an
+    internal energy that has drifted from rho e_T by 5 %.  Returns (fp32 state (6,N,N,N), eta)."""
+    gas, _ = W.smooth_random_state(N, seed, amp=amp, n_part_side=2, mach=mach)
+    rho = gas[0]
+    eT = gas[4] / rho - 0.5 * np.sum(gas[1:4] ** 2, axis=0) / rho ** 2
+    rng = np.random.default_rng(seed + 1)
+    q = rho * eT * (1.0 + 0.05 * rng.standard_normal(rho.shape))
+    g6 = np.concatenate([gas, q[None]], axis=0).astype(np.float32)
+    frac = (g6[4].astype(np.float64) - 0.5 * np.sum(g6[1:4].astype(np.float64) ** 2, axis=0) / g6[0]) / g6[4]
+    return g6, float(np.median(frac))
+
+
+def _err6(got, ref):
+    e = PT.field_err(got[:5], ref[:5])
+    e["q"] = np.max(np.abs(got[5].astype(np.float64) - ref[5])) / np.max(np.abs(ref[5]))
+    return e
+
+
+@pytest.mark.parametrize("N", [32, 64, 96])
+@pytest.mark.parametrize("d", [0, 1, 2])
+@pytest.mark.parametrize("with_g", [True, False])
+def test_de_sweep_matches_oracle(api, torch_, DE, W, N, d, with_g):
+    g6, eta = _state6(W, N, 200 + d)
+    rng = np.random.default_rng(9)
+    g = (0.3 * rng.standard_normal((N, N, N))).astype(np.float32) if with_g else None
+    lam, kap, gamma = 0.07, 0.05 if with_g else 0.0, 1.5
+    eT = g6[4] / g6[0] - 0.5 * np.sum(g6[1:4].astype(np.float64) ** 2, axis=0) / g6[0].astype(np.float64) ** 2
+    e_floor = float(np.quantile(eT, 0.05))
+    ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=e_floor, dual_energy=1,
+                      dual_eta=eta)
+    cm = torch_.zeros(1, device="cuda")
+    out = ctx.dh_sweep_de(d, _gpu(torch_, g6), _gpu(torch_, g) if with_g else None, lam, kap, cm).cpu().numpy()
+    ref, cm_ref = DE.sweep(g6, d, lam, kap, gamma, g, e_floor=e_floor, eta=eta)
+    # cells whose selection sits within fp32 rounding of the threshold -- in the input or in the half-step state u* -- may
+    # take the other branch (q differs from rho e_T by 5 % there)
+    frac = eT * g6[0] / g6[4]
+    comp = (0, 1 + d, 1 + (d + 1) % 3, 1 + (d + 2) % 3, 4)
+    R = DE._forward([g6[k].astype(np.float64) for k in comp], g6[5].astype(np.float64),
+                    None if g is None else g.astype(np.float64), lam, kap, gamma, e_floor, 1e-20, eta, 2 - d)
+    us = R["us"]
+    frac_s = 1.0 - 0.5 * (us[1] ** 2 + us[2] ** 2 + us[3] ** 2) / (us[0] * us[4])
+    near = (np.abs(frac - eta) < 1e-5) | (np.abs(frac_s - eta) < 1e-5)
+    e = _err6(out, ref)
+    print(f"DE sweep N={N} d={d} g={with_g}: {e}; cells within 1e-5 of the selection threshold: {near.sum()}")
+    if near.sum() == 0:
+        assert max(e.values()) < TOL_STEP, e
+    else:
+        far = ~np.logical_or.reduce([np.roll(near, s, axis=2 - d) for s in range(-4, 5)])
+        for k in range(6):
+            assert np.max(np.abs(out[k] - ref[k])[far]) < TOL_STEP * np.max(np.abs(ref[k]))
+    assert abs(float(cm) / cm_ref - 1) < TOL_STEP
+    ctx.close()
+
+
+@pytest.mark.parametrize("N", [32, 64])
+@pytest.mark.parametrize("d", [0, 1, 2])
+@pytest.mark.parametrize("with_g", [True, False])
+def test_de_sweep_vjp_matches_oracle(api, torch_, DE, W, N, d, with_g):
+    g6, eta = _state6(W, N, 300 + d)
+    rng = np.random.default_rng(19)
+    g = (0.3 * rng.standard_normal((N, N, N))).astype(np.float32) if with_g else None
+    cot = rng.standard_normal(g6.shape).astype(np.float32)
+    lam, kap, gamma = 0.07, 0.05 if with_g else 0.0, 1.5
+    eT = g6[4] / g6[0] - 0.5 * np.sum(g6[1:4].astype(np.float64) ** 2, axis=0) / g6[0].astype(np.float64) ** 2
+    e_floor = float(np.quantile(eT, 0.05))
+    ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=e_floor, dual_energy=1,
+                      dual_eta=eta)
+    cin, gb, sc = ctx.dh_sweep_de_vjp(d, _gpu(torch_, g6), _gpu(torch_, g) if with_g else None, lam, kap, _gpu(torch_, cot))
+    cin, sc = cin.cpu().numpy(), sc.cpu().numpy()
+    rin, rgb, rsc = DE.sweep_vjp(g6, d, lam, kap, gamma, cot, g, e_floor=e_floor, eta=eta)
+    assert np.all(np.isfinite(cin))
+    e_all, e_trim = PT.rel_l2(cin, rin), PT.rel_l2_trimmed(cin, rin, frac=1e-3)
+    e_q = PT.rel_l2_trimmed(cin[5], rin[5], frac=1e-3)
+    print(f"DE sweep vjp N={N} d={d} g={with_g}: rel L2 {e_all:.2e}, trimmed 1e-3 {e_trim:.2e}, q component {e_q:.2e}; "
+          f"scalars {sc} vs {rsc}")
+    # smooth state: the switches (limiter gate, floor, selection) that fp32 rounding can flip are few (reading R28)
+    assert e_trim < 2e-5 and e_q < 2e-5 and e_all < 5e-3
+    if with_g:
+        assert PT.rel_l2(gb.cpu().numpy(), rgb) < 1e-3
+    for k, key in ((0, "lam"), (1, "kap"), (2, "gamma")):
+        assert abs(sc[k] - rsc[key]) < 1e-3 * max(abs(rsc[key]), np.sqrt(g6[0].size)), (key, sc[k], rsc[key])
+    ctx.close()
+
+
+def test_de_hydro_run_and_reverse_match_oracle(api, torch_, DE, W):
+    """Static hydro-only run of 6 steps (one Strang cycle) with dual energy: dh_run / dh_run_vjp (snapshots, tapes with six
+    fields) against the oracle's run and reverse pass."""
+    N, gamma = 32, 1.5
+    g6, eta = _state6(W, N, 400)
+    lams = [0.05, 0.06, 0.04, 0.05, 0.055, 0.045]
+    ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-6, dual_energy=1,
+                      dual_eta=eta)
+    st = api.State(g6, np.zeros((6, 0), dtype=np.float32), 1.0)
+    ctx.dh_run(st, np.ones(len(lams)), np.array(lams), 4)                 # static mode: dtau = dt, dx = 1 -> lam = dt
+    ref, cm_ref = DE.hydro_run(g6, gamma, lams, e_floor=1e-6, eta=eta)
+    e = _err6(st.gas.cpu().numpy(), ref)
+    print(f"DE hydro run: {e}")
+    assert max(e.values()) < 1e-4, e
+    assert np.max(np.abs(ctx.dh_get_cmax(len(lams)) / cm_ref - 1)) < 1e-4
+    cot = np.zeros_like(ref); cot[0] = ref[0]; cot[5] = 1.0
+    ct = api.Cot(_gpu(torch_, cot), torch_.zeros((6, 0), device="cuda"))
+    dp = ctx.dh_run_vjp(ct, ct)
+    rg, dgamma = DE.hydro_run_vjp(g6, gamma, lams, cot, e_floor=1e-6, eta=eta)
+    got = ct.gas.cpu().numpy()
+    e_all, e_trim = PT.rel_l2(got, rg), PT.rel_l2_trimmed(got, rg, frac=1e-2)
+    print(f"DE hydro run VJP: rel L2 {e_all:.2e} (all but the worst 1 %: {e_trim:.2e}), dgamma {dp.dgamma:.6g} vs {dgamma:.6g}")
+    assert np.all(np.isfinite(got)) and e_trim < TOL_GRAD and e_all < 2e-2
+    assert abs(dp.dgamma / dgamma - 1) < 5e-3
+    ctx.close()
+
+
+def test_de_coupled_run_matches_oracle_and_ic_fills_q(api, torch_, O, DE, W, IC):
+    """Config 0's recipe for 6 steps with dual energy on: the coupled run against the oracle's composition, from the state
+    the library's IC map makes (q = rho e~_0)."""
+    cfg = W.scaled_config(0, 32, n_steps=6, a1=0.03)
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    ctx = api.context_for(cfg, dual_energy=1, dual_eta=1e-3)
+    vf, e0 = api.ic_factors_for(cfg)
+    st = ctx.dh_ic_zeldovich(_gpu(torch_, delta), cfg.a0, vf, e0)
+    g0 = st.gas.cpu().numpy()
+    assert g0.shape[0] == 6
+    assert np.max(np.abs(g0[5] - e0 * g0[0].astype(np.float64))) < 1e-6 * np.max(g0[5])
+    assert max(PT.field_err(g0[:5], gas).values()) < 1e-5
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    part0 = st.part.cpu().numpy()
+    ref6, refp, cm_ref = DE.coupled_run(O, P, g0, part0, cfg.a0, a_s[1:], dt_s, eta=1e-3)
+    ctx.dh_run(st, a_s[1:], dt_s, 3)
+    e = _err6(st.gas.cpu().numpy(), ref6)
+    e.update(PT.part_err(st.part.cpu().numpy(), refp, cfg.N))
+    print(f"DE coupled run (6 steps): {e}")
+    assert max(e.values()) < 1e-4, e
+    assert np.max(np.abs(ctx.dh_get_cmax(cfg.n_steps) / cm_ref - 1)) < 1e-4
+    ctx.close()
+
+
+def test_de_gradient_against_finite_differences_of_the_gpu_loss(api, torch_, W):
+    """delta_init -> IC map (six fields) -> 20 steps with dual energy -> loss, and back through dh_run_vjp and the IC
+    transpose: <dL/d delta_init, v> against central differences of the library's own loss."""
+    cfg = W.CONFIGS[0]
+    delta = W.gaussian_field(cfg.N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)
+    target = _gpu(torch_, cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, 4242, cfg.rms_delta)))
+    ctx = api.context_for(cfg, dual_energy=1, dual_eta=1e-3)
+    vf, e0 = api.ic_factors_for(cfg)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+
+    def loss(d_, want_grad=False):
+        dd = _gpu(torch_, d_)
+        st = ctx.dh_ic_zeldovich(dd, cfg.a0, vf, e0)
+        ctx.dh_run(st, a_s[1:], dt_s, 10 if want_grad else 0)
+        if not want_grad:
+            return ctx.dh_data_term(0, st.gas, target, None, 1.0, 1.0, None), st
+        cg = torch_.zeros_like(st.gas)
+        L = ctx.dh_data_term(0, st.gas, target, None, 1.0, 1.0, cg)
+        ct = api.Cot(cg, torch_.zeros_like(st.part))
+        ctx.dh_run_vjp(ct, ct)
+        return L, ctx.dh_ic_zeldovich_vjp(dd, vf, e0, ct).double().cpu().numpy(), st
+    L, grad, st = loss(delta, True)
+    g = st.gas.double()
+    eT = g[4] / g[0] - 0.5 * (g[1:4] ** 2).sum(0) / g[0] ** 2
+    used_q = float((eT <= 1e-3 * g[4] / g[0]).double().mean())
+    print(f"DE chain: loss {L:.6e}; cells whose pressure comes from q at the end of the run: {used_q:.2f}")
+    assert used_q > 0.05
+    c = (np.arange(cfg.N) + 0.5) / cfg.N
+    z, y, x = np.meshgrid(c, c, c, indexing="ij")
+    for j, k in enumerate([(1, 0, 0), (1, 2, 1)]):
+        v = np.cos(2 * np.pi * (k[0] * x + k[1] * y + k[2] * z) + 0.3 * j)
+        an = float(np.sum(grad * v))
+        best = None
+        for h in (1e-2, 3e-3, 1e-3, 3e-4):
+            fd = (loss((delta + h * v).astype(np.float32))[0] - loss((delta - h * v).astype(np.float32))[0]) / (2 * h)
+            print(f"DE chain dir {j} h {h}: <grad,v> {an:.6e}  FD {fd:.6e}  ratio-1 {an / fd - 1:+.2e}")
+            best = abs(an / fd - 1) if best is None else min(best, abs(an / fd - 1))
+        assert best < 2e-2
+    ctx.close()
+
+
+def _advect_gpu(api, torch_, N, mach, steps, dual):
+    gamma = 5.0 / 3.0
+    x = (np.arange(N) + 0.5) / N
+    rho = np.broadcast_to(1.0 + 0.3 * np.sin(2 * np.pi * x), (N, N, N))
+    p0 = 1.0
+    cs = np.sqrt(gamma * p0 / 0.7)
+    v = mach * np.sqrt(gamma * p0)
+    u = np.zeros((6, N, N, N))
+    u[0] = rho; u[1] = rho * v
+    u[4] = p0 / (gamma - 1) + 0.5 * rho * v * v
+    u[5] = p0 / (gamma - 1)
+    lam = 0.4 / (v + cs)
+    ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-6,
+                      dual_energy=int(dual), dual_eta=1e-3)
+    cur = _gpu(torch_, u if dual else u[:5])
+    for _ in range(steps):
+        cur = ctx.dh_sweep_de(0, cur, None, lam, 0.0) if dual else ctx.dh_sweep(0, cur, None, lam, 0.0)
+    ctx.close()
+    out = cur.double().cpu().numpy()
+    eT = out[4] / out[0] - 0.5 * out[1] ** 2 / out[0] ** 2
+    if dual:
+        e = np.where(eT > 1e-3 * out[4] / out[0], eT, out[5] / out[0])
+    else:
+        e = eT
+    return (gamma - 1) * out[0] * e / p0
+
+
+def test_mach_1000_flow_keeps_its_temperature_only_with_dual_energy(api, torch_):
+    """PAPER.md:85.  A 30 % density wave carried at Mach 1000 with uniform pressure, 200 x sweeps on the GPU (fp32): the
+    single-energy path loses the temperature to the cancellation in e_T, the dual-energy path keeps it (the oracle's fp32
+    emulation of the same experiment: tests/test_oracle_dual_energy.py)."""
+    p_single = _advect_gpu(api, torch_, 32, 1000.0, 200, dual=False)
+    p_dual = _advect_gpu(api, torch_, 32, 1000.0, 200, dual=True)
+    print(f"Mach 1000 advection on the GPU: max |p/p0 - 1| single energy {np.max(np.abs(p_single - 1)):.3f}, "
+          f"dual energy {np.max(np.abs(p_dual - 1)):.2e}")
+    assert np.max(np.abs(p_single - 1)) > 0.1
+    assert np.max(np.abs(p_dual - 1)) < 1e-3
+
+
+def test_config2_thermal_energy_at_late_time_with_and_without_dual_energy(api, torch_, O, DE, W, IC):
+    """VERDICT r01 missing #1: "measure the thermal-energy error of config 2 at a = 0.33 in fp32 with and without it"
+    (SURVEY.md section 7 hard part 3: e~ = eps/rho - |m|^2/(2 rho^2) has an fp32 error of 6e-8 Mach^2).  Four runs of
+    config 2's 100 steps from the same fp32 state: GPU and fp64 oracle, each single and dual energy.  Reported: the Mach
+    numbers reached, the error of the thermal energy each fp32 run has against its own fp64 oracle, per Mach-number class."""
+    cfg = W.CONFIGS[2]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    vf, e0 = api.ic_factors_for(cfg)
+    eta = 1e-3
+    g6 = np.concatenate([gas, (e0 * gas[0].astype(np.float64))[None].astype(np.float32)], axis=0)
+    # fp64 references
+    ref1, _, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:], dt_s)
+    ref2, _, _ = DE.coupled_run(O, P, g6, part, cfg.a0, a_s[1:], dt_s, eta=eta)
+    # fp32 runs
+    c1 = api.context_for(cfg)
+    s1 = api.State(gas, part, cfg.a0)
+    c1.dh_run(s1, a_s[1:], dt_s, 0)
+    got1 = s1.gas.double().cpu().numpy()
+    c1.close()
+    c2 = api.context_for(cfg, dual_energy=1, dual_eta=eta)
+    s2 = api.State(g6, part, cfg.a0)
+    c2.dh_run(s2, a_s[1:], dt_s, 0)
+    got2 = s2.gas.double().cpu().numpy()
+    c2.close()
+
+    def e_single(g):
+        return g[4] / g[0] - 0.5 * np.sum(g[1:4] ** 2, axis=0) / g[0] ** 2
+    fl = cfg.e_floor()
+    eR1, eG1 = np.maximum(e_single(ref1), fl), np.maximum(e_single(got1), fl)
+    eR2, eG2 = np.maximum(DE.thermal_energy(ref2, eta), fl), np.maximum(DE.thermal_energy(got2, eta), fl)
+    ke = 0.5 * np.sum(ref1[1:4] ** 2, axis=0) / ref1[0] ** 2
+    mach = np.sqrt(2 * ke / (cfg.gamma * (cfg.gamma - 1) * eR1))
+    print(f"config2 at a = {cfg.a1}: Mach number median {np.median(mach):.0f}, max {mach.max():.0f}; cells at the energy "
+          f"floor: single fp64 {np.mean(eR1 <= fl):.3f}, fp32 {np.mean(eG1 <= fl):.3f}; dual fp64 {np.mean(eR2 <= fl):.3f}, "
+          f"fp32 {np.mean(eG2 <= fl):.3f}")
+    print(f"   conserved fields fp32 vs fp64: single {max(PT.field_err(got1[:5], ref1).values()):.1e}, dual "
+          f"{max(PT.field_err(got2[:5], ref2[:5]).values()):.1e}")
+    rows = []
+    for lo, hi in ((0, 30), (30, 100), (100, 300), (300, 1e9)):
+        m = (mach >= lo) & (mach < hi)
+        if m.sum() == 0:
+            continue
+        r1 = np.abs(eG1 / eR1 - 1)[m]
+        r2 = np.abs(eG2 / eR2 - 1)[m]
+        rows.append((lo, hi, m.mean(), np.median(r1), np.quantile(r1, 0.99), np.median(r2), np.quantile(r2, 0.99)))
+        print(f"   Mach [{lo}, {hi}): {m.mean():.3f} of the cells; |e~_fp32 / e~_fp64 - 1| median / 99 %: single "
+              f"{rows[-1][3]:.1e} / {rows[-1][4]:.1e}, dual {rows[-1][5]:.1e} / {rows[-1][6]:.1e}")
+    # fp32 parity of the dual-energy run with its own oracle in the R25 norms, and finite everywhere
+    assert np.all(np.isfinite(got2))
+    # (the selection is one more switch that an fp32 rounding can flip, and unlike the limiter gate it is a jump in the
+    # VALUE of the pressure where q and rho e_T have drifted apart: B200 measures 1.2e-3 after 100 steps, 2.2e-4 without)
+    assert max(PT.field_err(got2[:5], ref2[:5]).values()) < 5e-3
+    # what the formalism is for: where the single-energy run has lost the thermal energy (Mach > 100) the dual-energy run
+    # keeps it to a few per cent, and nothing sits on the floor
+    hi = [r for r in rows if r[0] >= 100]
+    assert all(r[5] < 1e-2 for r in hi) and np.mean(eG2 <= fl) < 0.01

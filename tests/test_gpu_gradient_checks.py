@@ -181,10 +181,102 @@ def test_config2_late_step_vjp_matches_oracle(api, torch_, O, W, IC, k):
     # the floor switch (R17, R26) falls on either side there and those entries -- and d gamma, which sums rho e+ terms --
     # move by O(1).  North-star bound on all but the worst 0.1 % of entries; everything finite; particles (no floor) tight.
     assert np.all(np.isfinite(co.gas.cpu().numpy())) and np.all(np.isfinite(co.part.cpu().numpy()))
-    assert et < 1e-3 and ep < 5e-3 and eg < 0.3
+    assert et < 1e-3 and ep < 5e-3
     got = np.array([dp.dgamma, dp.dDtau, dp.dkappa, dp.dK, dp.dA])
     scale = np.abs(rdp) + 1e-3 * np.max(np.abs(rdp))
-    print("   dparams", got, "oracle", rdp)
-    assert np.all(np.abs(got - rdp)[1:] < 5e-3 * scale[1:]), (got, rdp)
-    assert abs(got[0] - rdp[0]) < 0.2 * max(abs(rdp[0]), 1.0)
+    # the scalar cotangents are sums over all cells, the switched entries included: the same oracle VJP with its input
+    # moved by one fp32 rounding says how far they are defined (reading R28)
+    prng = np.random.default_rng(1000 + k)
+    s_pert = O.State(gas_k.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas_k.shape)), part_k, a_s[k],
+                     dt_prev=dt_s[k - 1], step=k)
+    rg2, rp2, rdp2 = O.step_vjp(P, s_pert, dt_s[k], a_s[k + 1], cg, cp)
+    sens_g = PT.rel_l2(rg2, rg)
+    print(f"   the oracle's gas cotangent under one fp32 rounding of its input moves by {sens_g:.2e}")
+    assert eg < max(0.3, 2.0 * sens_g)
+    print("   dparams", got, "oracle", rdp, "oracle under one fp32 rounding of its input", rdp2)
+    assert np.all(np.abs(got - rdp)[1:] < np.maximum(5e-3 * scale[1:], 3.0 * np.abs(rdp2 - rdp)[1:])), (got, rdp, rdp2)
+    assert abs(got[0] - rdp[0]) < max(0.2 * max(abs(rdp[0]), 1.0), 3.0 * abs(rdp2[0] - rdp[0])), (got[0], rdp[0], rdp2[0])
     ctx.close()
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_sweep_and_its_vjp_with_a_large_limiter_epsilon(api, torch_, O, W, d):
+    """Eq. 18's epsilon at the scale of the limiter's arguments (lim_eps = 1e-2 on O(1) fluxes): the kernels' epsilon
+    branches (denominator and numerators of the partials) against the oracle, free of any multi-step amplification."""
+    N, eps = 64, 1e-2
+    gas, _ = W.smooth_random_state(N, 31 + d, amp=0.1, n_part_side=2)
+    gas = gas.astype(np.float32)
+    rng = np.random.default_rng(3 + d)
+    g = (0.2 * rng.standard_normal((N, N, N))).astype(np.float32)
+    cot = rng.standard_normal(gas.shape).astype(np.float32)
+    lam, kap, gamma = 0.11, 0.07, 5.0 / 3.0
+    ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-6, lim_eps=eps)
+    out = ctx.dh_sweep(d, _gpu(torch_, gas), _gpu(torch_, g), lam, kap).cpu().numpy()
+    ref, _ = O.sweep(gas.astype(np.float64), d, lam, kap, gamma, g.astype(np.float64), e_floor=1e-6, lim_eps=eps)
+    ref0, _ = O.sweep(gas.astype(np.float64), d, lam, kap, gamma, g.astype(np.float64), e_floor=1e-6, lim_eps=1e-20)
+    assert max(PT.field_err(out, ref).values()) < 1e-5
+    assert max(PT.field_err(ref0, ref).values()) > 1e-4          # the epsilon matters at this size
+    cin, gb, sc = ctx.dh_sweep_vjp(d, _gpu(torch_, gas), _gpu(torch_, g), lam, kap, _gpu(torch_, cot))
+    rin, rgb, rsc = O.sweep_vjp(gas.astype(np.float64), d, lam, kap, gamma, cot.astype(np.float64), g.astype(np.float64),
+                                e_floor=1e-6, lim_eps=eps)
+    e_all, e_trim = PT.rel_l2(cin.cpu().numpy(), rin), PT.rel_l2_trimmed(cin.cpu().numpy(), rin, frac=2e-4)
+    print(f"sweep vjp with lim_eps 1e-2, d={d}: rel L2 {e_all:.2e} (trimmed {e_trim:.2e}), g_bar {PT.rel_l2(gb.cpu().numpy(), rgb):.2e}")
+    assert e_all < 1e-3 and e_trim < 2e-5 and PT.rel_l2(gb.cpu().numpy(), rgb) < 1e-3
+    sc = sc.cpu().numpy()
+    for k, key in ((0, "lam"), (1, "kap"), (2, "gamma")):
+        assert abs(sc[k] - rsc[key]) < 1e-3 * max(abs(rsc[key]), np.sqrt(gas[0].size)), (key, sc[k], rsc[key])
+    ctx.close()
+
+
+@pytest.mark.parametrize("which", [0, 2])
+def test_gradient_conditioning_against_the_limiter_epsilon(api, torch_, O, W, IC, which):
+    """VERDICT r01 weak #2 (iv), the experiment of DESIGN.md reading R28: the same gradient (configs 0 and 2, the configs'
+    own losses) with the epsilon of Eq. 18 ("regular near a = b = 0") raised from 1e-20 to the scale of
+    the limiter's arguments.  For each value: how far the fp64 oracle's gradient moves under one fp32 rounding of its
+    input, and how far the GPU is from it.  With |a + b| << eps the jump of d phi / d a at the gate, 2 b / (b + eps), closes, so
+    both numbers must fall together; the bound on the GPU is the conditioning rule of R28 at every epsilon."""
+    cfg = W.CONFIGS[which]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    target = None
+    if which == 2:
+        target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.target_seed, cfg.rms_delta))
+    rows = []
+    for eps in (1e-20, 1e-4, 1e-2, 1.0):
+        P = PT.oracle_params(O, cfg, lim_eps=eps)
+        a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+
+        def oracle_grad(g_, p_):
+            gf, pf, _, _ = O.run(P, g_, p_, cfg.a0, a_s[1:], dt_s)
+            cot = np.zeros_like(gf)
+            cot[0] = gf[0] / np.linalg.norm(gf[0]) if target is None else 2.0 * (gf[0] - target)
+            return O.run_vjp(P, g_, p_, cfg.a0, a_s[1:], dt_s, cot, np.zeros_like(pf))[0], gf
+        rg, gf = oracle_grad(gas, part)
+        prng = np.random.default_rng(7)
+        rg2, _ = oracle_grad(gas.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(gas.shape)),
+                             part.astype(np.float64) * (1.0 + 6e-8 * prng.standard_normal(part.shape)))
+        sens = PT.rel_l2(rg2, rg)
+        ctx = api.context_for(cfg, lim_eps=eps)
+        sg = api.State(gas, part, cfg.a0)
+        ctx.dh_run(sg, a_s[1:], dt_s, 10)
+        e_fwd = max(PT.field_err(sg.gas.cpu().numpy(), gf).values())
+        cg = torch_.zeros_like(sg.gas)
+        if target is None:
+            rho = sg.gas[0].double()
+            cg[0] = (rho / rho.norm()).float()
+        else:
+            cg[0] = 2.0 * (sg.gas[0] - _gpu(torch_, target))
+        ct = api.Cot(cg, torch_.zeros_like(sg.part))
+        ctx.dh_run_vjp(ct, ct)
+        got = ct.gas.cpu().numpy()
+        ctx.close()
+        err, err_t = PT.rel_l2(got, rg), PT.rel_l2_trimmed(got, rg, frac=1e-2)
+        rows.append((eps, sens, err, err_t, e_fwd))
+        print(f"config{which} lim_eps {eps:.0e}: oracle moves itself {sens:.2e}; GPU vs oracle {err:.2e} "
+              f"(all but the worst 1 %: {err_t:.2e}); forward {e_fwd:.1e}")
+        assert np.all(np.isfinite(got))
+    # an experiment, so loose assertions: the GPU stays within a few times what the oracle does to itself at every epsilon
+    # (one perturbed copy is a noisy estimate of that), and the looseness follows the gate -- it shrinks once epsilon
+    # dominates the limiter's arguments (the scheme is first order by then)
+    for eps, sens, err, err_t, e_fwd in rows:
+        assert err < 5.0 * max(1e-3, sens), rows
+    assert rows[-1][1] < rows[0][1] / 2.0 and rows[-1][2] < rows[0][2] / 2.0, rows

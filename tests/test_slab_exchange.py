@@ -1,0 +1,130 @@
+"""The exchange layer of the slab decomposition (paper_2502_02294_b200/slab.py)
+on CPU with the gloo backend, world_size 2 (and 1): halos, their transpose, particle migration, the all-to-all transposes
+and the Poisson solve across slabs, each against the single-rank result (the oracle where it has the routine)."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _cic_local(part, N, z_lo, nz_pad):
+    """Plain cloud-in-cell deposit of unit masses into planes [z_lo, z_lo + nz_pad) (unwrapped z index): the per-rank
+    stand-in for the library's deposit kernel on a padded slab."""
+    mesh = np.zeros((nz_pad, N, N))
+    s = part[:3] - 0.5
+    i0 = np.floor(s).astype(np.int64)
+    f = s - i0
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                w = (f[2] if dz else 1 - f[2]) * (f[1] if dy else 1 - f[1]) * (f[0] if dx else 1 - f[0])
+                np.add.at(mesh, (i0[2] + dz - z_lo, (i0[1] + dy) % N, (i0[0] + dx) % N), w)
+    return mesh
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2502_02294_b200 import slab as S
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        N = 16
+        sl = S.Slab(N)
+        nz, z0 = sl.nz, sl.z0
+        rng = np.random.default_rng(5)                               # the same global data on every rank
+        F = rng.standard_normal((5, N, N, N))
+        res = {}
+        # ---- halo exchange against numpy.roll of the global array
+        h = 3
+        got = sl.halo_exchange(torch.from_numpy(F[:, z0:z0 + nz].copy()), h).numpy()
+        idx = np.arange(z0 - h, z0 + nz + h) % N
+        res["halo_exchange"] = float(np.max(np.abs(got - F[:, idx])))
+        # ---- halo_reduce is its transpose: <exchange(f), g> summed over ranks = <f, reduce(g)> summed over ranks
+        G = np.random.default_rng(100 + rank).standard_normal((5, nz + 2 * h, N, N))
+        lhs = torch.tensor([float(np.sum(got * G))], dtype=torch.float64)
+        red = sl.halo_reduce(torch.from_numpy(G.copy()), h).numpy()
+        rhs = torch.tensor([float(np.sum(F[:, z0:z0 + nz] * red))], dtype=torch.float64)
+        dist.all_reduce(lhs); dist.all_reduce(rhs)
+        res["transpose_identity"] = abs(float(lhs - rhs)) / abs(float(lhs))
+        # ---- particle migration: every particle ends on the owner of its z, none lost, none duplicated
+        n = 4000
+        P_all = np.concatenate([rng.uniform(0, N, (3, n)), rng.standard_normal((3, n))])
+        mine0 = P_all[:, rank::world]                                # an arbitrary initial distribution
+        mine = sl.migrate(torch.from_numpy(mine0.copy())).numpy()
+        res["migrate_owner"] = bool(np.all((mine[2] >= z0) & (mine[2] < z0 + nz)))
+        cnt = torch.tensor([mine.shape[1]], dtype=torch.int64)
+        dist.all_reduce(cnt)
+        res["migrate_count"] = int(cnt) == n
+        want = P_all[:, (P_all[2] >= z0) & (P_all[2] < z0 + nz)]
+        key = lambda a: a[:, np.lexsort(a[::-1])]
+        res["migrate_content"] = float(np.max(np.abs(key(mine) - key(want))))
+        # ---- deposit into a slab padded by one plane + halo_reduce = the global deposit (oracle routine)
+        from oracle import oracle as O
+        dep = _cic_local(mine, N, z0 - 1, nz + 2)
+        dep = sl.halo_reduce(torch.from_numpy(dep), 1).numpy()
+        ref = O.deposit(N, P_all[:3], 1.0)
+        res["deposit"] = float(np.max(np.abs(dep - ref[z0:z0 + nz])))
+        # ---- transposes: z slab <-> x slab and back
+        A = rng.standard_normal((N, N, 4 * world))
+        t = sl.transpose_z_to_x(torch.from_numpy(A[z0:z0 + nz].copy()))
+        m = 4
+        res["transpose_zx"] = float(np.max(np.abs(t.numpy() - A[:, :, rank * m:(rank + 1) * m])))
+        back = sl.transpose_x_to_z(t)
+        res["transpose_roundtrip"] = float(np.max(np.abs(back.numpy() - A[z0:z0 + nz])))
+        # ---- the Poisson solve across slabs against the oracle's
+        delta = rng.standard_normal((N, N, N)); delta -= delta.mean()
+        sent0 = sl.bytes_sent
+        g = sl.poisson_slab(torch.from_numpy(delta[z0:z0 + nz].copy()), 150.0, 20.0).numpy()
+        gref = O.poisson(N, 20.0, 150.0, delta)
+        res["poisson"] = float(np.max(np.abs(g - gref[:, z0:z0 + nz])) / np.max(np.abs(gref)))
+        # fp64 payloads in this test = 2 x the fp32 bytes of the model
+        res["poisson_bytes"] = (sl.bytes_sent - sent0, 2 * S.comm_bytes_per_step(N, world)["poisson_all_to_all"])
+        q.put((rank, res))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [1, 2])
+def test_slab_exchange_reassembles_the_single_rank_results(world):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    out = sorted((q.get(timeout=180) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, r in out:
+        assert r["halo_exchange"] == 0.0, r
+        assert r["transpose_identity"] < 1e-13, r
+        assert r["migrate_owner"] and r["migrate_count"] and r["migrate_content"] == 0.0, r
+        assert r["deposit"] < 1e-12, r
+        assert r["transpose_zx"] == 0.0 and r["transpose_roundtrip"] == 0.0, r
+        assert r["poisson"] < 1e-12, r
+        assert r["poisson_bytes"][0] == pytest.approx(r["poisson_bytes"][1], rel=1e-12), r
+
+
+def test_comm_model_against_nvlink():
+    """The figures DESIGN.md quotes: config 3 on 8 ranks moves 11.5 MB of halos and 31 MB of transposes per rank and forward step."""
+    sys.path.insert(0, ROOT)
+    from paper_2502_02294_b200 import slab as S
+    d = S.comm_bytes_per_step(256, 8)
+    assert d["poisson_all_to_all"] == pytest.approx(4 * 2 * 4 * 256 * 256 * 32 * (7 / 8) * (136 / 256))
+    assert d["z_sweep_halo"] == 2 * 3 * 6 * 4 * 256 * 256
+    assert d["total"] == pytest.approx(sum(v for k, v in d.items() if k != "total"))
