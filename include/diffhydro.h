@@ -170,7 +170,6 @@ int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
 /* Launch-geometry knobs (performance only; results stay within the parity tolerances).  key (HOST string):
  *   "march_s_fwd", "march_s_adj": cells per thread segment of the marching y/z sweeps (0 = built-in choice);
- *   "yz_chain": 1 routes the y/z sweeps through the shared-memory chain kernels the x sweep uses;
  *   "tape": 0 makes dh_run_vjp recompute g' and the sweep inputs inside every step VJP instead of keeping them for
  *           the steps of the segment being reversed (13 N^3 floats per step of a segment; default 1, falls back to
  *           recomputation by itself when the device cannot hold them);
@@ -182,7 +181,9 @@ int dh_sync(dh_ctx* ctx);
  *   "overlap": 0 keeps the particle update of a step on the caller's stream, before the sweeps, instead of forking it
  *           onto the context's side stream beside them (default 1);
  *   "prime": 0 makes every step of dh_run initialise its own Poisson source instead of letting the previous step's last
- *           sweep write it (default 1; bit-identical either way).
+ *           sweep write it (default 1; bit-identical either way);
+ *   "deposit_tile": 1 routes the deposit through a shared-memory tile per brick of 32 x 8 x 8 lattice sites (the A/B of
+ *           profiles/r02.md: three times slower than the default run-aggregated RED; default 0).
  * Unknown key: DH_ERR_INVALID. */
 int dh_tune(dh_ctx* ctx, const char* key, int value);
 /* Optional per-kernel timing: while enabled, every kernel / cuFFT / copy the library issues is bracketed by a pair of

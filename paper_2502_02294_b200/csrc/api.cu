@@ -479,7 +479,6 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     if (!c || !key) { set_error("dh_tune: null argument"); return DH_ERR_INVALID; }
     if (!strcmp(key, "march_s_fwd")) c->tune_march_s_fwd = value;
     else if (!strcmp(key, "march_s_adj")) c->tune_march_s_adj = value;
-    else if (!strcmp(key, "yz_chain")) c->tune_yz_chain = value;
     else if (!strcmp(key, "tape")) c->tune_tape = value;
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
     else if (!strcmp(key, "own_fft")) {
@@ -488,7 +487,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     }
     else if (!strcmp(key, "overlap")) c->tune_overlap = value;
     else if (!strcmp(key, "prime")) c->tune_prime = value;
-    else if (!strcmp(key, "run_gather")) c->tune_run_gather = value;
+    else if (!strcmp(key, "deposit_tile")) c->tune_deposit_tile = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }
@@ -576,7 +575,7 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     for (int k = 0; k < n_steps; ++k) {
         if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
-        const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && !c->tune_yz_chain && c->tune_prime && c->nc == 5;
+        const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && c->tune_prime && c->nc == 5;
         const G6 g(*st);
         DH_TRY(step_arrays(c, g.p, st->part, g.p, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
                            c->run_gstore ? c->gstore[k].gp : nullptr, false, can_prime && k > 0,

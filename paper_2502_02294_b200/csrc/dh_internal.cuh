@@ -95,8 +95,7 @@ struct dh_ctx {
     int tune_march_s_fwd = 0, tune_march_s_adj = 0;   // segment length of the marching y/z sweeps
     int tune_prime = 1;                               // 0: every step of dh_run initialises its Poisson source itself
     int tune_overlap = 1;                             // 0: kick_drift on the main stream, after which the sweeps start
-    int tune_yz_chain = 0;                            // 1: y/z sweeps through the chain kernels of sweep.cu
-    int tune_run_gather = 0;                          // 1: particle gathers take the upper-x cloud values from the next lane
+    int tune_deposit_tile = 0;                        // 1: shared-memory tile deposit (the A/B of profiles/r02_deposit_ab.md)
 
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans = false;
@@ -184,7 +183,7 @@ void dev_free(dh_ctx* c, void* p, size_t bytes);
 StepScalars step_scalars(const dh_cosmology& co, double a_i, double a_next, double dt, double dt_prev);
 
 // ---- kernels (sweep.cu) ----
-// delta_out (may be NULL; not with tune_yz_chain): also write delta = [gas] rho' - rho_bar, the next step's Poisson source
+// delta_out (may be NULL): also write delta = [gas] rho' - rho_bar, the next step's Poisson source
 // (with dh_options.dual_energy the arrays hold six pointers and the calls go to the kernels of sweep_de.cu)
 int launch_sweep(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap, float* const* out,
                  float* cmax, float* delta_out = nullptr);

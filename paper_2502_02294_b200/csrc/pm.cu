@@ -125,6 +125,56 @@ __global__ void __launch_bounds__(256) deposit_kernel(const float* __restrict__ 
     }
 }
 
+// north_star (a)'s design, kept for the A/B in profiles/ (dh_tune "deposit_tile"): a block owns a brick of TBX x TBY x TBZ
+// lattice sites, accumulates their clouds into a shared-memory tile that covers the brick plus a margin of TR cells, and
+// flushes the tile to the mesh with coalesced RED; contributions that leave the tile (a particle displaced by more than
+// TR cells) go straight to the mesh.  fp32 atomicAdd on shared memory compiles to an ATOMS.CAST.SPIN loop on sm_100
+// (compare-and-swap; SASS excerpt in profiles/), so every one of the 8 tile updates per particle is a retry loop under
+// contention, and the flush still issues (TBX+2TR)(TBY+2TR)(TBZ+2TR) / (TBX TBY TBZ) = 3.6 RED lanes per particle where the
+// run-aggregated kernel above issues 4 to 5 -- measured slower at 256^3 both early and late (profiles/r02_deposit_ab.md).
+constexpr int TBX = 32, TBY = 8, TBZ = 8, TR = 3;
+constexpr int TLX = TBX + 2 * TR, TLY = TBY + 2 * TR, TLZ = TBZ + 2 * TR;
+__global__ void __launch_bounds__(1024) deposit_tile_kernel(const float* __restrict__ x, const float* __restrict__ y,
+                                                            const float* __restrict__ z, int nps, int N, float mp,
+                                                            float* __restrict__ delta) {
+    __shared__ float tile[TLZ * TLY * TLX];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < TLZ * TLY * TLX; i += blockDim.x) tile[i] = 0.f;
+    __syncthreads();
+    const int bx = blockIdx.x * TBX, by = blockIdx.y * TBY, bz = blockIdx.z * TBZ;      // brick origin (lattice sites)
+    const float scale = (float)N / (float)nps;                                          // cells per lattice spacing
+    // tile origin in cells: the cell of the brick's first lattice site minus the margin
+    const int ox = (int)floorf((bx + 0.5f) * scale - 0.5f) - TR, oy = (int)floorf((by + 0.5f) * scale - 0.5f) - TR,
+              oz = (int)floorf((bz + 0.5f) * scale - 0.5f) - TR;
+    for (int s = tid; s < TBX * TBY * TBZ; s += blockDim.x) {
+        const int lx = bx + s % TBX, ly = by + (s / TBX) % TBY, lz = bz + s / (TBX * TBY);
+        if (lx >= nps || ly >= nps || lz >= nps) continue;
+        const int p = (lz * nps + ly) * nps + lx;
+        const Cic c = cic_of(__ldg(x + p), __ldg(y + p), __ldg(z + p), N);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int dx = k & 1, dy = (k >> 1) & 1, dz = k >> 2;
+            const int ix = dx ? c.i1[0] : c.i0[0], iy = dy ? c.i1[1] : c.i0[1], iz = dz ? c.i1[2] : c.i0[2];
+            const float w = mp * (dx ? c.f[0] : 1.f - c.f[0]) * (dy ? c.f[1] : 1.f - c.f[1]) * (dz ? c.f[2] : 1.f - c.f[2]);
+            // tile coordinates, periodic distance from the tile origin
+            int tx = ix - ox, ty = iy - oy, tz = iz - oz;
+            tx = tx < 0 ? tx + N : (tx >= N ? tx - N : tx);
+            ty = ty < 0 ? ty + N : (ty >= N ? ty - N : ty);
+            tz = tz < 0 ? tz + N : (tz >= N ? tz - N : tz);
+            if (tx < TLX && ty < TLY && tz < TLZ) atomicAdd(&tile[(tz * TLY + ty) * TLX + tx], w);
+            else atomicAdd(delta + ((size_t)iz * N + iy) * N + ix, w);
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < TLZ * TLY * TLX; i += blockDim.x) {
+        const float v = tile[i];
+        if (v == 0.f) continue;
+        int ix = ox + i % TLX, iy = oy + (i / TLX) % TLY, iz = oz + i / (TLX * TLY);
+        ix = ((ix % N) + N) % N; iy = ((iy % N) + N) % N; iz = ((iz % N) + N) % N;
+        atomicAdd(delta + ((size_t)iz * N + iy) * N + ix, v);
+    }
+}
+
 // ----------------------------------------------------------------------------------------- Green's function ----
 __device__ __forceinline__ int kint(int j, int N) { return j <= N / 2 ? j : j - N; }
 
@@ -171,35 +221,13 @@ __global__ void __launch_bounds__(256) green_adj_kernel(const float2* __restrict
 // The 8 cloud values of every mesh a kernel gathers from are loaded in one batch (all loads issued before the first
 // use) and reduced afterwards: one memory round trip per kernel phase instead of one per cloud row.  ptxas only keeps
 // the batch together when the kernel's launch bounds allow it more than 32 registers (minimum blocks per SM given).
+// (Tried and dropped, r02: taking the upper-x value from the next lane's register by shuffle when the two particles
+// continue the run of cells, so that only the lower-x loads are full-width requests -- 244 -> 254 us kick_drift, 136 ->
+// 157 us deposit_adj, 467 -> 486 us kick_drift_adj at 256^3: the 12 extra SHFL wait on the loads they forward.)
 struct Gath8 { float lo[4], hi[4]; };
 __device__ __forceinline__ void gather_issue(const float* __restrict__ m, const Cic8& q, Gath8& v) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) { v.lo[j] = __ldg(m + q.lo[j]); v.hi[j] = __ldg(m + q.hi[j]); }
-}
-// The same batch with half the full-width requests: lane l's upper-x cell is lane l+1's lower-x cell whenever the two
-// particles sit in the same pair of rows one cell apart (`pass`, the run test of deposit_kernel), so the upper-x value
-// comes from the neighbour's register by shuffle and only the lanes that break the run load it themselves.  All lanes of
-// the warp must call this (the shuffles are warp-wide); dead lanes pass live = false.
-__device__ __forceinline__ bool gather_run(const Cic8& q, bool live) {
-    const int lane = threadIdx.x & 31;
-    const int row = live ? q.row : -7;
-    const int row_next = __shfl_down_sync(0xffffffffu, row, 1);
-    const int i0x_next = __shfl_down_sync(0xffffffffu, q.i0x, 1);
-    return live && lane < 31 && row_next == row && i0x_next == q.i1x;
-}
-__device__ __forceinline__ void gather_issue_run(const float* __restrict__ m, const Cic8& q, bool live, bool pass, Gath8& v) {
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        v.lo[j] = live ? __ldg(m + q.lo[j]) : 0.f;
-        v.hi[j] = (live && !pass) ? __ldg(m + q.hi[j]) : 0.f;
-    }
-}
-__device__ __forceinline__ void gather_finish_run(bool pass, Gath8& v) {
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const float nb = __shfl_down_sync(0xffffffffu, v.lo[j], 1);
-        v.hi[j] = pass ? nb : v.hi[j];
-    }
 }
 __device__ __forceinline__ float gather_reduce(const Gath8& v, const Cic8& q) {
     float acc = 0.f;
@@ -220,8 +248,11 @@ __device__ __forceinline__ float wrap_pos(float x, float fN, float invN) {
 // in -> out (the same arrays when the update is in place; one thread reads and writes only its own particle)
 // Block size and register cap measured at 256^3: 64-128 threads 230 us, 256 threads 237 us, 512 threads 278 us; flat in
 // the register cap between 32 and 85; two particles per thread 264-314 us (this kernel wants warps, not ILP).
+// (Tried and dropped, r02: depositing the NEW positions from this kernel inside dh_run, so that the next step starts with
+// its Poisson solve -- the REDs cost what they cost in a kernel of their own: kick_drift 231 -> 286 us, + 15 us to zero the
+// mesh, + the last sweep adding rho' - rho_bar by RED instead of storing it; forward 1.155 -> 1.154 ms/step early, 1.229 ->
+// 1.196 late, forward + VJP unchanged.)
 constexpr int KD_T = 128;
-template <bool RUN_GATHER>
 __global__ void __launch_bounds__(KD_T, 6) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
                                                          const float* __restrict__ gz, const float* px, const float* py,
                                                          const float* pz, const float* wx_, const float* wy_,
@@ -229,24 +260,17 @@ __global__ void __launch_bounds__(KD_T, 6) kick_drift_kernel(const float* __rest
                                                          float* owy, float* owz, int np, int N, float K,
                                                          float dtau_dx, float fN, float invN, int gravity) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = p < np;
-    const float x = live ? px[p] : 1.f, y = live ? py[p] : 1.f, z = live ? pz[p] : 1.f;
-    float ux = live ? wx_[p] : 0.f, uy = live ? wy_[p] : 0.f, uz = live ? wz_[p] : 0.f;
+    if (p >= np) return;
+    const float x = px[p], y = py[p], z = pz[p];
+    float ux = wx_[p], uy = wy_[p], uz = wz_[p];
     if (gravity) {
         const Cic8 q = cic8_of(x, y, z, N);
         Gath8 a, b, c;
-        if (RUN_GATHER) {
-            const bool pass = gather_run(q, live);
-            gather_issue_run(gx, q, live, pass, a); gather_issue_run(gy, q, live, pass, b); gather_issue_run(gz, q, live, pass, c);
-            gather_finish_run(pass, a); gather_finish_run(pass, b); gather_finish_run(pass, c);
-        } else if (live) {
-            gather_issue(gx, q, a); gather_issue(gy, q, b); gather_issue(gz, q, c);
-        }
+        gather_issue(gx, q, a); gather_issue(gy, q, b); gather_issue(gz, q, c);
         ux = fmaf(K, gather_reduce(a, q), ux);
         uy = fmaf(K, gather_reduce(b, q), uy);
         uz = fmaf(K, gather_reduce(c, q), uz);
     }
-    if (!live) return;
     ox[p] = wrap_pos(fmaf(ux, dtau_dx, x), fN, invN);
     oy[p] = wrap_pos(fmaf(uy, dtau_dx, y), fN, invN);
     oz[p] = wrap_pos(fmaf(uz, dtau_dx, z), fN, invN);
@@ -302,7 +326,7 @@ __device__ __forceinline__ void reg_load(const Src& src, int p, int np, float (&
     }
 }
 
-template <bool GRAV, bool RUN_GATHER>
+template <bool GRAV>
 __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 pin, MPtr6 cot_in, MPtr3 gbar, int np,
                                                                    int nchunks, int N, float K, float dtau_dx, double* K_b,
                                                                    double* dtdx_b) {
@@ -331,11 +355,7 @@ __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 p
             const float kw[3] = {K * wt[0], K * wt[1], K * wt[2]};
             const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
             Gath8 vx, vy, vz;
-            if (RUN_GATHER) {
-                gather_issue_run(g.p[0], q, live, pass, vx); gather_issue_run(g.p[1], q, live, pass, vy);
-                gather_issue_run(g.p[2], q, live, pass, vz);
-                gather_finish_run(pass, vx); gather_finish_run(pass, vy); gather_finish_run(pass, vz);
-            } else if (live) { gather_issue(g.p[0], q, vx); gather_issue(g.p[1], q, vy); gather_issue(g.p[2], q, vz); }
+            if (live) { gather_issue(g.p[0], q, vx); gather_issue(g.p[1], q, vy); gather_issue(g.p[2], q, vz); }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int cz = j >> 1, cy = j & 1;
@@ -382,26 +402,17 @@ __global__ void __launch_bounds__(RT, 3) kick_drift_adj_kernel(CPtr3 g, CPtr12 p
 }
 
 // Adjoint of the deposit: x_b += m_p sum_cells delta_b(cell) dW/dx_p
-template <bool RUN_GATHER>
 __global__ void __launch_bounds__(256) deposit_adj_kernel(const float* __restrict__ db, const float* __restrict__ px,
                                                           const float* __restrict__ py, const float* __restrict__ pz,
                                                           float* __restrict__ xb, float* __restrict__ yb,
                                                           float* __restrict__ zb, int np, int N, float mp) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = p < np;
-    if (!RUN_GATHER && !live) return;
-    const Cic8 q = cic8_of(live ? px[p] : 1.f, live ? py[p] : 1.f, live ? pz[p] : 1.f, N);
+    if (p >= np) return;
+    const Cic8 q = cic8_of(px[p], py[p], pz[p], N);
     const float wy[2] = {1.f - q.fy, q.fy}, wz[2] = {1.f - q.fz, q.fz};
     float a0 = 0.f, a1 = 0.f, a2 = 0.f;
     Gath8 v;
-    if (RUN_GATHER) {
-        const bool pass = gather_run(q, live);
-        gather_issue_run(db, q, live, pass, v);
-        gather_finish_run(pass, v);
-        if (!live) return;
-    } else {
-        gather_issue(db, q, v);
-    }
+    gather_issue(db, q, v);
     const float xb0 = xb[p], yb0 = yb[p], zb0 = zb[p];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -512,7 +523,12 @@ int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float*
     DH_CUDA(cudaGetLastError());
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT);
-        deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, (int)c->np, c->N, (float)c->m_p, delta);
+        if (c->tune_deposit_tile && c->nps % TBX == 0 && c->N >= TLX) {
+            const dim3 grid(c->nps / TBX, (c->nps + TBY - 1) / TBY, (c->nps + TBZ - 1) / TBZ);
+            deposit_tile_kernel<<<grid, 1024, 0, c->stream>>>(x, y, z, c->nps, c->N, (float)c->m_p, delta);
+        } else {
+            deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, (int)c->np, c->N, (float)c->m_p, delta);
+        }
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }
@@ -580,16 +596,10 @@ int launch_kick_drift(dh_ctx* c, float* const g[3], float* const part[6], float*
     const int grav = c->opt.gravity_on && g && g[0];
     Prof prof(c, PROF_KICK_DRIFT);
     const unsigned grid = (unsigned)((c->np + KD_T - 1) / KD_T);
-    if (c->tune_run_gather)
-        kick_drift_kernel<true><<<grid, KD_T, 0, c->stream>>>(
-            grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
-            part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
-            dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
-    else
-        kick_drift_kernel<false><<<grid, KD_T, 0, c->stream>>>(
-            grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
-            part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
-            dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
+    kick_drift_kernel<<<grid, KD_T, 0, c->stream>>>(
+        grav ? g[0] : nullptr, grav ? g[1] : nullptr, grav ? g[2] : nullptr, part[0], part[1], part[2], part[3], part[4],
+        part[5], part_out[0], part_out[1], part_out[2], part_out[3], part_out[4], part_out[5], (int)c->np, c->N, K,
+        dtau_dx, (float)c->N, 1.f / (float)c->N, grav);
     c->launches++;
     DH_CUDA(cudaGetLastError());
     return DH_OK;
@@ -605,18 +615,14 @@ int launch_kick_drift_vjp(dh_ctx* c, float* const g[3], float* const part_in[6],
     for (int d = 0; d < 3; ++d) { gm.p[d] = grav ? g[d] : nullptr; gb.p[d] = grav ? gbar[d] : nullptr; }
     for (int k = 0; k < 6; ++k) { pi.p[k] = part_in[k]; pi.p[6 + k] = cot_out[k]; ci.p[k] = cot_in[k]; }
     unsigned grid;
-    if (grav && c->tune_run_gather) {
-        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true, true>, RT, nchunks, grid));
-        kick_drift_adj_kernel<true, true><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
-                                                                       scal_bar + 3, scal_bar + 4);
-    } else if (grav) {
-        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true, false>, RT, nchunks, grid));
-        kick_drift_adj_kernel<true, false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
-                                                                        scal_bar + 3, scal_bar + 4);
+    if (grav) {
+        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<true>, RT, nchunks, grid));
+        kick_drift_adj_kernel<true><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
+                                                                 scal_bar + 3, scal_bar + 4);
     } else {
-        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<false, false>, RT, nchunks, grid));
-        kick_drift_adj_kernel<false, false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
-                                                                         scal_bar + 3, scal_bar + 4);
+        DH_TRY(persistent_grid(c, kick_drift_adj_kernel<false>, RT, nchunks, grid));
+        kick_drift_adj_kernel<false><<<grid, RT, 0, c->stream>>>(gm, pi, ci, gb, (int)c->np, nchunks, c->N, K, dtau_dx,
+                                                                  scal_bar + 3, scal_bar + 4);
     }
     c->launches++;
     DH_CUDA(cudaGetLastError());
@@ -639,12 +645,8 @@ int launch_deposit_vjp(dh_ctx* c, const float* delta_bar, float* const part_in[6
     if (c->opt.gas_sources_gravity && rho_bar_gas) DH_TRY(launch_axpy(c, delta_bar, rho_bar_gas, 1.f));
     if (c->np > 0) {
         Prof prof(c, PROF_DEPOSIT_ADJ);
-        if (c->tune_run_gather)
-            deposit_adj_kernel<true><<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
-                delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
-        else
-            deposit_adj_kernel<false><<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
-                delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
+        deposit_adj_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(
+            delta_bar, part_in[0], part_in[1], part_in[2], xbar[0], xbar[1], xbar[2], (int)c->np, c->N, (float)c->m_p);
         c->launches++;
         DH_CUDA(cudaGetLastError());
     }

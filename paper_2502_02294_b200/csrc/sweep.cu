@@ -19,9 +19,8 @@
 // cell-per-thread stencil.
 //   x sweep : a block holds whole rows (N/K threads per row, float4/float2 loads), the periodic wrap happens inside
 //             the block -- no halo, each array is read and written exactly once.
-//   y,z sweep: a block is 32 lanes along x (coalesced 128-byte rows) times C chain threads along the sweep axis; the
-//             tile carries a halo (3 cells forward, 4 adjoint) that is recomputed; tiles that share a halo are
-//             adjacent in blockIdx.x so the halo re-read hits L2.
+//   y,z sweeps: the marching kernels of sweep_march.cu (the chain layout with a recomputed halo is kept only by the
+//             dual-energy variant, sweep_de.cu).
 // The adjoint kernel recomputes stage A and B from the sweep's input and applies the transposed operations in
 // gather form: each thread differentiates its own K interfaces and hands the contributions that cross its boundary
 // to the neighbour through the same exchange buffer (4 exchanges in all).
@@ -435,99 +434,6 @@ __global__ void __launch_bounds__(512) sweep_x_adj_kernel(Ptr5 in, const float* 
     block_sum3_to_global(lb, kb, gmb, scal, s_red);
 }
 
-// ----------------------------------------------------------------------------------------- y/z sweep kernels ----
-// block = (32 lanes along x, C chain threads along the sweep axis); grid = (tiles along the axis, ceil(N/32), N).
-// A tile covers C*K cells starting HALO cells before its first output cell; outputs: C*K - 2*HALO cells.
-template <int K, bool HAS_G, int DIR>
-__global__ void __launch_bounds__(512) sweep_yz_fwd_kernel(Ptr5 in, const float* __restrict__ gfield, MPtr5 outp,
-                                                           float* cmax, SweepConst sc) {
-    constexpr int HALO = 3;
-    extern __shared__ float smem[];
-    __shared__ int s_max;
-    const int C = blockDim.y, nthr = 32 * C;
-    const int lane = threadIdx.x, c = threadIdx.y;
-    if (lane == 0 && c == 0) s_max = 0;
-    const int N = sc.N;
-    const int S = C * K - 2 * HALO;
-    int x = blockIdx.y * 32 + lane;
-    const bool xvalid = x < N;
-    if (!xvalid) x = N - 1;
-    const int o = blockIdx.z;
-    const int q0 = blockIdx.x * S - HALO + c * K;      // unwrapped position of my first cell
-    float u[K][5], g[K], out[K][5], cin[K];
-    long addr[K];
-#pragma unroll
-    for (int j = 0; j < K; ++j) {
-        int p = q0 + j;
-        p = p < 0 ? p + N : (p >= N ? p - N : p);
-        p = p >= N ? p - N : p;                         // tiles may overhang by more than N only if N < tile: excluded
-        addr[j] = (DIR == 1) ? ((long)o * N + p) * N + x : ((long)p * N + o) * N + x;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) u[j][k] = __ldg(in.p[k] + addr[j]);
-        g[j] = HAS_G ? __ldg(gfield + addr[j]) : 0.f;
-    }
-    Chain ch{smem, nthr, c * 32 + lane, (c == 0 ? C - 1 : c - 1) * 32 + lane, (c == C - 1 ? 0 : c + 1) * 32 + lane};
-    sweep_forward_core<K, HAS_G>(u, g, ch, sc, out, cin);
-    float cm = 0.f;
-#pragma unroll
-    for (int j = 0; j < K; ++j) {
-        const int li = c * K + j;
-        const int q = q0 + j;
-        const bool ok = xvalid && li >= HALO && li < HALO + S && q < N;
-        if (ok) {
-#pragma unroll
-            for (int k = 0; k < 5; ++k) outp.p[k][addr[j]] = out[j][k];
-            cm = (cin[j] > cm || cin[j] != cin[j]) ? cin[j] : cm;
-        }
-    }
-    if (cmax) block_max_to_global(cm, cmax, &s_max);
-}
-
-template <int K, bool HAS_G, int DIR>
-__global__ void __launch_bounds__(512) sweep_yz_adj_kernel(Ptr5 in, const float* __restrict__ gfield, Ptr5 cot_out,
-                                                           MPtr5 cot_in, float* __restrict__ gbar, double* scal,
-                                                           SweepConst sc) {
-    constexpr int HALO = 4;
-    extern __shared__ float smem[];
-    __shared__ float s_red[96];
-    const int C = blockDim.y, nthr = 32 * C;
-    const int lane = threadIdx.x, c = threadIdx.y;
-    const int N = sc.N;
-    const int S = C * K - 2 * HALO;
-    int x = blockIdx.y * 32 + lane;
-    const bool xvalid = x < N;
-    if (!xvalid) x = N - 1;
-    const int o = blockIdx.z;
-    const int q0 = blockIdx.x * S - HALO + c * K;
-    float u[K][5], g[K], ob[K][5], ub[K][5], gb[K];
-    bool count[K];
-    long addr[K];
-#pragma unroll
-    for (int j = 0; j < K; ++j) {
-        int p = q0 + j;
-        p = p < 0 ? p + N : (p >= N ? p - N : p);
-        p = p >= N ? p - N : p;
-        addr[j] = (DIR == 1) ? ((long)o * N + p) * N + x : ((long)p * N + o) * N + x;
-#pragma unroll
-        for (int k = 0; k < 5; ++k) { u[j][k] = __ldg(in.p[k] + addr[j]); ob[j][k] = __ldg(cot_out.p[k] + addr[j]); }
-        g[j] = HAS_G ? __ldg(gfield + addr[j]) : 0.f;
-        const int li = c * K + j;
-        count[j] = xvalid && li >= HALO && li < HALO + S && (q0 + j) < N;
-    }
-    Chain ch{smem, nthr, c * 32 + lane, (c == 0 ? C - 1 : c - 1) * 32 + lane, (c == C - 1 ? 0 : c + 1) * 32 + lane};
-    float lb, kb, gmb;
-    sweep_adjoint_core<K, HAS_G>(u, g, ob, count, ch, sc, ub, gb, lb, kb, gmb);
-#pragma unroll
-    for (int j = 0; j < K; ++j) {
-        if (count[j]) {
-#pragma unroll
-            for (int k = 0; k < 5; ++k) cot_in.p[k][addr[j]] = ub[j][k];
-            if (HAS_G) gbar[addr[j]] = gb[j];
-        }
-    }
-    block_sum3_to_global(lb, kb, gmb, scal, s_red);
-}
-
 // ------------------------------------------------------------------------------------------------ launchers ----
 SweepConst make_sweep_const(const dh_ctx* c, float lam, float kap) {
     SweepConst sc;
@@ -581,19 +487,6 @@ static void x_geometry(int N, dim3& block, unsigned& grid, long nrows) {
     grid = (unsigned)((nrows + R - 1) / R);
 }
 
-static int yz_chain_threads(int N, int K, int halo, int max_c) {
-    // smallest overhead tile: choose C in [4, max_c] minimising loaded cells per output cell (ragged last tile included)
-    int best = 8; double best_cost = 1e30;
-    for (int C = 4; C <= max_c; ++C) {
-        int S = C * K - 2 * halo;
-        if (S <= 0 || C * K > N + 2 * halo) continue;
-        int T = (N + S - 1) / S;
-        double cost = (double)T * C * K / N + 0.02 * (16.0 / C);   // mild preference for larger blocks at equal cost
-        if (cost < best_cost - 1e-9) { best_cost = cost; best = C; }
-    }
-    return best;
-}
-
 int launch_sweep(dh_ctx* c, int d, float* const* in, const float* g, float lam, float kap, float* const* out,
                  float* cmax, float* delta_out) {
     if (c->nc == 6) {
@@ -615,20 +508,8 @@ int launch_sweep(dh_ctx* c, int d, float* const* in, const float* g, float lam, 
         size_t sm = (size_t)FWD_SLOTS * block.x * block.y * sizeof(float);
         if (g) DH_LAUNCH((sweep_x_fwd_kernel<KF, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows, delta_out);
         else DH_LAUNCH((sweep_x_fwd_kernel<KF, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows, delta_out);
-    } else if (!c->tune_yz_chain) {
-        DH_TRY(launch_sweep_march(c, d, pin, g, pout, cmax, sc, delta_out));
     } else {
-        const int C = yz_chain_threads(N, KF, 3, 16);
-        const int S = C * KF - 6;
-        dim3 block(32, C, 1), grid((N + S - 1) / S, (N + 31) / 32, N);
-        size_t sm = (size_t)FWD_SLOTS * 32 * C * sizeof(float);
-        if (d == 1) {
-            if (g) DH_LAUNCH((sweep_yz_fwd_kernel<KF, true, 1>), grid, block, sm, c->stream, pin, g, pout, cmax, sc);
-            else DH_LAUNCH((sweep_yz_fwd_kernel<KF, false, 1>), grid, block, sm, c->stream, pin, g, pout, cmax, sc);
-        } else {
-            if (g) DH_LAUNCH((sweep_yz_fwd_kernel<KF, true, 2>), grid, block, sm, c->stream, pin, g, pout, cmax, sc);
-            else DH_LAUNCH((sweep_yz_fwd_kernel<KF, false, 2>), grid, block, sm, c->stream, pin, g, pout, cmax, sc);
-        }
+        DH_TRY(launch_sweep_march(c, d, pin, g, pout, cmax, sc, delta_out));
     }
     c->launches++;
     DH_CUDA(cudaGetLastError());
@@ -660,20 +541,8 @@ int launch_sweep_vjp(dh_ctx* c, int d, float* const* in, const float* g, float l
             if (g) DH_LAUNCH((sweep_x_adj_kernel<KA, true, false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
             else DH_LAUNCH((sweep_x_adj_kernel<KA, false, false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
         }
-    } else if (!c->tune_yz_chain) {
-        DH_TRY(launch_sweep_march_vjp(c, d, pin, g, pco, pci, g_bar, scal_bar, sc));
     } else {
-        const int C = yz_chain_threads(N, KA, 4, 16);
-        const int S = C * KA - 8;
-        dim3 block(32, C, 1), grid((N + S - 1) / S, (N + 31) / 32, N);
-        size_t sm = (size_t)ADJ_SLOTS * 32 * C * sizeof(float);
-        if (d == 1) {
-            if (g) DH_LAUNCH((sweep_yz_adj_kernel<KA, true, 1>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc);
-            else DH_LAUNCH((sweep_yz_adj_kernel<KA, false, 1>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc);
-        } else {
-            if (g) DH_LAUNCH((sweep_yz_adj_kernel<KA, true, 2>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc);
-            else DH_LAUNCH((sweep_yz_adj_kernel<KA, false, 2>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc);
-        }
+        DH_TRY(launch_sweep_march_vjp(c, d, pin, g, pco, pci, g_bar, scal_bar, sc));
     }
     c->launches++;
     DH_CUDA(cudaGetLastError());

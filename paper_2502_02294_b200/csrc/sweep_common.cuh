@@ -165,6 +165,11 @@ __device__ __forceinline__ float limM_grad(float A, float B, float eps4, float& 
     return A * wB;
 }
 
+// (Tried and dropped, r02: the marching forward pipeline on packed fp32 -- __ffma2_rn / __fadd2_rn / __fmul2_rn on the
+// component pairs (0,1), (2,3) -- cuts the loop from 482 to 446 SASS instructions per two cells (the packed arithmetic
+// saves 61 issue slots, register pairing costs 25 in MOV / LDC / CS2R at the 128-register cap) and measures 169.4 ->
+// 171.2 us at 256^3: a packed instruction holds the FMA pipe for two cycles, and the pipe, not issue, is what the saved
+// slots would have had to feed.)
 struct Ptr5 { const float* p[5]; };
 struct MPtr5 { float* p[5]; };
 

@@ -160,7 +160,9 @@ def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, 
     print(f"config3 segment reverse vs oracle: gas {eg:.2e} (trimmed 1e-2: {et:.2e}), particles {ep:.2e}, "
           f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}; the oracle under one fp32 rounding of its input moves by {sens:.2e} "
           f"(trimmed {sens_t:.2e}), particles {sens_p:.2e}, dgamma {rdp2[0]:.6g}")
-    tol_all, tol_trim = max(2e-2, 2.0 * sens), max(TOL_GRAD, 2.0 * sens_t)
+    # (one perturbed copy of the INPUT is a lower estimate of what rounding at every operation does: B200 measures 1.3e-3
+    # GPU-oracle and 1.8e-3 between two GPU passes on all but the worst 1 % of entries where the oracle moves by 5e-4)
+    tol_all, tol_trim = max(2e-2, 2.0 * sens), max(TOL_GRAD, 4.0 * sens_t)
     assert et < tol_trim and eg < tol_all and ep < max(2e-2, 2.0 * sens_p)
     assert e_self[1] < tol_trim and e_self[0] < tol_all
     tol_dg = max(TOL_GRAD, 3.0 * abs(rdp2[0] / rdp[0] - 1))
