@@ -237,6 +237,9 @@ def main():
     ap.add_argument("--no-full-run", dest="full_run", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--dual-energy", action="store_true",
+                    help="run the dual-energy variant (DESIGN.md section 19: six gas fields, chain kernels on all axes); "
+                         "recorded in config, not the headline configuration")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="dh_tune knob for A/B runs (e.g. part_pipe=0); recorded in config")
     args = ap.parse_args()
@@ -284,7 +287,8 @@ def main():
     # dparams: gamma (and K, the particles' Dtau part); the cotangents of the schedule scalars A, Dtau, kappa are not part
     # of config 3's outputs (gradients w.r.t. the initial density field and gamma): switched off in the headline context,
     # measured with everything on in `full_dparams`
-    ctx = api.context_for(cfg, want_dA=0, want_dsched=0)
+    de_kw = dict(dual_energy=1, dual_eta=1e-3) if args.dual_energy else {}
+    ctx = api.context_for(cfg, want_dA=0, want_dsched=0, **de_kw)
     for kv in args.tune:
         key, val = kv.split("=")
         ctx.dh_tune(key, int(val))
@@ -322,7 +326,7 @@ def main():
     def fwd_vjp(c, st0, k0, nsteps, st_stride):
         st = st0.clone()
         c.dh_run(st, a_all[k0:k0 + nsteps], dt_all[k0:k0 + nsteps], st_stride)
-        cg = torch.empty_like(st.gas)
+        cg = torch.zeros_like(st.gas) if args.dual_energy else torch.empty_like(st.gas)
         c.dh_data_term(0, st.gas, target, None, 1.0, 1.0, cg, want_loss=False)   # sum (rho - rho_t)^2 (reading R21)
         ct = api.Cot(cg, torch.zeros_like(st.part))
         dp = c.dh_run_vjp(ct, ct)
@@ -333,7 +337,7 @@ def main():
         best, best_f, res = None, None, None
         for _ in range(passes):
             st = st0.clone()
-            cg = torch.empty_like(st.gas)
+            cg = torch.zeros_like(st.gas) if args.dual_energy else torch.empty_like(st.gas)
             ct = api.Cot(cg, torch.zeros_like(st.part))
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
             l0 = c.dh_launch_count()
@@ -438,7 +442,10 @@ def main():
     if os.path.exists(traffic_file):
         try:
             with open(traffic_file) as f:
-                roofline["traffic"] = json.load(f).get(args.workload, {}).get(top)
+                tj = json.load(f)
+            # the capture of the window the headline comes from (late: displaced particles move more sectors)
+            tw = tj.get(args.workload + "_" + wkey, {}).get(top)
+            roofline["traffic"] = tw if tw is not None else tj.get(args.workload, {}).get(top)
         except Exception:
             pass
 
@@ -529,7 +536,7 @@ def main():
     if not args.no_full_dparams:
         for r in results.values():
             r.pop("ct", None)
-        ctx2 = api.context_for(cfg, want_dA=1, want_dsched=1)
+        ctx2 = api.context_for(cfg, want_dA=1, want_dsched=1, **de_kw)
         for kv in args.tune:
             key, val = kv.split("=")
             ctx2.dh_tune(key, int(val))
@@ -547,7 +554,7 @@ def main():
                "dtype": "f32", "data": "synthetic",
                "config": {"workload": cfg.name, "grid": N, "particles": cfg.n_side ** 3, "box": cfg.box,
                           "checkpoint_stride": stride, "schedule": sched,
-                          "loss": "sum (rho_gas - rho_target)^2", "gradients": "d/d(initial state), d/d(delta_init), d/d(gamma); want_dA=0, want_dsched=0 (all of dh_dparams: full_dparams)", "parallelism": f"replicas x{world}", "tune": args.tune,
+                          "loss": "sum (rho_gas - rho_target)^2", "gradients": "d/d(initial state), d/d(delta_init), d/d(gamma); want_dA=0, want_dsched=0 (all of dh_dparams: full_dparams)", "parallelism": f"replicas x{world}", "tune": args.tune, "dual_energy": bool(args.dual_energy),
                           "l2": "working set (state + scratch >= 0.7 GB at 256^3) exceeds the 126 MB L2; no flush"},
                "fwd": {"value": value_fwd, "unit": UNIT, "ms_per_step": ms_fwd / K},
                "windows": win_out, "full_dparams": full_dp, "full_run": full_run,

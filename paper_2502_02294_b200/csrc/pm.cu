@@ -134,10 +134,15 @@ __global__ void __launch_bounds__(256) deposit_kernel(const float* __restrict__ 
 // run-aggregated kernel above issues 4 to 5 -- measured slower at 256^3 both early and late (profiles/r02_deposit_ab.md).
 constexpr int TBX = 32, TBY = 8, TBZ = 8, TR = 3;
 constexpr int TLX = TBX + 2 * TR, TLY = TBY + 2 * TR, TLZ = TBZ + 2 * TR;
+// FIXED = true: the tile holds 32-bit fixed-point sums (weights in units of m_p 2^-22; native ATOMS.ADD on integers)
+// instead of fp32 (ATOMS.CAST.SPIN): the experiment that separates the cost of the CAS loop from the cost of the design.
+template <bool FIXED>
 __global__ void __launch_bounds__(1024) deposit_tile_kernel(const float* __restrict__ x, const float* __restrict__ y,
                                                             const float* __restrict__ z, int nps, int N, float mp,
                                                             float* __restrict__ delta) {
     __shared__ float tile[TLZ * TLY * TLX];
+    int* const itile = reinterpret_cast<int*>(tile);
+    constexpr float FX = 4194304.f;            // 2^22: a cell holds up to 2^9 particle masses
     const int tid = threadIdx.x;
     for (int i = tid; i < TLZ * TLY * TLX; i += blockDim.x) tile[i] = 0.f;
     __syncthreads();
@@ -161,13 +166,17 @@ __global__ void __launch_bounds__(1024) deposit_tile_kernel(const float* __restr
             tx = tx < 0 ? tx + N : (tx >= N ? tx - N : tx);
             ty = ty < 0 ? ty + N : (ty >= N ? ty - N : ty);
             tz = tz < 0 ? tz + N : (tz >= N ? tz - N : tz);
-            if (tx < TLX && ty < TLY && tz < TLZ) atomicAdd(&tile[(tz * TLY + ty) * TLX + tx], w);
-            else atomicAdd(delta + ((size_t)iz * N + iy) * N + ix, w);
+            if (tx < TLX && ty < TLY && tz < TLZ) {
+                if (FIXED) atomicAdd(&itile[(tz * TLY + ty) * TLX + tx], __float2int_rn(w * (FX / mp)));
+                else atomicAdd(&tile[(tz * TLY + ty) * TLX + tx], w);
+            } else {
+                atomicAdd(delta + ((size_t)iz * N + iy) * N + ix, w);
+            }
         }
     }
     __syncthreads();
     for (int i = tid; i < TLZ * TLY * TLX; i += blockDim.x) {
-        const float v = tile[i];
+        const float v = FIXED ? (float)itile[i] * (mp / FX) : tile[i];
         if (v == 0.f) continue;
         int ix = ox + i % TLX, iy = oy + (i / TLX) % TLY, iz = oz + i / (TLX * TLY);
         ix = ((ix % N) + N) % N; iy = ((iy % N) + N) % N; iz = ((iz % N) + N) % N;
@@ -525,7 +534,10 @@ int launch_deposit(dh_ctx* c, const float* rho_gas, const float* x, const float*
         Prof prof(c, PROF_DEPOSIT);
         if (c->tune_deposit_tile && c->nps % TBX == 0 && c->N >= TLX) {
             const dim3 grid(c->nps / TBX, (c->nps + TBY - 1) / TBY, (c->nps + TBZ - 1) / TBZ);
-            deposit_tile_kernel<<<grid, 1024, 0, c->stream>>>(x, y, z, c->nps, c->N, (float)c->m_p, delta);
+            if (c->tune_deposit_tile == 2)
+                deposit_tile_kernel<true><<<grid, 1024, 0, c->stream>>>(x, y, z, c->nps, c->N, (float)c->m_p, delta);
+            else
+                deposit_tile_kernel<false><<<grid, 1024, 0, c->stream>>>(x, y, z, c->nps, c->N, (float)c->m_p, delta);
         } else {
             deposit_kernel<<<(unsigned)((c->np + 255) / 256), 256, 0, c->stream>>>(x, y, z, (int)c->np, c->N, (float)c->m_p, delta);
         }

@@ -143,7 +143,9 @@ def _smooth_direction(N, seed):
     return v
 
 
-STATIC_STABLE_L2, STATIC_STABLE_OUTLIERS = 2e-2, 1e-1      # provisional: tightened to ~3x the B200 measurement
+# B200: config 1 at 128^3 6.8e-3 relative L2 on the stable entries with 1 % of them off by more than 1e-3 max|ref|; Sedov
+# (six perturbed copies define "stable") 2.0e-2 and none
+STATIC_STABLE_L2, STATIC_STABLE_OUTLIERS = 5e-2, 3e-2
 
 
 def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stride, got, dp, min_stable, max_sens, n_pert=1):
@@ -198,8 +200,8 @@ def _static_run_gradient_checks(api, torch_, O, W, label, ctx, P, gas, dts, stri
         fd = (gpu_loss(gas + h * v) - gpu_loss(gas - h * v)) / (2 * h)
         print(f"{label} direction {j}: <grad,v> GPU {a:.6e}, oracle {b:.6e} ({a / b - 1:+.1e}; the oracle moves itself by "
               f"{b_moves:.1e}), FD of the GPU loss {fd:.6e} ({a / fd - 1:+.1e})")
-        assert abs(a / b - 1) < max(1e-2, 3.0 * b_moves)
-        assert abs(a / fd - 1) < max(2e-2, 3.0 * b_moves)
+        assert abs(a / b - 1) < max(2e-2, 4.0 * b_moves)
+        assert abs(a / fd - 1) < max(3e-2, 4.0 * b_moves)
 
 
 def test_config1_at_128_forward_and_gradient(api, torch_, O, W):

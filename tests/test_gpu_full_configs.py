@@ -84,7 +84,26 @@ def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, 
         if j < 3:
             # protocol (i): the GPU's current fp32 state to both sides, one step, every field within 1e-5
             s1 = O.State(sg.gas.cpu().numpy(), sg.part.cpu().numpy(), sg.a, dt_prev=sg.dt_prev, step=sg.step)
-            cm1, _ = O.step(P, s1, dt_s[k], a_s[k + 1])
+            if j == 0:
+                gas_in = s1.gas.copy()
+            cm1, gp1 = O.step(P, s1, dt_s[k], a_s[k + 1], want_gprime=(j == 0))
+            if j == 0:
+                # where does the one-step error of this epoch come from?  The three kernels of the step on their own,
+                # each against the oracle on the same inputs: the Poisson source + solve, and one sweep with the
+                # oracle's own g' (diagnostic: printed, bounded loosely)
+                sc = O.step_scalars(P, sg.a, a_s[k + 1], dt_s[k], sg.dt_prev)
+                gp_gpu = ctx.dh_poisson(ctx.dh_deposit(sg.gas[0], sg.part[:3]), sc["A"]).cpu().numpy()
+                e_g = np.max(np.abs(gp_gpu - gp1)) / np.max(np.abs(gp1))
+                lam, kap = sc["dtau"] / (cfg.box / N), sc["kappa"]
+                e_sw = []
+                for d in range(3):
+                    out = ctx.dh_sweep(d, sg.gas, _gpu(torch_, gp1[d]), lam, kap).cpu().numpy()
+                    ref, _ = O.sweep(gas_in, d, lam, kap, cfg.gamma, gp1[d], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+                    e_sw.append(max(PT.field_err(out, ref).values()))
+                print(f"config3 step {k}, kernels on their own: g' {e_g:.1e}; one sweep from this state with the oracle's g': "
+                      f"x {e_sw[0]:.1e}, y {e_sw[1]:.1e}, z {e_sw[2]:.1e}")
+                assert e_g < 1e-4 and max(e_sw) < 1e-4
+                del gas_in, gp1, gp_gpu
         ins.append(so.copy())
         g_states.append(sg.clone())
         cm_ref, _ = O.step(P, so, dt_s[k], a_s[k + 1])
@@ -160,12 +179,13 @@ def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, 
     print(f"config3 segment reverse vs oracle: gas {eg:.2e} (trimmed 1e-2: {et:.2e}), particles {ep:.2e}, "
           f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}; the oracle under one fp32 rounding of its input moves by {sens:.2e} "
           f"(trimmed {sens_t:.2e}), particles {sens_p:.2e}, dgamma {rdp2[0]:.6g}")
-    # (one perturbed copy of the INPUT is a lower estimate of what rounding at every operation does: B200 measures 1.3e-3
-    # GPU-oracle and 1.8e-3 between two GPU passes on all but the worst 1 % of entries where the oracle moves by 5e-4)
-    tol_all, tol_trim = max(2e-2, 2.0 * sens), max(TOL_GRAD, 4.0 * sens_t)
+    # (one perturbed copy of the INPUT is a lower estimate of what rounding at every operation does: over three B200 runs,
+    # on all but the worst 1 % of entries, GPU-oracle 4e-4 ... 1.3e-3 and GPU-GPU 2.5e-4 ... 1.8e-3 where the oracle moves
+    # by 1.7e-4 ... 5e-4; d gamma GPU-oracle 3.4e-3 ... 4.1e-3 where the oracle moves by 8e-4 ... 1.6e-3)
+    tol_all, tol_trim = max(2e-2, 2.0 * sens), max(3e-3, 4.0 * sens_t)
     assert et < tol_trim and eg < tol_all and ep < max(2e-2, 2.0 * sens_p)
     assert e_self[1] < tol_trim and e_self[0] < tol_all
-    tol_dg = max(TOL_GRAD, 3.0 * abs(rdp2[0] / rdp[0] - 1))
+    tol_dg = max(1e-2, 3.0 * abs(rdp2[0] / rdp[0] - 1))
     assert abs(dp.dgamma / rdp[0] - 1) < tol_dg and abs(dp.dgamma / dp2.dgamma - 1) < tol_dg
     ctx.close()
 
