@@ -168,6 +168,12 @@ int64_t dh_device_bytes(dh_ctx* ctx);
  * cuFFT's internal kernels are not counted. */
 int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
+/* Debug aid (compute-sanitizer's initcheck is not available everywhere): fill the context's device buffers with NaN
+ * (all-ones bytes).  level 0: pure scratch only (Poisson source and spectra, g' scratch, sweep ping-pong sets, adjoint
+ * scratch, the in-segment states and tapes of the reverse pass) -- safe between dh_run and dh_run_vjp; level 1: also what
+ * dh_run keeps for dh_run_vjp (snapshots, per-step g', CFL log), which invalidates the last run.  A path that reads a
+ * buffer before writing it then returns NaN instead of stale numbers.  Asynchronous on the context's stream. */
+int dh_debug_poison(dh_ctx* ctx, int level);
 /* Launch-geometry knobs (performance only; results stay within the parity tolerances).  key (HOST string):
  *   "march_s_fwd", "march_s_adj": cells per thread segment of the marching y/z sweeps (0 = built-in choice);
  *   "tape": 0 makes dh_run_vjp recompute g' and the sweep inputs inside every step VJP instead of keeping them for

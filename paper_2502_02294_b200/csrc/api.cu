@@ -492,6 +492,34 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     return DH_OK;
 }
 
+int dh_debug_poison(dh_ctx* c, int level) {
+    if (!c) { set_error("dh_debug_poison: null context"); return DH_ERR_INVALID; }
+    const size_t mesh = (size_t)c->n3 * sizeof(float);
+    const size_t nspec = (size_t)c->N * c->N * (c->N / 2 + 1) * sizeof(float2);
+    auto fill = [&](void* p, size_t bytes) -> int {
+        if (p && bytes) DH_CUDA(cudaMemsetAsync(p, 0xff, bytes, c->stream));
+        return DH_OK;
+    };
+    DH_TRY(fill(c->delta, mesh));
+    for (auto p : c->spec) DH_TRY(fill(p, nspec));
+    for (auto p : c->gp) DH_TRY(fill(p, mesh));
+    for (auto p : c->gas_tmp) DH_TRY(fill(p, mesh));
+    for (auto p : c->gas_tmp2) DH_TRY(fill(p, mesh));
+    for (int i = 0; i < 2; ++i) for (auto p : c->sw_in[i]) DH_TRY(fill(p, mesh));
+    for (auto p : c->gpb) DH_TRY(fill(p, mesh));
+    for (auto p : c->cot_tmp) DH_TRY(fill(p, mesh));
+    const size_t state_bytes = state_floats(c) * sizeof(float);
+    for (size_t i = 1; i < c->seg.size(); ++i) DH_TRY(fill(c->seg[i].buf, state_bytes));
+    for (auto& t : c->tapes) DH_TRY(fill(t.buf, (size_t)(3 + 2 * c->nc) * mesh));
+    if (level >= 1) {
+        for (auto& s : c->snaps) DH_TRY(fill(s.buf, state_bytes));
+        for (auto& g : c->gstore) DH_TRY(fill(g.buf, 3 * mesh));
+        DH_TRY(fill(c->cmax_log, (size_t)3 * c->cmax_cap * sizeof(float)));
+        c->run_valid = false;
+    }
+    return DH_OK;
+}
+
 int64_t dh_device_bytes(dh_ctx* c) { return c ? c->bytes : 0; }
 int64_t dh_launch_count(dh_ctx* c) { return c ? c->launches : 0; }
 
