@@ -10,6 +10,8 @@ import ctypes as C
 import numpy as np
 import pytest
 
+import parity as PT
+
 pytestmark = pytest.mark.gpu
 
 
@@ -61,12 +63,15 @@ def test_poisoned_scratch_changes_nothing(api, torch_, W, IC, case):
         ctx.dh_tune(k, v)
     ref = _run_and_reverse(api, torch_, ctx, gas, part, cfg, a_s, dt_s, 3, poison=False)      # also allocates everything
     got = _run_and_reverse(api, torch_, ctx, gas, part, cfg, a_s, dt_s, 3, poison=True)
-    for a, b in zip(ref[:4], got[:4]):
+    for j, (a, b) in enumerate(zip(ref[:4], got[:4])):
         assert bool(torch_.isfinite(b).all())
         if case == "hydro_only":
             assert torch_.equal(a, b)                             # no atomics anywhere: the same bits
-        elif a.numel():
-            assert float((a - b).abs().max()) <= 2e-3 * float(a.abs().max()) + 1e-30      # atomic order only (R28)
+        elif a.numel() and j < 2:                                 # forward fields: the order of the deposits' atomics only
+            assert float((a - b).abs().max()) <= 2e-5 * float(a.abs().max())
+        elif a.numel():                                           # cotangents: the same, amplified at the switches (R28)
+            an, bn = a.double().cpu().numpy(), b.double().cpu().numpy()
+            assert PT.rel_l2_trimmed(bn, an, frac=1e-2) < 1e-3 and PT.rel_l2(bn, an) < 5e-2
     assert all(np.isfinite(v) for v in got[4].values())
     assert abs(got[4]["dgamma"] - ref[4]["dgamma"]) <= 1e-3 * abs(ref[4]["dgamma"]) + 1e-12
     # the single-step calls and the host-buffer chain after a poisoning of everything
