@@ -40,7 +40,8 @@ class Cosmo(C.Structure):
 class Opt(C.Structure):
     _fields_ = [("n_part_side", C.c_int32), ("gravity_on", C.c_int32), ("hydro_on", C.c_int32),
                 ("gas_sources_gravity", C.c_int32), ("e_floor", C.c_double), ("lim_eps", C.c_double),
-                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32), ("want_dsched", C.c_int32)]
+                ("cuda_stream", C.c_void_p), ("want_dA", C.c_int32), ("want_dsched", C.c_int32),
+                ("dual_energy", C.c_int32), ("dual_eta", C.c_double)]
 
 
 def test_init_rejects_bad_arguments_and_missing_device(lib):
@@ -48,9 +49,12 @@ def test_init_rejects_bad_arguments_and_missing_device(lib):
     lib.dh_last_error.restype = C.c_char_p
     h = C.c_void_p()
     co = Cosmo(100.0, 1.0, 0.16, 0.0, 0)
-    op = Opt(32, 1, 1, 1, 1e-6, 1e-20, None, 1, 1)
+    op = Opt(32, 1, 1, 1, 1e-6, 1e-20, None, 1, 1, 0, 0.0)
     assert lib.dh_init(C.byref(h), 30, C.c_double(10.0), C.c_double(1.4), C.byref(co), C.byref(op)) == -1   # DH_ERR_INVALID
     assert b"multiple of 32" in lib.dh_last_error()
+    bad = Opt(32, 1, 1, 1, 1e-6, 1e-20, None, 1, 1, 1, -1.0)
+    assert lib.dh_init(C.byref(h), 32, C.c_double(10.0), C.c_double(1.4), C.byref(co), C.byref(bad)) == -1
+    assert b"dual_eta" in lib.dh_last_error()
     assert lib.dh_init(C.byref(h), 32, C.c_double(10.0), C.c_double(1.0), C.byref(co), C.byref(op)) == -1
     if not torch.cuda.is_available():
         rc = lib.dh_init(C.byref(h), 32, C.c_double(10.0), C.c_double(1.4), C.byref(co), C.byref(op))
