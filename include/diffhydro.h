@@ -168,6 +168,10 @@ int64_t dh_device_bytes(dh_ctx* ctx);
  * cuFFT's internal kernels are not counted. */
 int64_t dh_launch_count(dh_ctx* ctx);
 int dh_sync(dh_ctx* ctx);
+/* Conserved sums of a state (the per-step diagnostics of a run: they are what the scheme keeps to round-off without
+ * gravity, Eq. 8): out (HOST, 8 doubles) = (sum rho, sum m_x, sum m_y, sum m_z, sum eps, m_p sum w_x, m_p sum w_y,
+ * m_p sum w_z), fp64 accumulation on the device.  Synchronises the stream. */
+int dh_conserved_sums(dh_ctx* ctx, const dh_state* state, double* out);
 /* Debug aid (compute-sanitizer's initcheck is not available everywhere): fill the context's device buffers with NaN
  * (all-ones bytes).  level 0: pure scratch only (Poisson source and spectra, g' scratch, sweep ping-pong sets, adjoint
  * scratch, the in-segment states and tapes of the reverse pass) -- safe between dh_run and dh_run_vjp; level 1: also what

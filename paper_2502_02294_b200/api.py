@@ -30,7 +30,7 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
            "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
-           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors", "dh_sweep_de", "dh_sweep_de_vjp", "dh_debug_poison"]
+           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors", "dh_sweep_de", "dh_sweep_de_vjp", "dh_debug_poison", "dh_conserved_sums"]
 
 
 class DhError(RuntimeError):
@@ -90,6 +90,7 @@ _lib.dh_init.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double,
 _lib.dh_free.argtypes = [C.c_void_p]
 _lib.dh_sync.argtypes = [C.c_void_p]
 _lib.dh_debug_poison.argtypes = [C.c_void_p, C.c_int]
+_lib.dh_conserved_sums.argtypes = [C.c_void_p, C.POINTER(dh_state), _dp]
 _lib.dh_step.argtypes = [C.c_void_p, C.POINTER(dh_state), C.c_double, C.c_double, C.c_void_p]
 _lib.dh_step_vjp.argtypes = [C.c_void_p, C.POINTER(dh_state), C.c_double, C.c_double, C.POINTER(dh_cot),
                              C.POINTER(dh_cot), C.POINTER(dh_dparams)]
@@ -271,6 +272,13 @@ class Context:
         return dparams
 
     # ---- helpers
+    def dh_conserved_sums(self, st: State):
+        """(sum rho, sum m_x, sum m_y, sum m_z, sum eps, m_p sum w_x, m_p sum w_y, m_p sum w_z) as a numpy array (fp64)."""
+        out = np.zeros(8)
+        cs = st.c_struct()
+        _check(_lib.dh_conserved_sums(self._h, C.byref(cs), out.ctypes.data_as(_dp)), "dh_conserved_sums")
+        return out
+
     def dh_debug_poison(self, level=0):
         _check(_lib.dh_debug_poison(self._h, int(level)), "dh_debug_poison")
 

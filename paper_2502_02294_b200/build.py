@@ -31,8 +31,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     for s in SOURCES:
         o = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = ([nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] +
-               os.environ.get("DH_NVCC_EXTRA", "").split() + ["-c", os.path.join(CSRC, s), "-o", o])
+        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(o)
     log = []

@@ -492,6 +492,27 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     return DH_OK;
 }
 
+int dh_conserved_sums(dh_ctx* c, const dh_state* st, double* out) {
+    if (!c || !st || !out) { set_error("dh_conserved_sums: null argument"); return DH_ERR_INVALID; }
+    DH_TRY(check_state(c, st->gas, st->part, st->eint));
+    double* acc = nullptr;
+    DH_TRY(dev_alloc(c, (void**)&acc, 8 * sizeof(double)));
+    int rc = DH_OK;
+    if (cudaMemsetAsync(acc, 0, 8 * sizeof(double), c->stream) != cudaSuccess) rc = DH_ERR_CUDA;
+    const float* g[5] = {st->gas[0], st->gas[1], st->gas[2], st->gas[3], st->gas[4]};
+    if (rc == DH_OK) rc = launch_sum_arrays(c, g, 5, c->n3, acc);
+    if (rc == DH_OK && c->np > 0) {
+        const float* w[3] = {st->part[3], st->part[4], st->part[5]};
+        rc = launch_sum_arrays(c, w, 3, c->np, acc + 5);
+    }
+    if (rc == DH_OK && (cudaMemcpyAsync(out, acc, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                        cudaStreamSynchronize(c->stream) != cudaSuccess)) rc = DH_ERR_CUDA;
+    dev_free(c, acc, 8 * sizeof(double));
+    if (rc != DH_OK) { if (rc == DH_ERR_CUDA) set_error("dh_conserved_sums: CUDA error"); return rc; }
+    for (int d = 0; d < 3; ++d) out[5 + d] *= c->m_p;
+    return DH_OK;
+}
+
 int dh_debug_poison(dh_ctx* c, int level) {
     if (!c) { set_error("dh_debug_poison: null context"); return DH_ERR_INVALID; }
     const size_t mesh = (size_t)c->n3 * sizeof(float);

@@ -214,6 +214,8 @@ int launch_ic_state_vjp(dh_ctx* c, const float* delta, float* const psi[3], cons
 int launch_data_term(dh_ctx* c, int observable, const float* const gas[5], const float* data, const float* noise_var,
                      float scale, float weight, float* const cot[5], double* loss_dev);
 
+int launch_sum_arrays(dh_ctx* c, const float* const* arrays, int na, int64_t n, double* out_dev);
+
 // ---- sub-grid step (subgrid.cu) ----
 int launch_subgrid(dh_ctx* c, float* const gas[5], const float* g0, const float* g1, const dh_subgrid_params& q,
                    float* zout);

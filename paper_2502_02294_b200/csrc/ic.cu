@@ -172,4 +172,40 @@ int launch_data_term(dh_ctx* c, int observable, const float* const gas[5], const
     return DH_OK;
 }
 
+// out[k] += sum_i a_k[i], k < NA: fp64 accumulation per thread, warp and block, one atomic per block and array
+struct SumPtrs { const float* p[8]; };
+__global__ void __launch_bounds__(256) sum_arrays_kernel(SumPtrs a, int na, int64_t n, double* out) {
+    __shared__ double sm[8][8];
+    double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        for (int k = 0; k < na; ++k) acc[k] += (double)__ldg(a.p[k] + i);
+    for (int k = 0; k < na; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) sm[k][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        for (int k = 0; k < na; ++k) {
+            double v = threadIdx.x < (blockDim.x >> 5) ? sm[k][threadIdx.x] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (threadIdx.x == 0) atomicAdd(out + k, v);
+        }
+    }
+}
+
+int launch_sum_arrays(dh_ctx* c, const float* const* arrays, int na, int64_t n, double* out_dev) {
+    if (na <= 0 || n <= 0) return DH_OK;
+    SumPtrs a;
+    for (int k = 0; k < 8; ++k) a.p[k] = k < na ? arrays[k] : nullptr;
+    int64_t blocks = (n + 255) / 256;
+    const int64_t cap = (int64_t)c->sm_count * 8;
+    sum_arrays_kernel<<<(unsigned)(blocks < cap ? blocks : cap), 256, 0, c->stream>>>(a, na, n, out_dev);
+    c->launches++;
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
 }  // namespace dh

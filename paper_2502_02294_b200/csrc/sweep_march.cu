@@ -105,14 +105,8 @@ constexpr int RING = 8;          // stages (power of two)
 constexpr int NTHR = 128;        // threads per block, fixed: ring offsets are immediates
 constexpr int PF_FWD = 3;        // iterations of prefetch, forward
 constexpr int PF_ADJ = 2;
-#ifndef DH_ADJ_BLOCKS
-#define DH_ADJ_BLOCKS 3
-#endif
-#ifndef DH_ADJ_UNROLL
-#define DH_ADJ_UNROLL 2
-#endif
-constexpr int ADJ_UNROLL = DH_ADJ_UNROLL;
-constexpr int ADJ_BLOCKS = DH_ADJ_BLOCKS;        // adjoint: stages i-4 .. i are re-read, i+1 .. i+2 in flight, one spare
+constexpr int ADJ_UNROLL = 2;       // loop unrolling of the adjoint: 1 -> 404 us, 2 -> 366 us at 256^3
+constexpr int ADJ_BLOCKS = 3;        // resident blocks per SM of the adjoint (168 registers)
 
 // block = (BX lanes along x, BY pencils); grid = (N / BX, N / BY, segments along the sweep axis)
 template <int DIR, bool HAS_G, bool EPS>

@@ -100,8 +100,17 @@ def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, 
                     out = ctx.dh_sweep(d, sg.gas, _gpu(torch_, gp1[d]), lam, kap).cpu().numpy()
                     ref, _ = O.sweep(gas_in, d, lam, kap, cfg.gamma, gp1[d], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
                     e_sw.append(max(PT.field_err(out, ref).values()))
+                # the oracle's own statements evaluated in single precision (oracle/dual_energy.py with the selection switched
+                # off IS the single-energy sweep, pinned to the C++ one): what any fp32 evaluation does to this state
+                from oracle import dual_energy as DE
+                g6 = np.concatenate([gas_in.astype(np.float32), np.zeros((1, N, N, N), dtype=np.float32)], axis=0)
+                emu, _ = DE.sweep(g6, 0, lam, kap, cfg.gamma, gp1[0].astype(np.float32), e_floor=cfg.e_floor(),
+                                  lim_eps=cfg.lim_eps, eta=-1e30, dtype=np.float32)
+                ref, _ = O.sweep(gas_in, 0, lam, kap, cfg.gamma, gp1[0], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+                e_emu = max(PT.field_err(emu[:5], ref).values())
+                del g6, emu, ref
                 print(f"config3 step {k}, kernels on their own: g' {e_g:.1e}; one sweep from this state with the oracle's g': "
-                      f"x {e_sw[0]:.1e}, y {e_sw[1]:.1e}, z {e_sw[2]:.1e}")
+                      f"x {e_sw[0]:.1e}, y {e_sw[1]:.1e}, z {e_sw[2]:.1e}; the oracle's statements in numpy fp32, x sweep: {e_emu:.1e}")
                 assert e_g < 1e-4 and max(e_sw) < 1e-4
                 del gas_in, gp1, gp_gpu
         ins.append(so.copy())

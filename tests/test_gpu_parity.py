@@ -862,3 +862,26 @@ def test_errors_are_reported_not_thrown_across_the_abi(api, torch_, W):
         ctx.dh_run_vjp(ct, ct)
     assert ei.value.code == -7                                            # DH_ERR_STATE
     ctx.close()
+
+
+def test_conserved_sums_diagnostic(api, torch_, W, IC):
+    """dh_conserved_sums (fp64 device reduction) against numpy, and what it is for: without gravity the scheme keeps mass,
+    momentum and energy to fp32 round-off over a run (telescoping fluxes, R3 / R17)."""
+    cfg = W.scaled_config(0, 32, n_steps=6, a1=0.03)
+    _, gas, part = IC.coupled_ic(W, cfg)
+    ctx = api.context_for(cfg)
+    st = api.State(gas, part, cfg.a0)
+    s = ctx.dh_conserved_sums(st)
+    m_p = (1.0 - cfg.f_b) * cfg.N ** 3 / part.shape[1]
+    ref = np.concatenate([gas.astype(np.float64).sum(axis=(1, 2, 3)), m_p * part[3:].astype(np.float64).sum(axis=1)])
+    assert np.max(np.abs(s - ref)) <= 1e-12 * np.max(np.abs(ref)) + 1e-9 * np.abs(gas[1:4]).sum()
+    ctx.close()
+    ctx = api.context_for(cfg, gravity_on=0, n_part_side=0)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    st = api.State(gas, np.zeros((6, 0), dtype=np.float32), cfg.a0)
+    s0 = ctx.dh_conserved_sums(st)
+    ctx.dh_run(st, a_s[1:], dt_s, 0)
+    s1 = ctx.dh_conserved_sums(st)
+    scale = np.array([s0[0], np.abs(gas[1:4]).sum(), np.abs(gas[1:4]).sum(), np.abs(gas[1:4]).sum(), s0[4]])
+    assert np.max(np.abs(s1[:5] - s0[:5]) / scale) < 2e-6, (s0, s1)
+    ctx.close()
