@@ -12,6 +12,8 @@ pytestmark = pytest.mark.gpu
 TOL_STEP = 1e-5
 # One step from config 3's state at a = 0.23 (overdensities of 8, Mach ~ 600 gas): B200 measures 4e-6 ... 1.4e-5 in the R25
 # norms, varying from run to run with the order of the deposits' atomics (the same step from the initial state: 1.6e-7).
+# One sweep alone from that state: kernels 2e-6 ... 5e-6, the oracle's own statements in numpy float32 4.4e-6 (printed
+# by the test): the bound below is what fp32 arithmetic does to Mach-100 gas, three sweeps per step.
 TOL_STEP_LATE = 3e-5
 TOL_GRAD = 1e-3
 TOL_RUN = 1e-3
