@@ -295,6 +295,85 @@ def coupled_step(O, P, gas6, part, a_i, a_next, dt, dt_prev, step, eta=1e-3):
     return gas6, part, cm
 
 
+def _cic(pos, N):
+    """Cloud-in-cell indices and weights (reading R13: s = x - 1/2, i0 = floor(s), f = s - i0), per axis."""
+    s_ = pos - 0.5
+    i0 = np.floor(s_).astype(np.int64)
+    f = s_ - i0
+    return i0 % N, (i0 + 1) % N, f
+
+
+def _gather_grad(mesh, pos, N):
+    """d/dx_p of the CIC interpolation of `mesh` at the particles: (3, n_p); the weights' derivatives are -1 | +1."""
+    (i0, i1, f) = _cic(pos, N)
+    out = np.zeros((3, pos.shape[1]))
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                ix = i1[0] if dx else i0[0]; iy = i1[1] if dy else i0[1]; iz = i1[2] if dz else i0[2]
+                wx = f[0] if dx else 1 - f[0]; wy = f[1] if dy else 1 - f[1]; wz = f[2] if dz else 1 - f[2]
+                v = mesh[iz, iy, ix]
+                out[0] += (1.0 if dx else -1.0) * wy * wz * v
+                out[1] += (1.0 if dy else -1.0) * wx * wz * v
+                out[2] += (1.0 if dz else -1.0) * wx * wy * v
+    return out
+
+
+def coupled_step_vjp(O, P, gas6, part, a_i, a_next, dt, dt_prev, step, cot_gas6, cot_part, eta=1e-3):
+    """Transpose of coupled_step at (gas6, part): returns (cot_gas6_in, cot_part_in, d gamma).  Reverse of S4 (the sweeps,
+    last first, each handing back the cotangent of g'_d), S3 (w_t_b = w'_b + (dtau/dx) x'_b; x_b = x'_b + K sum_d w_t_b,d
+    dg_p,d/dx; g'_b += K W w_t_b), S2 (delta_b = sum_d G_d^T g'_b,d) and S1 (rho_b += delta_b; x_b += m_p sum delta_b dW/dx)."""
+    N = P.N
+    sc = O.step_scalars(P, a_i, a_next, dt, dt_prev)
+    dx = P.box / N
+    gas6 = np.asarray(gas6, dtype=np.float64); part = np.asarray(part, dtype=np.float64)
+    npart = part.shape[1]
+    f_b = P.Omega_b / P.Omega_m
+    m_p = (1.0 - f_b) * N ** 3 / npart if npart else 0.0
+    g = None
+    if P.gravity_on:
+        rho_bar = (1.0 - f_b if npart else 0.0) + (f_b if P.gas_sources_gravity else 0.0)
+        delta = (gas6[0] if P.gas_sources_gravity else 0.0) - rho_bar + (O.deposit(N, part[:3], m_p) if npart else 0.0)
+        g = O.poisson(N, P.box, sc["A"], delta)
+    # forward sweeps, keeping every sweep's input
+    lam = sc["dtau"] / dx
+    ins, cur = [], gas6
+    for d in STRANG[step % 6]:
+        ins.append((cur, d))
+        cur, _ = sweep(cur, d, lam, sc["kappa"], P.gamma, None if g is None else g[d], P.e_floor, P.lim_eps, eta)
+    cot = np.asarray(cot_gas6, dtype=np.float64)
+    gb = np.zeros((3, N, N, N))
+    dgamma = 0.0
+    for u_in, d in reversed(ins):
+        cot, gbd, scb = sweep_vjp(u_in, d, lam, sc["kappa"], P.gamma, cot, None if g is None else g[d], P.e_floor, P.lim_eps, eta)
+        dgamma += scb["gamma"]
+        if gbd is not None:
+            gb[d] += gbd
+    cp = np.asarray(cot_part, dtype=np.float64).copy()
+    if npart:
+        wt = cp[3:] + (sc["dtau"] / dx) * cp[:3]
+        xb = cp[:3].copy()
+        if g is not None:
+            for d in range(3):
+                xb += sc["K"] * wt[d] * _gather_grad(g[d], part[:3], N)
+                # vector deposit of K w_t_b with the gather's own weights (adjoint pair of gather / deposit)
+                i0, i1, f = _cic(part[:3], N)
+                for dz in (0, 1):
+                    for dy in (0, 1):
+                        for dxx in (0, 1):
+                            ix = i1[0] if dxx else i0[0]; iy = i1[1] if dy else i0[1]; iz = i1[2] if dz else i0[2]
+                            w_ = (f[0] if dxx else 1 - f[0]) * (f[1] if dy else 1 - f[1]) * (f[2] if dz else 1 - f[2])
+                            np.add.at(gb[d], (iz, iy, ix), sc["K"] * wt[d] * w_)
+        cp = np.concatenate([xb, wt])
+    if g is not None:
+        db = O.poisson_vjp(N, P.box, sc["A"], gb)
+        if P.gas_sources_gravity:
+            cot = cot.copy(); cot[0] += db
+        if npart:
+            cp[:3] += m_p * _gather_grad(db, part[:3], N)
+    return cot, cp, dgamma
+
+
 def coupled_run(O, P, gas6, part, a0, a_sched, dt_sched, eta=1e-3, step0=0):
     a, dtp = a0, 0.0
     cmax = []

@@ -314,3 +314,43 @@ def test_config2_thermal_energy_at_late_time_with_and_without_dual_energy(api, t
     # keeps it to a few per cent, and nothing sits on the floor
     hi = [r for r in rows if r[0] >= 100]
     assert all(r[5] < 1e-2 for r in hi) and np.mean(eG2 <= fl) < 0.01
+
+
+def test_de_coupled_step_vjp_matches_oracle(api, torch_, O, DE, W, IC):
+    """One coupled step with dual energy and its VJP (dh_step_vjp: recomputes g' and the sweep inputs, six-field sweep
+    transposes, particle and Poisson adjoints) against the oracle's composition, from an evolved state with the selection
+    threshold at the median thermal fraction (q carries the pressure in half of the cells)."""
+    cfg = W.scaled_config(0, 32, n_steps=6, a1=0.03)
+    _, gas, part = IC.coupled_ic(W, cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    k = 3
+    g, p, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:k + 1], dt_s[:k])
+    g = g.astype(np.float32); p = p.astype(np.float32)
+    g64 = g.astype(np.float64)
+    eT = g64[4] / g64[0] - 0.5 * np.sum(g64[1:4] ** 2, axis=0) / g64[0] ** 2
+    eta = float(np.median(eT * g64[0] / g64[4]))
+    rng = np.random.default_rng(8)
+    q = (g64[0] * eT * (1.0 + 0.05 * rng.standard_normal(eT.shape))).astype(np.float32)
+    g6 = np.concatenate([g, q[None]], axis=0)
+    cg = rng.standard_normal(g6.shape).astype(np.float32); cp = rng.standard_normal(p.shape).astype(np.float32)
+    ref_g, ref_p, _ = DE.coupled_step(O, P, g6, p, a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1], k, eta=eta)
+    rg, rp, rdg = DE.coupled_step_vjp(O, P, g6, p, a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1], k, cg, cp, eta=eta)
+    ctx = api.context_for(cfg, dual_energy=1, dual_eta=eta)
+    st = api.State(g6, p, a_s[k], dt_s[k - 1], k)
+    ctx.dh_step(st, dt_s[k], a_s[k + 1])
+    e = _err6(st.gas.cpu().numpy(), ref_g)
+    e.update(PT.part_err(st.part.cpu().numpy(), ref_p, cfg.N))
+    co = api.Cot(cg, cp)
+    dp = ctx.dh_step_vjp(api.State(g6, p, a_s[k], dt_s[k - 1], k), dt_s[k], a_s[k + 1], co, co)
+    got_g, got_p = co.gas.cpu().numpy(), co.part.cpu().numpy()
+    e_all, e_trim = PT.rel_l2(got_g, rg), PT.rel_l2_trimmed(got_g, rg, frac=1e-3)
+    print(f"DE coupled step: {e}; VJP gas rel L2 {e_all:.2e} (all but the worst 1e-3: {e_trim:.2e}), particles "
+          f"{PT.rel_l2(got_p, rp):.2e}, dgamma {dp.dgamma:.6g} vs {rdg:.6g}")
+    # forward: cells whose selection flips between fp32 and fp64 jump by the 5 % drift of q; everything else to 1e-5
+    bad = np.mean(np.abs(st.gas.cpu().numpy()[4] - ref_g[4]) > 1e-5 * np.max(np.abs(ref_g[4])))
+    assert bad < 2e-3 and max(e.values()) < 5e-3
+    assert np.all(np.isfinite(got_g)) and np.all(np.isfinite(got_p))
+    assert e_trim < 2e-5 and e_all < 2e-2 and PT.rel_l2(got_p, rp) < 2e-3
+    assert abs(dp.dgamma - rdg) < 2e-3 * max(abs(rdg), 1.0)
+    ctx.close()
