@@ -185,17 +185,21 @@ def test_config3_late_segment_three_steps_ten_steps_and_reverse(api, torch_, O, 
     rg2, rp2, rdp2 = oracle_chain(ins2, sp.gas)
     del ins, ins2
     sens, sens_t, sens_p = PT.rel_l2(rg2, rg), PT.rel_l2_trimmed(rg2, rg, frac=1e-2), PT.rel_l2(rp2, rp)
+    sens_pt = PT.rel_l2_trimmed(rp2, rp, frac=1e-2)
     eg, ep = PT.rel_l2(got_g, rg), PT.rel_l2(got_p, rp)
-    et = PT.rel_l2_trimmed(got_g, rg, frac=1e-2)
-    print(f"config3 segment reverse vs oracle: gas {eg:.2e} (trimmed 1e-2: {et:.2e}), particles {ep:.2e}, "
+    et, ept = PT.rel_l2_trimmed(got_g, rg, frac=1e-2), PT.rel_l2_trimmed(got_p, rp, frac=1e-2)
+    print(f"config3 segment reverse vs oracle: gas {eg:.2e} (trimmed 1e-2: {et:.2e}), particles {ep:.2e} (trimmed {ept:.2e}), "
           f"dgamma {dp.dgamma:.6g} vs {rdp[0]:.6g}; the oracle under one fp32 rounding of its input moves by {sens:.2e} "
-          f"(trimmed {sens_t:.2e}), particles {sens_p:.2e}, dgamma {rdp2[0]:.6g}")
-    # (one perturbed copy of the INPUT is a lower estimate of what rounding at every operation does: over three B200 runs,
-    # on all but the worst 1 % of entries, GPU-oracle 4e-4 ... 1.3e-3 and GPU-GPU 2.5e-4 ... 1.8e-3 where the oracle moves
-    # by 1.7e-4 ... 5e-4; d gamma GPU-oracle 3.4e-3 ... 4.1e-3 where the oracle moves by 8e-4 ... 1.6e-3)
-    tol_all, tol_trim = max(2e-2, 2.0 * sens), max(3e-3, 4.0 * sens_t)
-    assert et < tol_trim and eg < tol_all and ep < max(2e-2, 2.0 * sens_p)
-    assert e_self[1] < tol_trim and e_self[0] < tol_all
+          f"(trimmed {sens_t:.2e}), particles {sens_p:.2e} (trimmed {sens_pt:.2e}), dgamma {rdp2[0]:.6g}")
+    # Over ALL entries the relative L2 is not a statistic that can be bounded at this epoch: five B200 runs gave 1.0 ... 4.4
+    # GPU-oracle, 0.8 ... 4.7 between two GPU passes and 1.0 ... 2.7 for the oracle against its own perturbed copy -- a
+    # handful of entries next to floor-active Mach-600 cells carry it (R28a).  It is printed; what is asserted is
+    # all but the worst 1 % of entries (GPU-oracle 4e-4 ... 1.9e-3, GPU-GPU 2.5e-4 ... 1.8e-3 where the oracle moves by
+    # 1.7e-4 ... 7.8e-4; one perturbed copy of the INPUT is a lower estimate of what rounding at every operation does),
+    # the same for the particles, d gamma (GPU-oracle 1e-3 ... 4.1e-3 where the oracle moves by 5e-4 ... 1.6e-3), finiteness.
+    tol_trim = max(5e-3, 4.0 * sens_t)
+    assert et < tol_trim and e_self[1] < tol_trim
+    assert ept < max(5e-3, 4.0 * sens_pt)
     tol_dg = max(1e-2, 3.0 * abs(rdp2[0] / rdp[0] - 1))
     assert abs(dp.dgamma / rdp[0] - 1) < tol_dg and abs(dp.dgamma / dp2.dgamma - 1) < tol_dg
     ctx.close()
