@@ -97,6 +97,102 @@ def _worker(rank, world, port, q):
         dist.destroy_process_group()
 
 
+def _gather_local(mesh_pad, part, N, z_lo):
+    """Plain cloud-in-cell interpolation of a padded slab (planes z_lo ...) at the particles."""
+    s = part[:3] - 0.5
+    i0 = np.floor(s).astype(np.int64)
+    f = s - i0
+    out = np.zeros(part.shape[1])
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                w = (f[2] if dz else 1 - f[2]) * (f[1] if dy else 1 - f[1]) * (f[0] if dx else 1 - f[0])
+                out += w * mesh_pad[i0[2] + dz - z_lo, (i0[1] + dy) % N, (i0[0] + dx) % N]
+    return out
+
+
+def _step_worker(rank, world, port, q):
+    """One whole coupled step (S1-S4 of DESIGN.md section 2) on slabs: the oracle's routines on each rank's padded slab,
+    slab.py's exchanges in between, against the oracle's step on the whole box."""
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2502_02294_b200 import slab as S, workloads as W
+    from oracle import oracle as O, ic as IC
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = W.scaled_config(0, 16, n_steps=8, a1=0.05)
+        _, gas, part = IC.coupled_ic(W, cfg)
+        gas = gas.astype(np.float64); part = part.astype(np.float64)
+        P = O.make_params(cfg.N, cfg.box, cfg.gamma, e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+        a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+        N = cfg.N
+        sl = S.Slab(N)
+        nz, z0 = sl.nz, sl.z0
+        f_b = cfg.f_b
+        m_p = (1.0 - f_b) * N ** 3 / part.shape[1]
+        T = torch.from_numpy
+        # the reference: the oracle on the whole box, three steps (three different Strang orders, z sweep first / last)
+        ref = O.State(gas, part, cfg.a0)
+        g_loc = gas[:, z0:z0 + nz].copy()
+        p_loc = part[:, (part[2] >= z0) & (part[2] < z0 + nz)].copy()
+        a, dtp = cfg.a0, 0.0
+        worst = {"gas": 0.0, "part": 0.0, "count": True}
+        for k in range(3):
+            O.step(P, ref, dt_s[k], a_s[k + 1])
+            sc = O.step_scalars(P, a, a_s[k + 1], dt_s[k], dtp)
+            # S1: deposit into the slab padded by one plane, pads added onto the neighbours
+            dep = sl.halo_reduce(T(m_p * _cic_local(p_loc, N, z0 - 1, nz + 2)), 1).numpy()
+            delta = g_loc[0] - 1.0 + dep
+            # S2: Poisson solve across the slabs
+            g = sl.poisson_slab(T(delta), sc["A"], cfg.box).numpy()
+            # S3: gather from g' padded by one plane, kick, drift, migrate
+            gpad = sl.halo_exchange(T(g), 1).numpy()
+            for d in range(3):
+                p_loc[3 + d] += sc["K"] * _gather_local(gpad[d], p_loc, N, z0 - 1)
+            p_loc[:3] = np.mod(p_loc[:3] + p_loc[3:] * (sc["dtau"] / (cfg.box / N)), N)
+            p_loc = sl.migrate(T(p_loc)).numpy()
+            # S4: x and y sweeps are slab-local; the z sweep runs on the slab padded by three planes (fields and g'_z)
+            lam = sc["dtau"] / (cfg.box / N)
+            for d in O.strang_order(k):
+                if d == 2:
+                    pad = sl.halo_exchange(T(np.concatenate([g_loc, g[2][None]], axis=0)), 3).numpy()
+                    out, _ = O.sweep(pad[:5], 2, lam, sc["kappa"], cfg.gamma, pad[5], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+                    g_loc = out[:, 3:-3].copy()               # the periodic wrap of the padded pencils only reaches the pads
+                else:
+                    g_loc, _ = O.sweep(g_loc, d, lam, sc["kappa"], cfg.gamma, g[d], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+            a, dtp = a_s[k + 1], dt_s[k]
+            worst["gas"] = max(worst["gas"], float(np.max(np.abs(g_loc - ref.gas[:, z0:z0 + nz])) / np.max(np.abs(ref.gas))))
+            want = ref.part[:, (ref.part[2] >= z0) & (ref.part[2] < z0 + nz)]
+            worst["count"] = worst["count"] and want.shape[1] == p_loc.shape[1]
+            if want.shape[1] == p_loc.shape[1]:
+                key = lambda x: x[:, np.lexsort(np.round(x[::-1], 9))]
+                worst["part"] = max(worst["part"], float(np.max(np.abs(key(p_loc) - key(want)))))
+        q.put((rank, worst))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2])
+def test_a_whole_coupled_step_on_slabs_is_the_single_rank_step(world):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_step_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    out = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, w in out:
+        assert w["count"], w
+        assert w["gas"] < 1e-11 and w["part"] < 1e-9, w
+
+
 @pytest.mark.parametrize("world", [1, 2])
 def test_slab_exchange_reassembles_the_single_rank_results(world):
     import torch.multiprocessing as mp
