@@ -84,23 +84,42 @@ class Slab:
         """Rank that owns position z (grid units, [0, N)): floor(z / nz); the very test `migrate` applies."""
         return torch.clamp(torch.floor(z / self.nz).to(torch.int64), 0, self.P - 1)
 
-    def migrate(self, part: torch.Tensor) -> torch.Tensor:
-        """part (6, n): positions (grid units) and velocities.  Returns the particles this rank owns after the exchange
-        (those that stayed, in their order, followed by the arrivals ordered by source rank).  Counts first, then the
-        payload as one all-to-all with ragged splits."""
+    def migrate(self, part: torch.Tensor, return_route: bool = False):
+        """part (k, n), k >= 3: rows 0-2 are positions (grid units), the rest travels with them (velocities, ids, ...).
+        Returns the particles this rank owns after the exchange, grouped by source rank in rank order.
+        Counts first, then the payload as one all-to-all with ragged splits.  return_route: also the routing record that
+        `migrate_back` needs (the transpose: cotangents return to the rank and the slot their particle came from)."""
+        k, n = part.shape
         owner = self.owner_of(part[2])
         order = torch.argsort(owner, stable=True)
-        send = part[:, order].t().contiguous()                       # (n, 6) grouped by destination
+        send = part[:, order].t().contiguous()                       # (n, k) grouped by destination
         counts = torch.bincount(owner, minlength=self.P)
-        recv_counts = torch.empty_like(counts)
-        if self.P == 1:
-            return send.t().contiguous()
-        dist.all_to_all_single(recv_counts, counts, group=self.group)
-        out = torch.empty((int(recv_counts.sum()), 6), dtype=part.dtype, device=part.device)
-        self.bytes_sent += int(counts.sum() - counts[self.rank]) * 6 * part.element_size()
-        dist.all_to_all_single(out, send, output_split_sizes=recv_counts.tolist(), input_split_sizes=counts.tolist(),
-                               group=self.group)
-        return out.t().contiguous()
+        recv_counts = counts.clone()
+        if self.P > 1:
+            dist.all_to_all_single(recv_counts, counts, group=self.group)
+            out = torch.empty((int(recv_counts.sum()), k), dtype=part.dtype, device=part.device)
+            self.bytes_sent += int(counts.sum() - counts[self.rank]) * k * part.element_size()
+            dist.all_to_all_single(out, send, output_split_sizes=recv_counts.tolist(), input_split_sizes=counts.tolist(),
+                                   group=self.group)
+        else:
+            out = send
+        res = out.t().contiguous()
+        return (res, (order, counts.tolist(), recv_counts.tolist(), n)) if return_route else res
+
+    def migrate_back(self, cot: torch.Tensor, route) -> torch.Tensor:
+        """Transpose of migrate: cot (k, n_after) in the order migrate returned -> (k, n_before) in the order migrate was given."""
+        order, counts, recv_counts, n = route
+        k = cot.shape[0]
+        send = cot.t().contiguous()
+        if self.P > 1:
+            back = torch.empty((n, k), dtype=cot.dtype, device=cot.device)
+            self.bytes_sent += (sum(recv_counts) - recv_counts[self.rank]) * k * cot.element_size()
+            dist.all_to_all_single(back, send, output_split_sizes=counts, input_split_sizes=recv_counts, group=self.group)
+        else:
+            back = send
+        res = torch.empty_like(back)
+        res[order] = back                                             # undo the grouping by destination
+        return res.t().contiguous()
 
     # ------------------------------------------------------------------------------------------- transposes ----
     def transpose_z_to_x(self, a: torch.Tensor) -> torch.Tensor:
@@ -162,6 +181,36 @@ class Slab:
             back = torch.complex(self.transpose_x_to_z(gz.real.contiguous()), self.transpose_x_to_z(gz.imag.contiguous()))
             out.append(torch.fft.irfft2(back[..., :nxh], s=(N, N), dim=(-2, -1)))
         return torch.stack(out)
+
+
+    def poisson_slab_vjp(self, gb: torch.Tensor, A: float, box: float) -> torch.Tensor:
+        """Transpose of poisson_slab: delta_b (nz, N, N) = sum_d G_d^T g_b,d.  G_d = F^-1 (i k~_d A / k^2) F with an odd
+        imaginary symbol, so G_d^T = -G_d: three all-to-alls in, one out (the roles of the layouts swapped)."""
+        N, P = self.N, self.P
+        nxh = N // 2 + 1
+        M = P * math.ceil(nxh / P)
+        m = M // P
+        kf = 2.0 * math.pi / box
+        nfreq = torch.fft.fftfreq(N, d=1.0 / N, device=gb.device, dtype=torch.float64)
+        nz_ = nfreq[:, None, None]
+        ny_ = nfreq[None, :, None]
+        nx_ = (torch.arange(m, device=gb.device, dtype=torch.float64) + self.rank * m)[None, None, :]
+        k2 = kf * kf * (nx_ * nx_ + ny_ * ny_ + nz_ * nz_)
+        inv = torch.where(k2 > 0, 1.0 / torch.where(k2 > 0, k2, torch.ones_like(k2)), torch.zeros_like(k2))
+        live = (nx_ < nxh).to(torch.float64)
+        acc = None
+        for d, n_d in enumerate((nx_, ny_, nz_)):
+            spec = torch.fft.rfft2(gb[d].to(torch.float64), dim=(-2, -1))
+            pad = torch.zeros((self.nz, N, M), dtype=spec.dtype, device=spec.device)
+            pad[..., :nxh] = spec
+            colz = torch.fft.fft(torch.complex(self.transpose_z_to_x(pad.real.contiguous()),
+                                               self.transpose_z_to_x(pad.imag.contiguous())), dim=0)
+            nt = torch.where(n_d.abs() == N // 2, torch.zeros_like(n_d), n_d)
+            term = -(1j * kf * nt * A * inv * live) * colz
+            acc = term if acc is None else acc + term
+        dz = torch.fft.ifft(acc, dim=0)
+        back = torch.complex(self.transpose_x_to_z(dz.real.contiguous()), self.transpose_x_to_z(dz.imag.contiguous()))
+        return torch.fft.irfft2(back[..., :nxh], s=(N, N), dim=(-2, -1))
 
 
 def comm_bytes_per_step(N: int, P: int, n_part_cross: float = 0.0, adjoint: bool = False) -> dict:

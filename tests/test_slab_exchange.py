@@ -17,9 +17,9 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _cic_local(part, N, z_lo, nz_pad):
-    """Plain cloud-in-cell deposit of unit masses into planes [z_lo, z_lo + nz_pad) (unwrapped z index): the per-rank
-    stand-in for the library's deposit kernel on a padded slab."""
+def _cic_local(part, N, z_lo, nz_pad, weights=1.0):
+    """Plain cloud-in-cell deposit of unit masses (or `weights`) into planes [z_lo, z_lo + nz_pad) (unwrapped z index):
+    the per-rank stand-in for the library's deposit kernel on a padded slab."""
     mesh = np.zeros((nz_pad, N, N))
     s = part[:3] - 0.5
     i0 = np.floor(s).astype(np.int64)
@@ -28,7 +28,7 @@ def _cic_local(part, N, z_lo, nz_pad):
         for dy in (0, 1):
             for dx in (0, 1):
                 w = (f[2] if dz else 1 - f[2]) * (f[1] if dy else 1 - f[1]) * (f[0] if dx else 1 - f[0])
-                np.add.at(mesh, (i0[2] + dz - z_lo, (i0[1] + dy) % N, (i0[0] + dx) % N), w)
+                np.add.at(mesh, (i0[2] + dz - z_lo, (i0[1] + dy) % N, (i0[0] + dx) % N), w * weights)
     return mesh
 
 
@@ -173,6 +173,132 @@ def _step_worker(rank, world, port, q):
         q.put((rank, worst))
     finally:
         dist.destroy_process_group()
+
+
+def _gather_grad_local(mesh_pad, part, N, z_lo):
+    """d/dx_p of _gather_local: (3, n)."""
+    s = part[:3] - 0.5
+    i0 = np.floor(s).astype(np.int64)
+    f = s - i0
+    out = np.zeros((3, part.shape[1]))
+    for dz in (0, 1):
+        for dy in (0, 1):
+            for dx in (0, 1):
+                wx = f[0] if dx else 1 - f[0]; wy = f[1] if dy else 1 - f[1]; wz = f[2] if dz else 1 - f[2]
+                v = mesh_pad[i0[2] + dz - z_lo, (i0[1] + dy) % N, (i0[0] + dx) % N]
+                out[0] += (1.0 if dx else -1.0) * wy * wz * v
+                out[1] += (1.0 if dy else -1.0) * wx * wz * v
+                out[2] += (1.0 if dz else -1.0) * wx * wy * v
+    return out
+
+
+def _vjp_worker(rank, world, port, q):
+    """The reverse pass of one coupled step on slabs: the transposes of the forward's exchanges (halo_reduce where the
+    forward exchanges and vice versa, migrate_back, the Poisson transpose across slabs) around the oracle's per-kernel
+    VJPs, against the oracle's step VJP on the whole box."""
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2502_02294_b200 import slab as S, workloads as W
+    from oracle import oracle as O, ic as IC
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = W.scaled_config(0, 16, n_steps=8, a1=0.05)
+        _, gas, part = IC.coupled_ic(W, cfg)
+        P = O.make_params(cfg.N, cfg.box, cfg.gamma, e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+        a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+        N = cfg.N
+        k = 2                                                       # Strang order ZXY: the z sweep comes first
+        gas, part, _, _ = O.run(P, gas, part, cfg.a0, a_s[1:k + 1], dt_s[:k])
+        npart = part.shape[1]
+        sc0 = O.step_scalars(P, a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1])
+        part[5] += 0.6 * (cfg.box / N) / sc0["dtau"]                # a bulk drift of 0.6 cells along z: a plane of particles changes slab
+        rng = np.random.default_rng(3)                              # the same on every rank
+        cot_g = rng.standard_normal(gas.shape); cot_p = rng.standard_normal(part.shape)
+        s_in = O.State(gas, part, a_s[k], dt_prev=dt_s[k - 1], step=k)
+        rg, rp, _ = O.step_vjp(P, s_in, dt_s[k], a_s[k + 1], cot_g, cot_p)
+        sl = S.Slab(N)
+        nz, z0 = sl.nz, sl.z0
+        m_p = (1.0 - cfg.f_b) * N ** 3 / npart
+        T = torch.from_numpy
+        dxc = cfg.box / N
+        sc = O.step_scalars(P, a_s[k], a_s[k + 1], dt_s[k], dt_s[k - 1])
+        lam, kap = sc["dtau"] / dxc, sc["kappa"]
+        mine = (part[2] >= z0) & (part[2] < z0 + nz)
+        ids_in = np.nonzero(mine)[0]
+        p_in = part[:, mine].copy()
+        u0 = gas[:, z0:z0 + nz].copy()
+        # ---- forward on slabs, keeping what the reverse pass needs
+        dep = sl.halo_reduce(T(m_p * _cic_local(p_in, N, z0 - 1, nz + 2)), 1).numpy()
+        g = sl.poisson_slab(T(u0[0] - 1.0 + dep), sc["A"], cfg.box).numpy()
+        gpad = sl.halo_exchange(T(g), 1).numpy()
+        p_mid = p_in.copy()
+        for d in range(3):
+            p_mid[3 + d] += sc["K"] * _gather_local(gpad[d], p_in, N, z0 - 1)
+        p_mid[:3] = np.mod(p_mid[:3] + p_mid[3:] * (sc["dtau"] / dxc), N)
+        p_out, route = sl.migrate(T(np.concatenate([p_mid, ids_in[None].astype(np.float64)], axis=0)), return_route=True)
+        ids_out = p_out[6].numpy().astype(np.int64)
+        ins, cur = [], u0
+        for d in O.strang_order(k):
+            if d == 2:
+                pad = sl.halo_exchange(T(np.concatenate([cur, g[2][None]], axis=0)), 3).numpy()
+                ins.append((pad, 2))
+                cur = O.sweep(pad[:5], 2, lam, kap, cfg.gamma, pad[5], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)[0][:, 3:-3].copy()
+            else:
+                ins.append((cur, d))
+                cur, _ = O.sweep(cur, d, lam, kap, cfg.gamma, g[d], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+        # ---- reverse: S4
+        cg = cot_g[:, z0:z0 + nz].copy()
+        gb = np.zeros((3, nz, N, N))
+        for u_in, d in reversed(ins):
+            if d == 2:
+                cpad = np.zeros((5, nz + 6, N, N)); cpad[:, 3:-3] = cg             # the pads' outputs were discarded
+                cin, gbz, _ = O.sweep_vjp(u_in[:5], 2, lam, kap, cfg.gamma, cpad, u_in[5], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+                red = sl.halo_reduce(T(np.concatenate([cin, gbz[None]], axis=0)), 3).numpy()   # transpose of the exchange
+                cg, gb[2] = red[:5], gb[2] + red[5]
+            else:
+                cg, gbd, _ = O.sweep_vjp(u_in, d, lam, kap, cfg.gamma, cg, g[d], e_floor=cfg.e_floor(), lim_eps=cfg.lim_eps)
+                gb[d] += gbd
+        # ---- S3: cotangents travel back to where their particles came from, then drift / kick / gather transposed
+        cp_out = cot_p[:, ids_out]
+        cp_mid = sl.migrate_back(T(cp_out), route).numpy()
+        wt = cp_mid[3:] + (sc["dtau"] / dxc) * cp_mid[:3]
+        xb = cp_mid[:3].copy()
+        gb_pad = np.zeros((3, nz + 2, N, N))
+        for d in range(3):
+            xb += sc["K"] * wt[d] * _gather_grad_local(gpad[d], p_in, N, z0 - 1)
+            gb_pad[d] = _cic_local(p_in, N, z0 - 1, nz + 2, weights=sc["K"] * wt[d])
+        gb += sl.halo_reduce(T(gb_pad), 1).numpy()                  # transpose of the g' halo exchange
+        # ---- S2, S1
+        db = sl.poisson_slab_vjp(T(gb), sc["A"], cfg.box).numpy()
+        cg[0] += db
+        db_pad = sl.halo_exchange(T(db), 1).numpy()                 # transpose of the deposit's halo_reduce
+        xb += m_p * _gather_grad_local(db_pad, p_in, N, z0 - 1)
+        res = {"gas": float(np.max(np.abs(cg - rg[:, z0:z0 + nz])) / np.max(np.abs(rg))),
+               "part": float(np.max(np.abs(np.concatenate([xb, wt]) - rp[:, ids_in])) / np.max(np.abs(rp))),
+               "moved": int(np.sum(~np.isin(ids_out, ids_in)))}
+        q.put((rank, res))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_the_step_vjp_on_slabs_is_the_single_rank_step_vjp():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_vjp_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, w in out:
+        assert w["gas"] < 1e-11 and w["part"] < 1e-11, w
+    assert sum(w["moved"] for _, w in out) > 0          # some particles did change slabs: migrate_back was exercised
 
 
 @pytest.mark.parametrize("world", [2])
