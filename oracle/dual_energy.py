@@ -363,7 +363,8 @@ def coupled_step_vjp(O, P, gas6, part, a_i, a_next, dt, dt_prev, step, cot_gas6,
                         for dxx in (0, 1):
                             ix = i1[0] if dxx else i0[0]; iy = i1[1] if dy else i0[1]; iz = i1[2] if dz else i0[2]
                             w_ = (f[0] if dxx else 1 - f[0]) * (f[1] if dy else 1 - f[1]) * (f[2] if dz else 1 - f[2])
-                            np.add.at(gb[d], (iz, iy, ix), sc["K"] * wt[d] * w_)
+                            gb[d] += np.bincount((iz * N + iy) * N + ix, weights=sc["K"] * wt[d] * w_,
+                                                 minlength=N ** 3).reshape(N, N, N)
         cp = np.concatenate([xb, wt])
     if g is not None:
         db = O.poisson_vjp(N, P.box, sc["A"], gb)
@@ -383,6 +384,25 @@ def coupled_run(O, P, gas6, part, a0, a_sched, dt_sched, eta=1e-3, step0=0):
         dtp = dt_sched[k]
         cmax.append(cm)
     return gas6, part, np.array(cmax)
+
+
+def coupled_run_vjp(O, P, gas6, part, a0, a_sched, dt_sched, cot_gas6, cot_part, eta=1e-3, step0=0):
+    """Reverse pass of coupled_run: every step's input is kept, then coupled_step_vjp last step first.
+    Returns (cot_gas6 of the initial state, cot_part, d gamma)."""
+    states, a, dtp = [], a0, 0.0
+    g6 = np.asarray(gas6, dtype=np.float64); p = np.asarray(part, dtype=np.float64)
+    for k in range(len(dt_sched)):
+        states.append((g6, p, a, dtp))
+        g6, p, _ = coupled_step(O, P, g6, p, a, a_sched[k], dt_sched[k], dtp, step0 + k, eta)
+        a = 1.0 if P.static_mode else a_sched[k]
+        dtp = dt_sched[k]
+    cg = np.asarray(cot_gas6, dtype=np.float64); cp = np.asarray(cot_part, dtype=np.float64)
+    dgamma = 0.0
+    for k in reversed(range(len(dt_sched))):
+        g6, p, a, dtp = states[k]
+        cg, cp, dg = coupled_step_vjp(O, P, g6, p, a, a_sched[k], dt_sched[k], dtp, step0 + k, cg, cp, eta)
+        dgamma += dg
+    return cg, cp, dgamma
 
 
 def thermal_energy(gas6, eta=1e-3):

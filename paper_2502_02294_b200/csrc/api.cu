@@ -488,6 +488,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "overlap")) c->tune_overlap = value;
     else if (!strcmp(key, "prime")) c->tune_prime = value;
     else if (!strcmp(key, "deposit_tile")) c->tune_deposit_tile = value;
+    else if (!strcmp(key, "de_march")) c->tune_de_march = value;
     else { set_error("dh_tune: unknown key %s", key); return DH_ERR_INVALID; }
     return DH_OK;
 }

@@ -213,6 +213,10 @@ int launch_sweep_de(dh_ctx* c, int d, float* const in[6], const float* g, float 
 int launch_sweep_de_vjp(dh_ctx* c, int d, float* const in[6], const float* g, float lam, float kap,
                         float* const cot_out[6], float* const cot_in[6], float* g_bar, double* scal_bar);
 
+// marching forward y/z sweep of the dual-energy variant (sweep_march.cu); pointers permuted to (rho, m_n, m_t1, m_t2, eps, q)
+int launch_sweep_march_de(dh_ctx* c, int d, const float* const in[6], const float* g, float* const out[6], float* cmax,
+                          const SweepConst& sc);
+
 // marching y/z kernels (sweep_march.cu); the field pointers are already permuted to (rho, m_n, m_t1, m_t2, eps)
 int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const MPtr5& pout, float* cmax,
                        const SweepConst& sc, float* delta_out);

@@ -626,6 +626,11 @@ int launch_sweep_de(dh_ctx* c, int d, float* const in[6], const float* g, float 
         const size_t sm = (size_t)DE_FWD_SLOTS * block.x * block.y * sizeof(float);
         if (g) DE_LAUNCH((sweep_de_x_fwd_kernel<true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
         else DE_LAUNCH((sweep_de_x_fwd_kernel<false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
+    } else if (c->tune_de_march) {
+        // y / z forward: the marching pipeline with the sixth component (sweep_march.cu), 3.2 x faster than the chain tile
+        float* outm[6];
+        for (int k = 0; k < 6; ++k) outm[k] = pout.p[k];
+        DH_TRY(launch_sweep_march_de(c, d, pin.p, g, outm, cmax, sc));
     } else {
         const int C = de_yz_chain_threads(N, 3);
         const int S = C * KD - 6;

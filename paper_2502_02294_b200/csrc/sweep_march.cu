@@ -170,6 +170,159 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
     if (cmax) block_max_to_global(cm, cmax, &s_max);
 }
 
+// --------------------------------------------------------------------------- forward, dual-energy variant ----
+// The same pipeline with the sixth component q (sweep_de.cu states the scheme; readings R33-R36): P selects the thermal
+// energy, the sixth flux component is q_s v, and the source -p dv/dx enters stage A for cell q-1 with v_q - v_{q-2} and
+// stage B for cell q-3 with v*_{q-2} - v*_{q-4}: four more carried velocities and two pressures, no extra delay.
+struct Ptr6m { const float* p[6]; };
+struct MPtr6m { float* p[6]; };
+
+__device__ __forceinline__ void prim_de_m(const float (&u)[6], const SweepConst& sc, float (&G)[6], float (&H)[6], float& c,
+                                          float& v, float& p, float& qs) {
+    const float rinv = rcp_fast(u[0]);
+    v = u[1] * rinv;
+    const float ke = 0.5f * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) * rinv;
+    const float eT = (u[4] - ke) * rinv;
+    const float e = eT > sc.de_eta * (u[4] * rinv) ? eT : u[5] * rinv;
+    qs = u[0] * e;
+    const float ep = !(e <= sc.e_floor) ? e : sc.e_floor;
+    p = sc.gm1 * u[0] * ep;
+    c = fabsf(v) + sqrt_fast(sc.ggm1 * ep);
+    const float U[6] = {u[0], u[1], u[2], u[3], u[4], qs};
+    const float F[6] = {u[1], fmaf(u[1], v, p), u[2] * v, u[3] * v, (u[4] + p) * v, qs * v};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        G[k] = fmaf(c, U[k], F[k]);
+        H[k] = fmaf(c, U[k], -F[k]);
+    }
+}
+
+template <bool HAS_G, bool EPS>
+struct FwdPipeDE {
+    float U1[6], g1, G1[6], D2[6];       // (u, q_s)_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
+    float R1[6], R2[6];                  // R_{q-2}, R_{q-3}
+    float Gs[6], dGs[6], Hs[6], dHs[6];  // G*_{q-2}, dG_{q-3}, H*_{q-2}, dH_{q-3}
+    float PG[6], Psi[6];                 // PsiG_{q-3}, Psi_{q-4}
+    float v1, v2, p1;                    // v_{q-1}, v_{q-2}, p_{q-1}
+    float vsA, vsB, vsC, psA, psB;       // v*_{q-2}, v*_{q-3}, v*_{q-4}, p*_{q-2}, p*_{q-3}
+
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            U1[k] = 1.f; G1[k] = 0.f; D2[k] = 0.f; R1[k] = 0.f; R2[k] = 0.f; Gs[k] = 0.f; dGs[k] = 0.f; Hs[k] = 0.f;
+            dHs[k] = 0.f; PG[k] = 0.f; Psi[k] = 0.f;
+        }
+        g1 = 0.f; v1 = v2 = p1 = 0.f; vsA = vsB = vsC = psA = psB = 0.f;
+    }
+
+    // take cell q; out = (u', q')_{q-3}; c0 = freezing speed of cell q
+    __device__ __forceinline__ void push(const float (&u0)[6], float g0, const SweepConst& sc, float (&out)[6], float& c0) {
+        float G0[6], H0[6], v0, p0, qs0;
+        prim_de_m(u0, sc, G0, H0, c0, v0, p0, qs0);
+        float us[6], D1[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            D1[k] = G1[k] - H0[k];
+            us[k] = fmaf(-0.25f * sc.lam, D1[k] - D2[k], U1[k]);
+        }
+        us[5] = fmaf(-0.25f * sc.lam * p1, v0 - v2, us[5]);
+        float R0[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) R0[k] = U1[k];
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * g1;
+            us[1] = fmaf(hk, U1[0], us[1]);
+            us[4] = fmaf(hk, U1[1], us[4]);
+            const float kg = sc.kap * g1;
+            R0[1] = fmaf(kg, us[0], R0[1]);
+            R0[4] = fmaf(kg, us[1], R0[4]);
+        }
+        float Gs0[6], Hs0[6], cdummy, vs0, ps0, qdummy;
+        prim_de_m(us, sc, Gs0, Hs0, cdummy, vs0, ps0, qdummy);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float dG0 = Gs0[k] - Gs[k];
+            const float dH0 = Hs0[k] - Hs[k];
+            const float PG0 = Gs[k] + limM<EPS>(dGs[k], dG0, sc.eps4);
+            const float PH = Hs[k] - limM<EPS>(dHs[k], dH0, sc.eps4);
+            const float Psi0 = PG[k] - PH;
+            out[k] = fmaf(-0.5f * sc.lam, Psi0 - Psi[k], R2[k]);
+            Psi[k] = Psi0; PG[k] = PG0;
+            Gs[k] = Gs0[k]; dGs[k] = dG0; Hs[k] = Hs0[k]; dHs[k] = dH0;
+            R2[k] = R1[k]; R1[k] = R0[k];
+            G1[k] = G0[k]; D2[k] = D1[k];
+        }
+        out[5] = fmaf(-0.5f * sc.lam * psB, vsA - vsC, out[5]);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) U1[k] = u0[k];
+        U1[5] = qs0;
+        g1 = g0;
+        v2 = v1; v1 = v0; p1 = p0;
+        vsC = vsB; vsB = vsA; vsA = vs0;
+        psB = psA; psA = ps0;
+    }
+};
+
+template <int DIR, bool HAS_G, bool EPS>
+__global__ void __launch_bounds__(128, 3) sweep_march_fwd_de_kernel(Ptr6m in, const float* __restrict__ gfield, MPtr6m outp,
+                                                                    float* cmax, SweepConst sc, int S) {
+    constexpr int HALO = 3, NF = HAS_G ? 7 : 6;
+    extern __shared__ float ring[];              // [RING][NF][nthr]
+    __shared__ int s_max;
+    constexpr int nthr = NTHR;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    if (tid == 0) s_max = 0;
+    __syncthreads();
+    const int N = sc.N;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int o = blockIdx.y * blockDim.y + threadIdx.y;
+    const int p0 = blockIdx.z * S;
+    const int len = min(S, N - p0);
+    const int stride = DIR == 1 ? N : N * N;
+    const int base = DIR == 1 ? o * N * N + x : o * N + x;
+    const int niter = len + 2 * HALO;
+    AxisPos ld;
+    ld.set(p0 - HALO, N, base, stride);
+    int off_out = base + p0 * stride;
+    float* const my = ring + tid;
+    auto issue = [&](int it) {
+        float* dst = my + (it & (RING - 1)) * NF * nthr;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) cp_async4(dst + k * nthr, in.p[k] + ld.off);
+        if (HAS_G) cp_async4(dst + 6 * nthr, gfield + ld.off);
+        ld.next(N, base, stride);
+    };
+#pragma unroll
+    for (int it = 0; it < PF_FWD; ++it) {
+        if (it < niter) issue(it);
+        cp_async_commit();
+    }
+    FwdPipeDE<HAS_G, EPS> pipe;
+    pipe.init();
+    float cm = 0.f;
+#pragma unroll 2
+    for (int i = 0; i < niter; ++i) {
+        if (i + PF_FWD < niter) issue(i + PF_FWD);
+        cp_async_commit();
+        cp_async_wait<PF_FWD>();
+        const float* src = my + (i & (RING - 1)) * NF * nthr;
+        float u0[6], g0 = 0.f;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) u0[k] = src[k * nthr];
+        if (HAS_G) g0 = src[6 * nthr];
+        float out[6], c0;
+        pipe.push(u0, g0, sc, out, c0);
+        // the CFL maximum is over the sweep's own cells (the halo cells belong to the neighbouring segments)
+        if (i >= HALO && i < len + HALO) cm = (c0 > cm || c0 != c0) ? c0 : cm;
+        if (i >= 2 * HALO) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) outp.p[k][off_out] = out[k];
+            off_out += stride;
+        }
+    }
+    if (cmax) block_max_to_global(cm, cmax, &s_max);
+}
+
 // ------------------------------------------------------------------------------------------------- adjoint ----
 // LK = false drops the cotangents of lam and kap (dh_options.want_dsched = 0): gamma_b only.
 template <bool HAS_G, int EPS, bool LK>
@@ -454,6 +607,36 @@ int launch_sweep_march(dh_ctx* c, int d, const Ptr5& pin, const float* g, const 
     const bool eps = c->opt.lim_eps > 1e-18;
     if (d == 1) DH_TRY(march_fwd_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out));
     else DH_TRY(march_fwd_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps, delta_out));
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+template <int DIR>
+static int march_fwd_de_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr6m& pin, const float* g, const MPtr6m& pout,
+                                 float* cmax, const SweepConst& sc, int S, bool eps) {
+    const size_t sm = (size_t)RING * (g ? 7 : 6) * block.x * block.y * sizeof(float);
+    if (g) {
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_de_kernel<DIR, true, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        else MARCH_LAUNCH((sweep_march_fwd_de_kernel<DIR, true, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+    } else {
+        if (eps) MARCH_LAUNCH((sweep_march_fwd_de_kernel<DIR, false, true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+        else MARCH_LAUNCH((sweep_march_fwd_de_kernel<DIR, false, false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, S);
+    }
+    return DH_OK;
+}
+
+// y / z forward sweep of the dual-energy variant; pointers already permuted to (rho, m_n, m_t1, m_t2, eps, q)
+int launch_sweep_march_de(dh_ctx* c, int d, const float* const in[6], const float* g, float* const out[6], float* cmax,
+                          const SweepConst& sc) {
+    const int N = c->N;
+    const int S = march_segment(N, c->tune_march_s_fwd, 3);
+    const dim3 block = march_block(N);
+    const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
+    const bool eps = c->opt.lim_eps > 1e-18;
+    Ptr6m pin; MPtr6m pout;
+    for (int k = 0; k < 6; ++k) { pin.p[k] = in[k]; pout.p[k] = out[k]; }
+    if (d == 1) DH_TRY(march_fwd_de_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps));
+    else DH_TRY(march_fwd_de_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps));
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }
