@@ -354,3 +354,39 @@ def test_de_coupled_step_vjp_matches_oracle(api, torch_, O, DE, W, IC):
     assert e_trim < 2e-5 and e_all < 2e-2 and PT.rel_l2(got_p, rp) < 2e-3
     assert abs(dp.dgamma - rdg) < 2e-3 * max(abs(rdg), 1.0)
     ctx.close()
+
+
+def test_config2_full_run_gradient_with_dual_energy(api, torch_, O, DE, W, IC):
+    """Config 2 in full (64^3, 100 steps to a = 0.33) with dual energy: the gradient of sum (rho - rho_target)^2 through the
+    checkpointed reverse pass against the oracle's reverse pass of the same run.  Without dual energy this comparison is
+    ill-conditioned in any precision (a quarter of the cells sit on the energy floor: 2.6e-2 ... 1.4e-1 over all entries,
+    tests/test_gpu_parity.py); with it no cell does, the fp64 oracle moves itself by 1.2e-3 under one fp32 rounding of its
+    input (measured once: the perturbed copy costs another 4 minutes of numpy), and B200 lands at 1.45e-3 ... 1.55e-3 over
+    ALL entries, 6.9e-4 on all but the worst 1 %, particles 3e-3, d gamma 3e-5."""
+    cfg = W.CONFIGS[2]
+    delta, gas, part = IC.coupled_ic(W, cfg)
+    P = PT.oracle_params(O, cfg)
+    a_s, dt_s = O.schedule_lna(P, cfg.a0, cfg.a1, cfg.n_steps)
+    vf, e0 = api.ic_factors_for(cfg)
+    eta = 1e-3
+    target = cfg.f_b * (1.0 + W.gaussian_field(cfg.N, cfg.box, cfg.target_seed, cfg.rms_delta))
+    g6 = np.concatenate([gas, (e0 * gas[0].astype(np.float64))[None].astype(np.float32)], axis=0)
+    ref6, refp, _ = DE.coupled_run(O, P, g6, part, cfg.a0, a_s[1:], dt_s, eta=eta)
+    cot = np.zeros_like(ref6); cot[0] = 2.0 * (ref6[0] - target)
+    rg, rp, rdg = DE.coupled_run_vjp(O, P, g6, part, cfg.a0, a_s[1:], dt_s, cot, np.zeros_like(refp), eta=eta)
+    ctx = api.context_for(cfg, dual_energy=1, dual_eta=eta)
+    st = api.State(g6, part, cfg.a0)
+    ctx.dh_run(st, a_s[1:], dt_s, 10)
+    e_f = max(PT.field_err(st.gas[:5].cpu().numpy(), ref6[:5]).values())
+    cg = torch_.zeros_like(st.gas)
+    ctx.dh_data_term(0, st.gas, _gpu(torch_, target), None, 1.0, 1.0, cg, want_loss=False)
+    ct = api.Cot(cg, torch_.zeros_like(st.part))
+    dp = ctx.dh_run_vjp(ct, ct)
+    got, gotp = ct.gas.double().cpu().numpy(), ct.part.double().cpu().numpy()
+    e_all, e_trim, e_p = PT.rel_l2(got, rg), PT.rel_l2_trimmed(got, rg, frac=1e-2), PT.rel_l2(gotp, rp)
+    print(f"config2 with dual energy: fields {e_f:.2e}; gradient over all entries {e_all:.2e}, all but the worst 1 % {e_trim:.2e}, "
+          f"particles {e_p:.2e}, dgamma {dp.dgamma / rdg - 1:+.1e}")
+    assert np.all(np.isfinite(got)) and np.all(np.isfinite(gotp))
+    assert e_f < 5e-3 and e_all < 4e-3 and e_trim < 1.5e-3 and e_p < 8e-3
+    assert abs(dp.dgamma / rdg - 1) < 5e-4
+    ctx.close()
