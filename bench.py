@@ -237,6 +237,7 @@ def main():
     ap.add_argument("--no-full-run", dest="full_run", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-de-leg", action="store_true", help="skip the dual-energy leg of the default run")
     ap.add_argument("--dual-energy", action="store_true",
                     help="run the dual-energy variant (DESIGN.md section 19: six gas fields, chain kernels on all axes); "
                          "recorded in config, not the headline configuration")
@@ -326,7 +327,7 @@ def main():
     def fwd_vjp(c, st0, k0, nsteps, st_stride):
         st = st0.clone()
         c.dh_run(st, a_all[k0:k0 + nsteps], dt_all[k0:k0 + nsteps], st_stride)
-        cg = torch.zeros_like(st.gas) if args.dual_energy else torch.empty_like(st.gas)
+        cg = torch.zeros_like(st.gas) if st.gas.shape[0] == 6 else torch.empty_like(st.gas)
         c.dh_data_term(0, st.gas, target, None, 1.0, 1.0, cg, want_loss=False)   # sum (rho - rho_t)^2 (reading R21)
         ct = api.Cot(cg, torch.zeros_like(st.part))
         dp = c.dh_run_vjp(ct, ct)
@@ -337,7 +338,7 @@ def main():
         best, best_f, res = None, None, None
         for _ in range(passes):
             st = st0.clone()
-            cg = torch.zeros_like(st.gas) if args.dual_energy else torch.empty_like(st.gas)
+            cg = torch.zeros_like(st.gas) if st.gas.shape[0] == 6 else torch.empty_like(st.gas)
             ct = api.Cot(cg, torch.zeros_like(st.part))
             ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
             l0 = c.dh_launch_count()
@@ -546,6 +547,22 @@ def main():
                    "dparams": dp2.as_dict()}
         ctx2.close()
 
+    # ---- the dual-energy variant on the headline window, from the same state with q = rho e_T
+    de_leg = None
+    if not args.no_de_leg and not args.dual_energy and not cfg.static_mode and world == 1:
+        ctx3 = api.context_for(cfg, want_dA=0, want_dsched=0, dual_energy=1, dual_eta=1e-3)
+        g5 = R["st0"].gas
+        q0 = (g5[4] - 0.5 * (g5[1] ** 2 + g5[2] ** 2 + g5[3] ** 2) / g5[0]).clamp_min(0.0)
+        st_de = api.State(torch.cat([g5, q0[None]], dim=0), R["st0"].part, R["st0"].a, R["st0"].dt_prev, R["st0"].step)
+        fwd_vjp(ctx3, st_de, R["k0"], min(Wm, K), stride)
+        ms3, ms3f, _, _, dp3, _ = timed_window(ctx3, st_de, R["k0"], 1)
+        de_leg = {"value": job_throughput(world, n3, K, ms3), "unit": UNIT, "ms_per_step": ms3 / K,
+                  "fwd_ms_per_step": ms3f / K, "window": wkey, "dual_eta": 1e-3, "dgamma": dp3.dgamma,
+                  "note": "dh_options.dual_energy = 1: six gas fields; y/z forward on the marching pipeline, adjoint on the "
+                          "chain kernels (not tuned)"}
+        ctx3.close()
+        del st_de
+
     if rank == 0:
         sched = (f"{K} consecutive steps of the {cfg.n_steps}-step ln-a schedule per window; value = the slower window "
                  f"({wkey}, from step {R['k0']}), best of {args.passes} passes") if not cfg.static_mode else f"{K} steps at CFL 0.4"
@@ -557,7 +574,7 @@ def main():
                           "loss": "sum (rho_gas - rho_target)^2", "gradients": "d/d(initial state), d/d(delta_init), d/d(gamma); want_dA=0, want_dsched=0 (all of dh_dparams: full_dparams)", "parallelism": f"replicas x{world}", "tune": args.tune, "dual_energy": bool(args.dual_energy),
                           "l2": "working set (state + scratch >= 0.7 GB at 256^3) exceeds the 126 MB L2; no flush"},
                "fwd": {"value": value_fwd, "unit": UNIT, "ms_per_step": ms_fwd / K},
-               "windows": win_out, "full_dparams": full_dp, "full_run": full_run,
+               "windows": win_out, "full_dparams": full_dp, "dual_energy_variant": de_leg, "full_run": full_run,
                "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,
                "cpu_baseline": cpu, "clocks": clocks,
                "ic": ic_ms,

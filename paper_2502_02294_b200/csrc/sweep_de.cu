@@ -24,98 +24,6 @@ namespace dh {
 struct Ptr6 { const float* p[6]; };
 struct MPtr6s { float* p[6]; };
 
-// (G, H, c, v, p, q_s) = P(u, q);  u6 = (rho, m_n, m_t1, m_t2, eps, q)
-__device__ __forceinline__ void prim_de(const float (&u)[6], const SweepConst& sc, float (&G)[6], float (&H)[6], float& c,
-                                        float& v, float& p, float& qs) {
-    const float rinv = rcp_fast(u[0]);
-    v = u[1] * rinv;
-    const float ke = 0.5f * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) * rinv;
-    const float eT = (u[4] - ke) * rinv;
-    const bool useT = eT > sc.de_eta * (u[4] * rinv);
-    const float e = useT ? eT : u[5] * rinv;
-    qs = u[0] * e;
-    const float ep = !(e <= sc.e_floor) ? e : sc.e_floor;
-    p = sc.gm1 * u[0] * ep;
-    const float cs = sqrt_fast(sc.ggm1 * ep);
-    c = fabsf(v) + cs;
-    const float U[6] = {u[0], u[1], u[2], u[3], u[4], qs};
-    float F[6];
-    F[0] = u[1];
-    F[1] = fmaf(u[1], v, p);
-    F[2] = u[2] * v;
-    F[3] = u[3] * v;
-    F[4] = (u[4] + p) * v;
-    F[5] = qs * v;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        G[k] = fmaf(c, U[k], F[k]);
-        H[k] = fmaf(c, U[k], -F[k]);
-    }
-}
-
-// Transpose of P at (u, q): cotangents of G, H (six each) and the extra cotangents of v, p, q_s; returns ub (six: the last
-// is the cotangent of q) and adds to gamma_b.
-__device__ __forceinline__ void prim_de_vjp(const float (&u)[6], const SweepConst& sc, const float (&Gb)[6],
-                                            const float (&Hb)[6], float vb0, float pb0, float qsb0, float (&ub)[6],
-                                            float& gamma_b) {
-    const float rinv = rcp_fast(u[0]);
-    const float v = u[1] * rinv;
-    const float m2 = u[1] * u[1] + u[2] * u[2] + u[3] * u[3];
-    const float ke = 0.5f * m2 * rinv;
-    const float eT = (u[4] - ke) * rinv;
-    const bool useT = eT > sc.de_eta * (u[4] * rinv);
-    const float e = useT ? eT : u[5] * rinv;
-    const float qs = u[0] * e;
-    const bool active = !(e <= sc.e_floor);
-    const float ep = active ? e : sc.e_floor;
-    const float p = sc.gm1 * u[0] * ep;
-    const float cs = sqrt_fast(sc.ggm1 * ep);
-    const float c = fabsf(v) + cs;
-    const float U[6] = {u[0], u[1], u[2], u[3], u[4], qs};
-    float cub[6], Fb[6], Ub[6];
-    float cb = 0.f;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        cub[k] = Gb[k] + Hb[k];
-        Fb[k] = Gb[k] - Hb[k];
-        cb = fmaf(cub[k], U[k], cb);
-        Ub[k] = c * cub[k];
-    }
-    float mnb = fmaf(Fb[1], v, Fb[0]);
-    float vb = vb0 + Fb[1] * u[1] + Fb[2] * u[2] + Fb[3] * u[3] + Fb[4] * (u[4] + p) + Fb[5] * qs;
-    const float pb = pb0 + fmaf(Fb[4], v, Fb[1]);
-    float epsb = Fb[4] * v;
-    const float qsb = qsb0 + Ub[5] + Fb[5] * v;
-    const float sgn = (v > 0.f) ? 1.f : ((v < 0.f) ? -1.f : 0.f);
-    vb = fmaf(sgn, cb, vb);
-    const float half_cs_inv = 0.5f * rcp_fast(cs);
-    float epb = cb * sc.ggm1 * half_cs_inv;
-    gamma_b = fmaf(cb * (2.f * sc.gamma - 1.f) * ep, half_cs_inv, gamma_b);
-    gamma_b = fmaf(pb * u[0], ep, gamma_b);
-    float rhob = pb * sc.gm1 * ep;
-    epb = fmaf(pb * sc.gm1, u[0], epb);
-    float eb = active ? epb : 0.f;
-    eb = fmaf(qsb, u[0], eb);                    // q_s = rho e
-    rhob = fmaf(qsb, e, rhob);
-    const float eTb = useT ? eb : 0.f;           // e = e_T or q / rho
-    const float eIb = useT ? 0.f : eb;
-    const float qb = eIb * rinv;
-    rhob -= eIb * u[5] * rinv * rinv;
-    const float ebr = eTb * rinv;
-    epsb += ebr;
-    rhob += ebr * (2.f * ke * rinv - u[4] * rinv);
-    const float mcoef = -ebr * rinv;
-    mnb = fmaf(mcoef, u[1], mnb);
-    mnb = fmaf(vb, rinv, mnb);
-    rhob -= vb * v * rinv;
-    ub[0] = Ub[0] + rhob;
-    ub[1] = Ub[1] + mnb;
-    ub[2] = Ub[2] + fmaf(mcoef, u[2], Fb[2] * v);
-    ub[3] = Ub[3] + fmaf(mcoef, u[3], Fb[3] * v);
-    ub[4] = Ub[4] + epsb;
-    ub[5] = qb;
-}
-
 struct ChainDE {
     float* ex;
     int nthr, tid, ltid, rtid;
@@ -668,6 +576,11 @@ int launch_sweep_de_vjp(dh_ctx* c, int d, float* const in[6], const float* g, fl
         const size_t sm = (size_t)DE_ADJ_SLOTS * block.x * block.y * sizeof(float);
         if (g) DE_LAUNCH((sweep_de_x_adj_kernel<true>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
         else DE_LAUNCH((sweep_de_x_adj_kernel<false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
+    } else if (c->tune_de_march && !c->opt.want_dsched) {
+        // y / z adjoint without the cotangents of Dtau and kappa: the marching pipeline with the sixth component
+        float* cim[6];
+        for (int k = 0; k < 6; ++k) cim[k] = pci.p[k];
+        DH_TRY(launch_sweep_march_de_vjp(c, d, pin.p, g, pco.p, cim, g_bar, scal_bar, sc));
     } else {
         const int C = de_yz_chain_threads(N, 4);
         const int S = C * KD - 8;

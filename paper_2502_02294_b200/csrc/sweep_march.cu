@@ -177,26 +177,6 @@ __global__ void __launch_bounds__(128, 4) sweep_march_fwd_kernel(Ptr5 in, const 
 struct Ptr6m { const float* p[6]; };
 struct MPtr6m { float* p[6]; };
 
-__device__ __forceinline__ void prim_de_m(const float (&u)[6], const SweepConst& sc, float (&G)[6], float (&H)[6], float& c,
-                                          float& v, float& p, float& qs) {
-    const float rinv = rcp_fast(u[0]);
-    v = u[1] * rinv;
-    const float ke = 0.5f * (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]) * rinv;
-    const float eT = (u[4] - ke) * rinv;
-    const float e = eT > sc.de_eta * (u[4] * rinv) ? eT : u[5] * rinv;
-    qs = u[0] * e;
-    const float ep = !(e <= sc.e_floor) ? e : sc.e_floor;
-    p = sc.gm1 * u[0] * ep;
-    c = fabsf(v) + sqrt_fast(sc.ggm1 * ep);
-    const float U[6] = {u[0], u[1], u[2], u[3], u[4], qs};
-    const float F[6] = {u[1], fmaf(u[1], v, p), u[2] * v, u[3] * v, (u[4] + p) * v, qs * v};
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        G[k] = fmaf(c, U[k], F[k]);
-        H[k] = fmaf(c, U[k], -F[k]);
-    }
-}
-
 template <bool HAS_G, bool EPS>
 struct FwdPipeDE {
     float U1[6], g1, G1[6], D2[6];       // (u, q_s)_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
@@ -218,7 +198,7 @@ struct FwdPipeDE {
     // take cell q; out = (u', q')_{q-3}; c0 = freezing speed of cell q
     __device__ __forceinline__ void push(const float (&u0)[6], float g0, const SweepConst& sc, float (&out)[6], float& c0) {
         float G0[6], H0[6], v0, p0, qs0;
-        prim_de_m(u0, sc, G0, H0, c0, v0, p0, qs0);
+        prim_de(u0, sc, G0, H0, c0, v0, p0, qs0);
         float us[6], D1[6];
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
@@ -238,7 +218,7 @@ struct FwdPipeDE {
             R0[4] = fmaf(kg, us[1], R0[4]);
         }
         float Gs0[6], Hs0[6], cdummy, vs0, ps0, qdummy;
-        prim_de_m(us, sc, Gs0, Hs0, cdummy, vs0, ps0, qdummy);
+        prim_de(us, sc, Gs0, Hs0, cdummy, vs0, ps0, qdummy);
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
             const float dG0 = Gs0[k] - Gs[k];
@@ -541,6 +521,224 @@ __global__ void __launch_bounds__(128, ADJ_BLOCKS) sweep_march_adj_kernel(Ptr5 i
     block_sum3_to_global(lacc, kacc, gacc, scal, s_red);
 }
 
+// --------------------------------------------------------------------------- adjoint, dual-energy variant ----
+// AdjPipe with the sixth component and the transposes of the two source terms (gamma_b only: a context that wants the
+// cotangents of Dtau and kappa goes through the chain kernels of sweep_de.cu).  With t_n = p*_n q'_b,n and tA_n = p_n q*_b,n:
+//   cell m = q-3:  v*_b = -(lam/2)(t_{q-4} - t_{q-2}),   p*_b = -(lam/2) q'_b,m (v*_{q-2} - v*_{q-4})      -> P^T(u*_m, q*_m)
+//   cell r = q-4:  v_b  = -(lam/4)(tA_{q-5} - tA_{q-3}), p_b  = -(lam/4) q*_b,r (v_{q-3} - v_{q-5}),  q_s_b = q'_b,r + q*_b,r -> P^T(u_r, q_r)
+template <bool HAS_G, int EPS>
+struct AdjPipeDE {
+    float U1[6], g1, G1[6], D2[6];         // (u, q_s)_{q-1}, g_{q-1}, G_{q-1}, D_{q-2}
+    float us1[6], us2[6];                  // (u*, q*)_{q-2}, (u*, q*)_{q-3}
+    float Gs[6], dGs[6], Hs[6], dHs[6];    // G*_{q-2}, dG_{q-3}, H*_{q-2}, dH_{q-3}
+    float GB0[6], GB1[6], HB0[6], HB1[6];  // partial G*_b, H*_b in flight (as AdjPipe)
+    float accR[5], qsbR, usbR[6], DbR[6];  // cell q-4: ob + u*_b + source^T, q'_b + q*_b, (u*, q*)_b; D_b_{q-5}
+    float v1, v2, v3, v4, v5, p1, p2, p3;  // v_{q-1 .. q-5}, p_{q-1 .. q-3} of the input cells
+    float tA4, tA5;                        // tA_{q-4}, tA_{q-5}
+    float vsA, vsB, vsC, psA, psB, psC;    // v*, p* of cells q-2, q-3, q-4
+    float obq4;                            // q'_b of cell q-4
+
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            U1[k] = 1.f; G1[k] = 0.f; D2[k] = 0.f; us1[k] = 1.f; us2[k] = 1.f; Gs[k] = 0.f; dGs[k] = 0.f; Hs[k] = 0.f;
+            dHs[k] = 0.f; GB0[k] = 0.f; GB1[k] = 0.f; HB0[k] = 0.f; HB1[k] = 0.f; usbR[k] = 0.f; DbR[k] = 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k) accR[k] = 0.f;
+        qsbR = 0.f; g1 = 0.f;
+        v1 = v2 = v3 = v4 = v5 = p1 = p2 = p3 = tA4 = tA5 = 0.f;
+        vsA = vsB = vsC = psA = psB = psC = obq4 = 0.f;
+    }
+
+    __device__ __forceinline__ void push(const float (&u0)[6], float g0, const float (&ob0)[6], const float (&ob1)[6],
+                                         const float (&ob2)[6], const float (&uM)[6], float gM, const float (&uR)[6],
+                                         const SweepConst& sc, float (&ub)[6], float& gb, float& gamM, float& gamR) {
+        // ---- forward recompute: P(u_q), (u*, q*)_{q-1}, P of it
+        float G0[6], H0[6], cdummy, v0, p0, qs0;
+        prim_de(u0, sc, G0, H0, cdummy, v0, p0, qs0);
+        float us0[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float D1 = G1[k] - H0[k];
+            us0[k] = fmaf(-0.25f * sc.lam, D1 - D2[k], U1[k]);
+            D2[k] = D1;
+        }
+        us0[5] = fmaf(-0.25f * sc.lam * p1, v0 - v2, us0[5]);
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * g1;
+            us0[1] = fmaf(hk, U1[0], us0[1]);
+            us0[4] = fmaf(hk, U1[1], us0[4]);
+        }
+        float Gs0[6], Hs0[6], vs0, ps0, qdummy;
+        prim_de(us0, sc, Gs0, Hs0, cdummy, vs0, ps0, qdummy);
+        // ---- limiters: G side of interface q-2, H side of interface q-3; G*_b, H*_b of cell q-3 complete
+        float GsB[6], HsB[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float dG0 = Gs0[k] - Gs[k];
+            const float dH0 = Hs0[k] - Hs[k];
+            float LA, LB, MA, MB;
+            limM_grad<EPS>(dGs[k], dG0, sc.eps4, LA, LB);
+            limM_grad<EPS>(dHs[k], dH0, sc.eps4, MA, MB);
+            const float pb0 = -0.5f * sc.lam * (ob1[k] - ob0[k]);      // Psi_b of interface q-2
+            const float pb1 = -0.5f * sc.lam * (ob2[k] - ob1[k]);      // Psi_b of interface q-3
+            GsB[k] = fmaf(-LA, pb0, GB0[k]);
+            GB0[k] = fmaf(1.f + LA - LB, pb0, GB1[k]);
+            GB1[k] = LB * pb0;
+            HsB[k] = fmaf(-MA, pb1, HB0[k]);
+            HB0[k] = fmaf(-1.f + MA - MB, pb1, HB1[k]);
+            HB1[k] = MB * pb1;
+            Gs[k] = Gs0[k]; dGs[k] = dG0; Hs[k] = Hs0[k]; dHs[k] = dH0;
+        }
+        // ---- cell m = q-3
+        const float vsb = -0.5f * sc.lam * (psC * obq4 - psA * ob1[5]);
+        const float psb = -0.5f * sc.lam * ob2[5] * (vsA - vsC);
+        float usb[6];
+        gamM = 0.f;
+        prim_de_vjp(us2, sc, GsB, HsB, vsb, psb, 0.f, usb, gamM);
+        gb = 0.f;
+        if (HAS_G) {
+            const float kg = sc.kap * gM;
+            usb[0] = fmaf(kg, ob2[1], usb[0]);
+            usb[1] = fmaf(kg, ob2[4], usb[1]);
+        }
+        float acc[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) acc[k] = ob2[k] + usb[k];
+        const float qsb = ob2[5] + usb[5];
+        if (HAS_G) {
+            const float hk = 0.5f * sc.kap * gM;
+            acc[0] = fmaf(hk, usb[1], acc[0]);
+            acc[1] = fmaf(hk, usb[4], acc[1]);
+            const float tB = us2[0] * ob2[1] + us2[1] * ob2[4];
+            const float tAg = uM[0] * usb[1] + uM[1] * usb[4];
+            gb = sc.kap * fmaf(0.5f, tAg, tB);
+        }
+        // ---- cell r = q-4: stage-A transpose
+        float Gb[6], Hb[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float Db = -0.25f * sc.lam * (usbR[k] - usb[k]);
+            Gb[k] = Db;
+            Hb[k] = -DbR[k];
+            DbR[k] = Db;
+        }
+        const float tA3 = p3 * usb[5];
+        const float vb = -0.25f * sc.lam * (tA5 - tA3);
+        const float pb = -0.25f * sc.lam * usbR[5] * (v3 - v5);
+        gamR = 0.f;
+        prim_de_vjp(uR, sc, Gb, Hb, vb, pb, qsbR, ub, gamR);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            ub[k] += accR[k];
+            accR[k] = acc[k];
+        }
+        qsbR = qsb;
+        // ---- rotate
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            usbR[k] = usb[k];
+            us2[k] = us1[k]; us1[k] = us0[k];
+            G1[k] = G0[k];
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k) U1[k] = u0[k];
+        U1[5] = qs0;
+        g1 = g0;
+        v5 = v4; v4 = v3; v3 = v2; v2 = v1; v1 = v0;
+        p3 = p2; p2 = p1; p1 = p0;
+        tA5 = tA4; tA4 = tA3;
+        vsC = vsB; vsB = vsA; vsA = vs0;
+        psC = psB; psB = psA; psA = ps0;
+        obq4 = ob2[5];
+    }
+};
+
+template <int DIR, bool HAS_G, int EPS>
+__global__ void __launch_bounds__(128, 2) sweep_march_adj_de_kernel(Ptr6m in, const float* __restrict__ gfield, Ptr6m cot_out,
+                                                                    MPtr6m cot_in, float* __restrict__ gbar, double* scal,
+                                                                    SweepConst sc, int S) {
+    constexpr int HALO = 4, NF = HAS_G ? 13 : 12, OB = HAS_G ? 7 : 6;
+    extern __shared__ float ring[];              // [RING][NF][nthr]: (u, q) (6), g, ob (6) of one cell per stage
+    __shared__ float s_red[96];
+    constexpr int nthr = NTHR;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    const int N = sc.N;
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int o = blockIdx.y * blockDim.y + threadIdx.y;
+    const int p0 = blockIdx.z * S;
+    const int len = min(S, N - p0);
+    const int stride = DIR == 1 ? N : N * N;
+    const int base = DIR == 1 ? o * N * N + x : o * N + x;
+    const int niter = len + 2 * HALO;
+    AxisPos ld;
+    ld.set(p0 - HALO, N, base, stride);
+    int off_m = base + (p0 - 1) * stride;
+    int off_r = base + (p0 - 1) * stride;
+    float* const my = ring + tid;
+    auto issue = [&](int it) {
+        float* dst = my + (it & (RING - 1)) * NF * nthr;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            cp_async4(dst + k * nthr, in.p[k] + ld.off);
+            cp_async4(dst + (OB + k) * nthr, cot_out.p[k] + ld.off);
+        }
+        if (HAS_G) cp_async4(dst + 6 * nthr, gfield + ld.off);
+        ld.next(N, base, stride);
+    };
+#pragma unroll
+    for (int st = RING - 4; st < RING; ++st)
+#pragma unroll
+        for (int k = 0; k < NF; ++k) my[(st * NF + k) * nthr] = k < 6 ? 1.f : 0.f;
+#pragma unroll
+    for (int it = 0; it < PF_ADJ; ++it) {
+        if (it < niter) issue(it);
+        cp_async_commit();
+    }
+    AdjPipeDE<HAS_G, EPS> pipe;
+    pipe.init();
+    float gacc = 0.f;
+#pragma unroll 1
+    for (int i = 0; i < niter; ++i) {
+        if (i + PF_ADJ < niter) issue(i + PF_ADJ);
+        cp_async_commit();
+        cp_async_wait<PF_ADJ>();
+        const float* s0 = my + (i & (RING - 1)) * NF * nthr;
+        const float* s1 = my + ((i - 1) & (RING - 1)) * NF * nthr;
+        const float* s2 = my + ((i - 2) & (RING - 1)) * NF * nthr;
+        const float* s3 = my + ((i - 3) & (RING - 1)) * NF * nthr;
+        const float* s4 = my + ((i - 4) & (RING - 1)) * NF * nthr;
+        float u0[6], ob0[6], ob1[6], ob2[6], uM[6], uR[6], g0 = 0.f, gM = 0.f;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            u0[k] = s0[k * nthr];
+            ob0[k] = s1[(OB + k) * nthr];
+            ob1[k] = s2[(OB + k) * nthr];
+            ob2[k] = s3[(OB + k) * nthr];
+            uM[k] = s3[k * nthr];
+            uR[k] = s4[k * nthr];
+        }
+        if (HAS_G) { g0 = s0[6 * nthr]; gM = s3[6 * nthr]; }
+        float ub[6], gb, gamM, gamR;
+        pipe.push(u0, g0, ob0, ob1, ob2, uM, gM, uR, sc, ub, gb, gamM, gamR);
+        if (i >= 7) {
+            off_m += stride;
+            if (i < len + 7) {
+                gacc += gamM;
+                if (HAS_G) gbar[off_m] = gb;
+            }
+        }
+        if (i >= 8) {
+            off_r += stride;
+            gacc += gamR;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) cot_in.p[k][off_r] = ub[k];
+        }
+    }
+    block_sum3_to_global(0.f, 0.f, gacc, scal, s_red);
+}
+
 // ----------------------------------------------------------------------------------------------- launchers ----
 #define MARCH_LAUNCH(kern, grid, block, sm, stream, ...)                                                        \
     do {                                                                                                        \
@@ -637,6 +835,36 @@ int launch_sweep_march_de(dh_ctx* c, int d, const float* const in[6], const floa
     for (int k = 0; k < 6; ++k) { pin.p[k] = in[k]; pout.p[k] = out[k]; }
     if (d == 1) DH_TRY(march_fwd_de_dispatch<1>(c, grid, block, pin, g, pout, cmax, sc, S, eps));
     else DH_TRY(march_fwd_de_dispatch<2>(c, grid, block, pin, g, pout, cmax, sc, S, eps));
+    DH_CUDA(cudaGetLastError());
+    return DH_OK;
+}
+
+template <int DIR, bool HAS_G>
+static int march_adj_de_dispatch(dh_ctx* c, dim3 grid, dim3 block, const Ptr6m& pin, const float* g, const Ptr6m& pco,
+                                 const MPtr6m& pci, float* gbar, double* scal, const SweepConst& sc, int S, int eps_mode) {
+    const size_t sm = (size_t)RING * (HAS_G ? 13 : 12) * block.x * block.y * sizeof(float);
+    if (eps_mode == 1) MARCH_LAUNCH((sweep_march_adj_de_kernel<DIR, HAS_G, 1>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+    else if (eps_mode == 2) MARCH_LAUNCH((sweep_march_adj_de_kernel<DIR, HAS_G, 2>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+    else MARCH_LAUNCH((sweep_march_adj_de_kernel<DIR, HAS_G, 0>), grid, block, sm, c->stream, pin, g, pco, pci, gbar, scal, sc, S);
+    return DH_OK;
+}
+
+// y / z adjoint sweep of the dual-energy variant without the cotangents of Dtau and kappa; pointers already permuted
+int launch_sweep_march_de_vjp(dh_ctx* c, int d, const float* const in[6], const float* g, const float* const cot_out[6],
+                              float* const cot_in[6], float* gbar, double* scal, const SweepConst& sc) {
+    const int N = c->N;
+    const int S = march_segment(N, c->tune_march_s_adj, 4);
+    const dim3 block = march_block(N);
+    const dim3 grid(N / block.x, N / block.y, (N + S - 1) / S);
+    const int eps = c->opt.lim_eps > 1e-18 ? 1 : (c->opt.lim_eps > 0.0 ? 2 : 0);
+    Ptr6m pin, pco; MPtr6m pci;
+    for (int k = 0; k < 6; ++k) { pin.p[k] = in[k]; pco.p[k] = cot_out[k]; pci.p[k] = cot_in[k]; }
+    int rc;
+    if (d == 1) rc = g ? march_adj_de_dispatch<1, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps)
+                       : march_adj_de_dispatch<1, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    else rc = g ? march_adj_de_dispatch<2, true>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps)
+                : march_adj_de_dispatch<2, false>(c, grid, block, pin, g, pco, pci, gbar, scal, sc, S, eps);
+    DH_TRY(rc);
     DH_CUDA(cudaGetLastError());
     return DH_OK;
 }
