@@ -239,7 +239,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-de-leg", action="store_true", help="skip the dual-energy leg of the default run")
     ap.add_argument("--dual-energy", action="store_true",
-                    help="run the dual-energy variant (DESIGN.md section 19: six gas fields, chain kernels on all axes); "
+                    help="run the dual-energy variant (DESIGN.md section 19: six gas fields); "
                          "recorded in config, not the headline configuration")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="dh_tune knob for A/B runs (e.g. part_pipe=0); recorded in config")
@@ -558,8 +558,8 @@ def main():
         ms3, ms3f, _, _, dp3, _ = timed_window(ctx3, st_de, R["k0"], 1)
         de_leg = {"value": job_throughput(world, n3, K, ms3), "unit": UNIT, "ms_per_step": ms3 / K,
                   "fwd_ms_per_step": ms3f / K, "window": wkey, "dual_eta": 1e-3, "dgamma": dp3.dgamma,
-                  "note": "dh_options.dual_energy = 1: six gas fields; y/z forward on the marching pipeline, adjoint on the "
-                          "chain kernels (not tuned)"}
+                  "note": "dh_options.dual_energy = 1: six gas fields; y/z sweeps and their adjoints on the marching "
+                          "pipelines, x on the chain kernels"}
         ctx3.close()
         del st_de
 

@@ -192,8 +192,9 @@ int dh_debug_poison(dh_ctx* ctx, int level);
  *           onto the context's side stream beside them (default 1);
  *   "prime": 0 makes every step of dh_run initialise its own Poisson source instead of letting the previous step's last
  *           sweep write it (default 1; bit-identical either way);
- *   "de_march": 0 routes the y/z forward sweeps of the dual-energy variant through the chain tile kernels instead of
- *           the marching pipeline (default 1; 2.6 times slower, same numbers to rounding);
+ *   "de_march": 0 routes the y/z sweeps of the dual-energy variant (forward; adjoint when want_dsched = 0) through the
+ *           chain tile kernels instead of the marching pipelines (default 1; 2.0 - 2.6 times slower per sweep, same
+ *           numbers to rounding);
  *   "deposit_tile": 1 routes the deposit through a shared-memory tile per brick of 32 x 8 x 8 lattice sites (the A/B of
  *           profiles/r02.md: three times slower than the default run-aggregated RED; 2: the same tile in 32-bit fixed
  *           point; default 0).

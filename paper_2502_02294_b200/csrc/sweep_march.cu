@@ -742,7 +742,7 @@ __global__ void __launch_bounds__(128, 2) sweep_march_adj_de_kernel(Ptr6m in, co
 // ----------------------------------------------------------------------------------------------- launchers ----
 #define MARCH_LAUNCH(kern, grid, block, sm, stream, ...)                                                        \
     do {                                                                                                        \
-        if ((sm) > 48 * 1024)                                                                                   \
+        if ((sm) + 2048 > 48 * 1024)             /* static shared memory counts against the 48 KB default too */       \
             DH_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sm)));        \
         kern<<<grid, block, sm, stream>>>(__VA_ARGS__);                                                         \
     } while (0)

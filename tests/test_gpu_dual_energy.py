@@ -97,7 +97,10 @@ def test_de_sweep_matches_oracle(api, torch_, DE, W, N, d, with_g):
 @pytest.mark.parametrize("N", [32, 64])
 @pytest.mark.parametrize("d", [0, 1, 2])
 @pytest.mark.parametrize("with_g", [True, False])
-def test_de_sweep_vjp_matches_oracle(api, torch_, DE, W, N, d, with_g):
+@pytest.mark.parametrize("want_dsched", [1, 0])
+def test_de_sweep_vjp_matches_oracle(api, torch_, DE, W, N, d, with_g, want_dsched):
+    """want_dsched = 1: chain kernels with the cotangents of lam and kap; want_dsched = 0: x on the chain kernel, y / z on the
+    marching pipeline (gamma cotangent only)."""
     g6, eta = _state6(W, N, 300 + d)
     rng = np.random.default_rng(19)
     g = (0.3 * rng.standard_normal((N, N, N))).astype(np.float32) if with_g else None
@@ -106,7 +109,7 @@ def test_de_sweep_vjp_matches_oracle(api, torch_, DE, W, N, d, with_g):
     eT = g6[4] / g6[0] - 0.5 * np.sum(g6[1:4].astype(np.float64) ** 2, axis=0) / g6[0].astype(np.float64) ** 2
     e_floor = float(np.quantile(eT, 0.05))
     ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=e_floor, dual_energy=1,
-                      dual_eta=eta)
+                      dual_eta=eta, want_dsched=want_dsched)
     cin, gb, sc = ctx.dh_sweep_de_vjp(d, _gpu(torch_, g6), _gpu(torch_, g) if with_g else None, lam, kap, _gpu(torch_, cot))
     cin, sc = cin.cpu().numpy(), sc.cpu().numpy()
     rin, rgb, rsc = DE.sweep_vjp(g6, d, lam, kap, gamma, cot, g, e_floor=e_floor, eta=eta)
@@ -119,19 +122,20 @@ def test_de_sweep_vjp_matches_oracle(api, torch_, DE, W, N, d, with_g):
     assert e_trim < 2e-5 and e_q < 2e-5 and e_all < 5e-3
     if with_g:
         assert PT.rel_l2(gb.cpu().numpy(), rgb) < 1e-3
-    for k, key in ((0, "lam"), (1, "kap"), (2, "gamma")):
+    for k, key in ((0, "lam"), (1, "kap"), (2, "gamma"))[(0 if want_dsched else 2):]:
         assert abs(sc[k] - rsc[key]) < 1e-3 * max(abs(rsc[key]), np.sqrt(g6[0].size)), (key, sc[k], rsc[key])
     ctx.close()
 
 
-def test_de_hydro_run_and_reverse_match_oracle(api, torch_, DE, W):
+@pytest.mark.parametrize("want_dsched", [1, 0])
+def test_de_hydro_run_and_reverse_match_oracle(api, torch_, DE, W, want_dsched):
     """Static hydro-only run of 6 steps (one Strang cycle) with dual energy: dh_run / dh_run_vjp (snapshots, tapes with six
     fields) against the oracle's run and reverse pass."""
     N, gamma = 32, 1.5
     g6, eta = _state6(W, N, 400)
     lams = [0.05, 0.06, 0.04, 0.05, 0.055, 0.045]
     ctx = api.Context(N, float(N), gamma, n_part_side=0, static_mode=1, gravity_on=0, e_floor=1e-6, dual_energy=1,
-                      dual_eta=eta)
+                      dual_eta=eta, want_dsched=want_dsched)
     st = api.State(g6, np.zeros((6, 0), dtype=np.float32), 1.0)
     ctx.dh_run(st, np.ones(len(lams)), np.array(lams), 4)                 # static mode: dtau = dt, dx = 1 -> lam = dt
     ref, cm_ref = DE.hydro_run(g6, gamma, lams, e_floor=1e-6, eta=eta)

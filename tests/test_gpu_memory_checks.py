@@ -43,7 +43,7 @@ def _run_and_reverse(api, torch, ctx, gas, part, cfg, a_s, dt_s, stride, poison)
     return st.gas.clone(), st.part.clone(), ct.gas.clone(), ct.part.clone(), dp.as_dict()
 
 
-@pytest.mark.parametrize("case", ["hydro_only", "coupled", "coupled_recompute", "dual_energy"])
+@pytest.mark.parametrize("case", ["hydro_only", "coupled", "coupled_recompute", "dual_energy", "dual_energy_march"])
 def test_poisoned_scratch_changes_nothing(api, torch_, W, IC, case):
     cfg = W.scaled_config(0, 32, n_steps=7, a1=0.03)
     _, gas, part = IC.coupled_ic(W, cfg)
@@ -54,8 +54,8 @@ def test_poisoned_scratch_changes_nothing(api, torch_, W, IC, case):
         part = np.zeros((6, 0), dtype=np.float32)
     elif case == "coupled_recompute":
         tune = {"tape": 0, "gstore": 0}
-    elif case == "dual_energy":
-        kw = dict(dual_energy=1, dual_eta=1e-3)
+    elif case.startswith("dual_energy"):
+        kw = dict(dual_energy=1, dual_eta=1e-3, want_dsched=0 if case.endswith("march") else 1)
         vf, e0 = api.ic_factors_for(cfg)
         gas = np.concatenate([gas, (e0 * gas[0].astype(np.float64))[None].astype(np.float32)], axis=0)
     ctx = api.context_for(cfg, **kw)
