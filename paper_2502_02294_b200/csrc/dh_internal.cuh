@@ -96,7 +96,7 @@ struct dh_ctx {
     int tune_prime = 1;                               // 0: every step of dh_run initialises its Poisson source itself
     int tune_overlap = 1;                             // 0: kick_drift on the main stream, after which the sweeps start
     int tune_de_march = 1;                            // 0: dual-energy y/z forward sweeps on the chain tile kernels
-    int tune_deposit_tile = 0;                        // 1: shared-memory tile deposit (the A/B of profiles/r02_deposit_ab.md)
+    int tune_deposit_tile = 0;                        // 1: shared-memory tile deposit (the A/B of profiles/r02.md)
 
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans = false;

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(256) deposit_kernel(const float* __restrict__ 
 // TR cells) go straight to the mesh.  fp32 atomicAdd on shared memory compiles to an ATOMS.CAST.SPIN loop on sm_100
 // (compare-and-swap; SASS excerpt in profiles/), so every one of the 8 tile updates per particle is a retry loop under
 // contention, and the flush still issues (TBX+2TR)(TBY+2TR)(TBZ+2TR) / (TBX TBY TBZ) = 3.6 RED lanes per particle where the
-// run-aggregated kernel above issues 4 to 5 -- measured slower at 256^3 both early and late (profiles/r02_deposit_ab.md).
+// run-aggregated kernel above issues 4 to 5 -- measured slower at 256^3 both early and late (profiles/r02.md).
 constexpr int TBX = 32, TBY = 8, TBZ = 8, TR = 3;
 constexpr int TLX = TBX + 2 * TR, TLY = TBY + 2 * TR, TLZ = TBZ + 2 * TR;
 // FIXED = true: the tile holds 32-bit fixed-point sums (weights in units of m_p 2^-22; native ATOMS.ADD on integers)
@@ -260,7 +260,9 @@ __device__ __forceinline__ float wrap_pos(float x, float fN, float invN) {
 // (Tried and dropped, r02: depositing the NEW positions from this kernel inside dh_run, so that the next step starts with
 // its Poisson solve -- the REDs cost what they cost in a kernel of their own: kick_drift 231 -> 286 us, + 15 us to zero the
 // mesh, + the last sweep adding rho' - rho_bar by RED instead of storing it; forward 1.155 -> 1.154 ms/step early, 1.229 ->
-// 1.196 late, forward + VJP unchanged.)
+// 1.196 late, forward + VJP unchanged.  Persistent blocks with the next chunk's six fields prefetched into registers, the
+// adjoint's schedule: 246 - 300 us against 231 for 128 x 4 ... 256 x 4 threads x blocks per SM -- with 60 B per particle the
+// one-shot grid's 24 warps per SM already cover the two round trips, and the persistent loop only lowers occupancy.)
 constexpr int KD_T = 128;
 __global__ void __launch_bounds__(KD_T, 6) kick_drift_kernel(const float* __restrict__ gx, const float* __restrict__ gy,
                                                          const float* __restrict__ gz, const float* px, const float* py,

@@ -72,7 +72,8 @@ def test_poisoned_scratch_changes_nothing(api, torch_, W, IC, case):
         elif a.numel():                                           # cotangents: the same, amplified at the switches (R28)
             an, bn = a.double().cpu().numpy(), b.double().cpu().numpy()
             assert PT.rel_l2_trimmed(bn, an, frac=1e-2) < 1e-3 and PT.rel_l2(bn, an) < 5e-2
-    assert all(np.isfinite(v) for v in got[4].values())
+    # want_dsched = 0 leaves the cotangents of Dtau and kappa unset (NaN by contract, include/diffhydro.h)
+    assert all(np.isfinite(v) for k, v in got[4].items() if kw.get("want_dsched", 1) or k not in ("dDtau", "dkappa"))
     assert abs(got[4]["dgamma"] - ref[4]["dgamma"]) <= 1e-3 * abs(ref[4]["dgamma"]) + 1e-12
     # the single-step calls and the host-buffer chain after a poisoning of everything
     st = api.State(gas, part, cfg.a0)
