@@ -394,3 +394,64 @@ def test_config2_full_run_gradient_with_dual_energy(api, torch_, O, DE, W, IC):
     assert e_f < 5e-3 and e_all < 4e-3 and e_trim < 1.5e-3 and e_p < 8e-3
     assert abs(dp.dgamma / rdg - 1) < 5e-4
     ctx.close()
+
+
+def test_config3_late_step_with_dual_energy_at_256(api, torch_, O, DE, W):
+    """The dual-energy variant in the launch configuration bench.py times (config 3, 256^3 cells and particles, late epoch).
+    The GPU runs the config's own initial state through 180 of its 200 steps with dual_energy = 1; from that fp32 state
+    (i) the step's VJP for the loss cotangent 2 (rho - rho_target) through the marching y/z adjoints (want_dsched = 0, what
+    the bench times) against the chain-tile adjoints (want_dsched = 1, the route the small-size tests pin to the oracle):
+    the same numbers up to rounding order; (ii) one coupled step against the oracle's composition on every cell and
+    particle."""
+    cfg = W.CONFIGS[3]
+    N, K0, eta = cfg.N, 180, 1e-3
+    delta = W.gaussian_field(N, cfg.box, cfg.seed, cfg.rms_delta).astype(np.float32)
+    target = (cfg.f_b * (1.0 + W.gaussian_field(N, cfg.box, cfg.target_seed, cfg.rms_delta))).astype(np.float32)
+    a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
+    vf, e0 = api.ic_factors_for(cfg)
+    ctx = api.context_for(cfg, dual_energy=1, dual_eta=eta, want_dsched=0)
+    st = ctx.dh_ic_zeldovich(_gpu(torch_, delta), cfg.a0, vf, e0)
+    del delta
+    assert st.gas.shape[0] == 6
+    ctx.dh_run(st, a_s[1:K0 + 1], dt_s[:K0], 0)
+    g6, p = st.gas.cpu().numpy(), st.part.cpu().numpy()
+    g64 = g6.astype(np.float64)
+    on_q = float(np.mean(g64[4] - 0.5 * np.sum(g64[1:4] ** 2, axis=0) / g64[0] <= eta * g64[4]))   # pressure comes from q there
+    del g64
+    start = api.State(g6, p, st.a, st.dt_prev, st.step)
+    # ---- (i) first (the oracle's 256^3 arrays are not alive yet): marching against chain-tile adjoints
+    cots = []
+    for want in (0, 1):
+        c2 = ctx if want == 0 else api.context_for(cfg, dual_energy=1, dual_eta=eta, want_dsched=1)
+        s2 = start.clone()
+        c2.dh_step(s2, dt_s[K0], a_s[K0 + 1])
+        cg = torch_.zeros_like(s2.gas)
+        c2.dh_data_term(0, s2.gas, _gpu(torch_, target), None, 1.0, 1.0, cg, want_loss=False)
+        co = api.Cot(cg, torch_.zeros_like(s2.part))
+        dp = c2.dh_step_vjp(start.clone(), dt_s[K0], a_s[K0 + 1], co, co)
+        cots.append((co.gas.cpu().numpy(), co.part.cpu().numpy(), dp.dgamma))
+        if want == 1:
+            c2.close()
+        del s2, cg, co
+    (g_m, p_m, dg_m), (g_c, p_c, dg_c) = cots
+    e_all, e_trim, e_p = PT.rel_l2(g_m, g_c), PT.rel_l2_trimmed(g_m, g_c, frac=1e-3), PT.rel_l2(p_m, p_c)
+    print(f"config3 + dual energy, step {K0} VJP, marching vs chain adjoints: gas {e_all:.2e} (all but the worst 1e-3: {e_trim:.2e}), "
+          f"particles {e_p:.2e}, dgamma {dg_m:.6g} vs {dg_c:.6g}")
+    assert np.all(np.isfinite(g_m)) and np.all(np.isfinite(p_m))
+    assert e_trim < 1e-4 and e_all < 2e-2 and e_p < 1e-3 and abs(dg_m - dg_c) < 2e-3 * abs(dg_c)
+    del cots, g_m, p_m, g_c, p_c
+    # ---- (ii) one step against the oracle
+    P = PT.oracle_params(O, cfg)
+    ref_g, ref_p, _ = DE.coupled_step(O, P, g6, p, a_s[K0], a_s[K0 + 1], dt_s[K0], dt_s[K0 - 1], K0, eta=eta)
+    ctx.dh_step(st, dt_s[K0], a_s[K0 + 1])
+    got = st.gas.cpu().numpy()
+    e = _err6(got, ref_g)
+    e.update(PT.part_err(st.part.cpu().numpy(), ref_p, N))
+    # a cell whose selection flips between fp32 and fp64 takes the other energy: a value jump (measured: 4e-6 of the cells,
+    # up to 6e-4 of the maximum in the conserved fields and 1e-2 in q, which is what the two branches differ in) -- counted
+    bad = float(np.mean(np.abs(got[4] - ref_g[4]) > 3e-5 * np.max(np.abs(ref_g[4]))))
+    print(f"config3 + dual energy, step {K0} vs oracle at 256^3: {e}; cells off by more than 3e-5 of the maximum: {bad:.2e}; "
+          f"cells on q: {on_q:.3f}")
+    assert bad < 1e-4, bad
+    assert max(v for k, v in e.items() if k != "q") < 5e-3 and e["q"] < 5e-2, e
+    ctx.close()
