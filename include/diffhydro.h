@@ -172,6 +172,22 @@ int dh_sync(dh_ctx* ctx);
  * gravity, Eq. 8): out (HOST, 8 doubles) = (sum rho, sum m_x, sum m_y, sum m_z, sum eps, m_p sum w_x, m_p sum w_y,
  * m_p sum w_z), fp64 accumulation on the device.  Synchronises the stream. */
 int dh_conserved_sums(dh_ctx* ctx, const dh_state* state, double* out);
+/* The same eight sums for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): no context (dh_init allocates), no cudaMalloc / cudaFree / allocating library routine, no synchronisation.
+ *   gas[5]   DEVICE, n_cells floats each: rho, m_x, m_y, m_z, eps;   w[3]  DEVICE, n_part floats each (may be NULL when
+ *   n_part = 0);   m_p  particle mass;   out  DEVICE, 8 doubles, written by the kernel (same order as dh_conserved_sums);
+ *   cuda_stream  a cudaStream_t or NULL: one memset node + one kernel are enqueued on it, nothing else happens.
+ * The per-block partial sums live in a static device array of 512 KiB + 8 B (csrc/noalloc.cu) that every GPU which loads
+ * the library holds until the process exits; it serves at most DH_NOALLOC_MAX_ELEMS cells and as many particles (512^3,
+ * the largest configuration of BASELINE.json): more is DH_ERR_INVALID with a message naming the limit, as are null
+ * pointers and n_cells <= 0.  The first call on each device looks the array's address up (cudaGetSymbolAddress, with that
+ * device current): make it outside a stream capture.  Every call on a device shares the array: calls that overlap on the
+ * GPU (different streams, or graphs replayed concurrently) race -- serialise them.  The additions are done in an order
+ * fixed by the sizes alone (block partials, then the last block adds them in block order): bit-identical from call to
+ * call, unlike dh_conserved_sums, whose blocks meet in fp64 atomics. */
+#define DH_NOALLOC_MAX_ELEMS 134217728LL
+int dh_conserved_sums_noalloc(const float* const gas[5], int64_t n_cells, const float* const w[3], int64_t n_part, double m_p,
+                              double* out, void* cuda_stream);
 /* Debug aid (compute-sanitizer's initcheck is not available everywhere): fill the context's device buffers with NaN
  * (all-ones bytes).  level 0: pure scratch only (Poisson source and spectra, g' scratch, sweep ping-pong sets, adjoint
  * scratch, the in-segment states and tapes of the reverse pass) -- safe between dh_run and dh_run_vjp; level 1: also what

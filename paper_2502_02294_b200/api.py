@@ -30,7 +30,8 @@ EXPORTS = ["dh_init", "dh_free", "dh_step", "dh_step_vjp", "dh_run", "dh_run_vjp
            "dh_poisson_vjp", "dh_kick_drift", "dh_profile_enable", "dh_profile_categories", "dh_profile_name",
            "dh_profile_read", "dh_reserve", "dh_tune", "dh_ic_zeldovich", "dh_ic_zeldovich_vjp", "dh_data_term", "dh_power_spectrum",
            "dh_power_spectrum_vjp", "dh_subgrid_step", "dh_subgrid_step_vjp", "dh_get_step_dparams",
-           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors", "dh_sweep_de", "dh_sweep_de_vjp", "dh_debug_poison", "dh_conserved_sums"]
+           "dh_chain_cosmology", "dh_value_and_grad_host", "dh_ic_factors", "dh_sweep_de", "dh_sweep_de_vjp", "dh_debug_poison", "dh_conserved_sums",
+           "dh_conserved_sums_noalloc"]
 
 
 class DhError(RuntimeError):
@@ -91,6 +92,8 @@ _lib.dh_free.argtypes = [C.c_void_p]
 _lib.dh_sync.argtypes = [C.c_void_p]
 _lib.dh_debug_poison.argtypes = [C.c_void_p, C.c_int]
 _lib.dh_conserved_sums.argtypes = [C.c_void_p, C.POINTER(dh_state), _dp]
+_lib.dh_conserved_sums_noalloc.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.POINTER(C.c_void_p), C.c_int64, C.c_double,
+                                          C.c_void_p, C.c_void_p]
 _lib.dh_step.argtypes = [C.c_void_p, C.POINTER(dh_state), C.c_double, C.c_double, C.c_void_p]
 _lib.dh_step_vjp.argtypes = [C.c_void_p, C.POINTER(dh_state), C.c_double, C.c_double, C.POINTER(dh_cot),
                              C.POINTER(dh_cot), C.POINTER(dh_dparams)]
@@ -468,6 +471,29 @@ class Context:
         _check(_lib.dh_ic_zeldovich_vjp(self._h, delta_init.data_ptr(), float(vel_factor), float(e_tilde0), C.byref(cs),
                                         grad.data_ptr()), "dh_ic_zeldovich_vjp")
         return grad
+
+
+DH_NOALLOC_MAX_ELEMS = 134217728
+
+
+def dh_conserved_sums_noalloc(gas: torch.Tensor, w: torch.Tensor | None, m_p: float, out: torch.Tensor, stream=None):
+    """include/diffhydro.h: the eight conserved sums without a context and without any allocation.  gas: (>= 5, ...) fp32
+    CUDA tensor (fields 0..4 are summed), w: (3, n_part) fp32 CUDA tensor of particle velocities or None, out: 8 fp64 on
+    the device, written by the kernel on `stream` (default: torch's current stream).  Marshalling only; asynchronous."""
+    assert gas.is_cuda and gas.dtype == torch.float32 and gas.is_contiguous() and gas.shape[0] >= 5
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 8
+    n_cells = gas[0].numel()
+    g = (C.c_void_p * 5)(*[gas[k].data_ptr() for k in range(5)])
+    n_part = 0 if w is None else int(w.shape[1])
+    wp = None
+    if n_part:
+        assert w.is_cuda and w.dtype == torch.float32 and w.is_contiguous() and w.shape[0] == 3
+        wp = (C.c_void_p * 3)(*[w[k].data_ptr() for k in range(3)])
+    stream = stream if stream is not None else torch.cuda.current_stream(gas.device)
+    with torch.cuda.device(gas.device):
+        _check(_lib.dh_conserved_sums_noalloc(g, n_cells, wp, n_part, float(m_p), C.c_void_p(out.data_ptr()),
+                                              C.c_void_p(stream.cuda_stream)), "dh_conserved_sums_noalloc")
+    return out
 
 
 def dh_schedule_lna(a0, a1, n, H0=100.0, Omega_m=1.0, Omega_b=0.16, Omega_L=0.0):

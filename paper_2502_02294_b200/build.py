@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdiffhydro.so")
-SOURCES = ["api.cu", "sweep.cu", "sweep_march.cu", "sweep_de.cu", "pm.cu", "fft.cu", "ic.cu", "subgrid.cu"]
+SOURCES = ["api.cu", "sweep.cu", "sweep_march.cu", "sweep_de.cu", "pm.cu", "fft.cu", "ic.cu", "subgrid.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "dh_internal.cuh"), os.path.join(CSRC, "sweep_common.cuh"), os.path.join(CSRC, "async_copy.cuh"), os.path.join(HERE, "..", "include", "diffhydro.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "--use_fast_math=false", "-Xptxas", "-v"]
