@@ -53,6 +53,10 @@ FWD_BYTES = 264        # forward coupled step: 8 + 16 + 80 (Pois
 FWD_BYTES_NOG = 120    # hydro only: 3 x 40
 BYTES_PER_CELL_NOG = {"sweep_x": 40, "sweep_y": 40, "sweep_z": 40, "sweep_x_adj": 60, "sweep_y_adj": 60,
                       "sweep_z_adj": 60, "copy": 40}
+# --dual-energy: the sixth field in and out of every sweep (+8), its value and two cotangents in
+# the adjoints (+12), one more field in a state copy (+8)
+BYTES_PER_CELL_DE_EXTRA = {"sweep_x": 8, "sweep_y": 8, "sweep_z": 8, "sweep_x_adj": 12, "sweep_y_adj": 12,
+                           "sweep_z_adj": 12, "copy": 8}
 
 
 def measured_peak():
@@ -375,6 +379,8 @@ def main():
         kernels, model_bytes = {}, 0.0
         for name, (ms, cnt) in prof.items():
             bpc = (BYTES_PER_CELL_NOG if nog and name in BYTES_PER_CELL_NOG else BYTES_PER_CELL)[name]
+            if args.dual_energy:
+                bpc += BYTES_PER_CELL_DE_EXTRA.get(name, 0)
             gbs = bpc * n3 * cnt / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
             kernels[name] = {"ms_per_step": ms / K, "launches": cnt, "avg_us": 1e3 * ms / cnt, "bytes_per_cell": bpc,
                              "GBps": gbs, "frac": gbs / peak}
