@@ -200,7 +200,11 @@ int dh_debug_poison(dh_ctx* ctx, int level);
  *           the steps of the segment being reversed (13 N^3 floats per step of a segment; default 1, falls back to
  *           recomputation by itself when the device cannot hold them);
  *   "gstore": 0 makes a checkpointed dh_run NOT keep every step's g' (3 N^3 floats per step of the run) for
- *           dh_run_vjp, which then repeats deposit + Poisson solve in the segment re-run (default 1, same fallback).
+ *           dh_run_vjp, which then repeats deposit + Poisson solve in the segment re-run (default 1, same fallback);
+ *   "pstore": 0 makes a checkpointed dh_run NOT keep the particles entering every step (6 n_part floats per step of the
+ *           run; its kick + drift then writes the next step's slot directly, no copy) for dh_run_vjp, whose segment re-run
+ *           then repeats the particle update (default 1; taken only while the device keeps room for the snapshots,
+ *           in-segment states, tapes and adjoint scratch the reverse pass still has to allocate, else the same fallback);
  *   "own_fft": 0 routes the Poisson solve through cuFFT (1 R2C + multiply kernel + 3 C2R) instead of the library's own
  *           FFT passes fused with the Green multiply (default 1 when grid_n is a power of two); the cuFFT plans are
  *           made by this call when they do not exist yet (DH_ERR_CUFFT / DH_ERR_OOM);

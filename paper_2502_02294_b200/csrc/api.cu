@@ -80,14 +80,14 @@ static int ensure_adjoint_scratch(dh_ctx* c) {
 
 static size_t state_floats(const dh_ctx* c) { return (size_t)(c->nc * c->n3 + 6 * c->np); }
 
-static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st) {
+static int snapshot_store(dh_ctx* c, Snapshot& s, const dh_state* st, float* const* part_src = nullptr) {
     if (!s.buf) DH_TRY(dev_alloc(c, (void**)&s.buf, state_floats(c) * sizeof(float)));
     Prof prof(c, PROF_COPY);
     const G6 g(*st);
     for (int k = 0; k < c->nc; ++k)
         DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)k * c->n3, g.p[k], c->n3 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     for (int k = 0; k < 6 && c->np > 0; ++k)
-        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)c->nc * c->n3 + (size_t)k * c->np, st->part[k], c->np * sizeof(float),
+        DH_CUDA(cudaMemcpyAsync(s.buf + (size_t)c->nc * c->n3 + (size_t)k * c->np, part_src ? part_src[k] : st->part[k], c->np * sizeof(float),
                                 cudaMemcpyDeviceToDevice, c->stream));
     s.a = st->a; s.dt_prev = st->dt_prev; s.step = st->step;
     return DH_OK;
@@ -141,6 +141,43 @@ static bool ensure_gstore(dh_ctx* c, int n_steps) {
             return false;
         }
         for (int d = 0; d < 3; ++d) g.gp[d] = g.buf + (size_t)d * c->n3;
+    }
+    return true;
+}
+
+// Per-step store of the particles (6 n_part floats per step of the run): dh_run's kick + drift of step k writes straight
+// into the slot of step k + 1 (no copy; the caller's arrays get the final particles from the last step), so the segment
+// re-run of the reverse pass has no particle update left to repeat.  All or nothing, and only when the device keeps room
+// for what the reverse pass still has to allocate (snapshots, in-segment states, tapes, adjoint scratch): losing the
+// tapes to this store would cost more than it saves.
+static bool ensure_pstore(dh_ctx* c, int n_steps, int stride) {
+    if (!c->tune_pstore || c->np <= 0 || n_steps < 2 || stride <= 0) return false;
+    const size_t bytes = (size_t)6 * c->np * sizeof(float);
+    if ((int)c->pstore.size() < n_steps) c->pstore.resize(n_steps);
+    size_t missing = 0;
+    for (int i = 1; i < n_steps; ++i) missing += c->pstore[i].buf ? 0 : 1;
+    if (missing > 0) {
+        const size_t mesh = (size_t)c->n3 * sizeof(float), state = state_floats(c) * sizeof(float);
+        const int in_seg = stride < n_steps ? stride : n_steps, nseg = (n_steps + stride - 1) / stride;
+        size_t later = c->adj_alloc ? 0 : (size_t)(3 * c->nc + 3) * mesh;
+        for (int i = 0; i < nseg; ++i) later += (i < (int)c->snaps.size() && c->snaps[i].buf) ? 0 : state;
+        for (int i = 1; i < in_seg; ++i) later += (i < (int)c->seg.size() && c->seg[i].buf) ? 0 : state;
+        if (c->tune_tape)
+            for (int i = 0; i < in_seg; ++i) later += (i < (int)c->tapes.size() && c->tapes[i].buf) ? 0 : (size_t)(3 + 2 * c->nc) * mesh;
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return false; }
+        if (free_b < missing * bytes + later + ((size_t)1 << 30)) return false;
+    }
+    for (int i = 1; i < n_steps; ++i) {
+        PartStore& ps = c->pstore[i];
+        if (ps.buf) continue;
+        if (dev_alloc(c, (void**)&ps.buf, bytes) != DH_OK) {
+            for (auto& t : c->pstore) { dev_free(c, t.buf, bytes); t.buf = nullptr; }
+            c->pstore.clear();
+            set_error("");
+            return false;
+        }
+        for (int k = 0; k < 6; ++k) ps.p[k] = ps.buf + (size_t)k * c->np;
     }
     return true;
 }
@@ -431,6 +468,7 @@ int dh_free(dh_ctx* c) {
     for (auto& s : c->seg) cudaFree(s.buf);
     for (auto& t : c->tapes) cudaFree(t.buf);
     for (auto& t : c->gstore) cudaFree(t.buf);
+    for (auto& t : c->pstore) cudaFree(t.buf);
     for (auto e : c->prof_ev) cudaEventDestroy(e);
     if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); }
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
@@ -481,6 +519,7 @@ int dh_tune(dh_ctx* c, const char* key, int value) {
     else if (!strcmp(key, "march_s_adj")) c->tune_march_s_adj = value;
     else if (!strcmp(key, "tape")) c->tune_tape = value;
     else if (!strcmp(key, "gstore")) c->tune_gstore = value;
+    else if (!strcmp(key, "pstore")) c->tune_pstore = value;
     else if (!strcmp(key, "own_fft")) {
         if (!value && c->opt.gravity_on) DH_TRY(ensure_cufft_plans(c));
         c->tune_own_fft = value;
@@ -536,6 +575,7 @@ int dh_debug_poison(dh_ctx* c, int level) {
     if (level >= 1) {
         for (auto& s : c->snaps) DH_TRY(fill(s.buf, state_bytes));
         for (auto& g : c->gstore) DH_TRY(fill(g.buf, 3 * mesh));
+        for (auto& t : c->pstore) DH_TRY(fill(t.buf, (size_t)6 * c->np * sizeof(float)));
         DH_TRY(fill(c->cmax_log, (size_t)3 * c->cmax_cap * sizeof(float)));
         c->run_valid = false;
     }
@@ -622,12 +662,17 @@ int dh_run(dh_ctx* c, dh_state* st, const double* a_sched, const double* dt_sche
     c->run_dt.assign(dt_sched, dt_sched + n_steps);
     c->run_n = n_steps; c->run_stride = stride;
     c->run_gstore = stride > 0 && ensure_gstore(c, n_steps);
+    c->run_pstore = ensure_pstore(c, n_steps, stride);
     for (int k = 0; k < n_steps; ++k) {
-        if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st));
+        // with the particle store, step k reads the slot of step k and writes the slot of step k + 1; the first step reads
+        // the caller's arrays and the last one writes them
+        float* const* pin = (c->run_pstore && k > 0) ? c->pstore[k].p : st->part;
+        float* const* pout = (c->run_pstore && k + 1 < n_steps) ? c->pstore[k + 1].p : st->part;
+        if (stride > 0 && k % stride == 0) DH_TRY(snapshot_store(c, c->snaps[k / stride], st, pin));
         const StepScalars s = step_scalars(c->cosmo, st->a, a_sched[k], dt_sched[k], st->dt_prev);
         const bool can_prime = c->opt.gravity_on && c->opt.hydro_on && c->tune_prime && c->nc == 5;
         const G6 g(*st);
-        DH_TRY(step_arrays(c, g.p, st->part, g.p, st->part, s, st->step, c->cmax_log + 3 * k, nullptr, true,
+        DH_TRY(step_arrays(c, g.p, pin, g.p, pout, s, st->step, c->cmax_log + 3 * k, nullptr, true,
                            c->run_gstore ? c->gstore[k].gp : nullptr, false, can_prime && k > 0,
                            can_prime && k + 1 < n_steps));
         st->a = c->cosmo.static_mode ? 1.0 : a_sched[k];
@@ -670,6 +715,7 @@ int dh_reserve(dh_ctx* c, int n_steps, int stride) {
     DH_TRY(ensure_adjoint_scratch(c));
     ensure_tapes(c, in_seg);
     ensure_gstore(c, n_steps);
+    ensure_pstore(c, n_steps, stride);
     c->run_valid = false;
     return DH_OK;
 }
@@ -723,15 +769,19 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             StepTape* tape = taped ? &c->tapes[k - k0] : nullptr;
             float* const* gk = c->run_gstore ? c->gstore[k].gp : nullptr;
             const G6 gin(in);
+            // the particles entering step k: kept by dh_run (then the re-run has no particle update to repeat), else the
+            // in-segment state's own
+            float* const* pin = (c->run_pstore && k > k0) ? c->pstore[k].p : in.part;
             if (last) {
-                DH_TRY(step_arrays(c, gin.p, in.part, gin.p, nullptr, s, in.step, nullptr, tape, false, gk, gk != nullptr));
+                DH_TRY(step_arrays(c, gin.p, pin, gin.p, nullptr, s, in.step, nullptr, tape, false, gk, gk != nullptr));
             } else {
                 Snapshot& nx = c->seg[k - k0 + 1];
                 if (!nx.buf) DH_TRY(dev_alloc(c, (void**)&nx.buf, state_floats(c) * sizeof(float)));
                 dh_state out;
                 snapshot_view(c, nx, &out);
                 const G6 gout(out);
-                DH_TRY(step_arrays(c, gin.p, in.part, gout.p, out.part, s, in.step, nullptr, tape, true, gk, gk != nullptr));
+                DH_TRY(step_arrays(c, gin.p, pin, gout.p, c->run_pstore ? nullptr : out.part, s, in.step, nullptr, tape, true, gk,
+                                   gk != nullptr));
                 nx.a = c->cosmo.static_mode ? 1.0 : c->run_a[k];
                 nx.dt_prev = c->run_dt[k];
                 nx.step = in.step + 1;
@@ -743,7 +793,8 @@ int dh_run_vjp(dh_ctx* c, const dh_cot* cot_final, dh_cot* cot_initial, dh_dpara
             snapshot_view(c, k == k0 ? c->snaps[sgi] : c->seg[k - k0], &in);
             const StepScalars s = step_scalars(c->cosmo, in.a, c->run_a[k], c->run_dt[k], in.dt_prev);
             const G6 gin(in);
-            DH_TRY(step_vjp_arrays(c, gin.p, in.part, s, in.step, cini.p, cot_initial->part, cini.p,
+            float* const* pin = (c->run_pstore && k > k0) ? c->pstore[k].p : in.part;
+            DH_TRY(step_vjp_arrays(c, gin.p, pin, s, in.step, cini.p, cot_initial->part, cini.p,
                                    cot_initial->part, taped ? &c->tapes[k - k0] : nullptr,
                                    c->run_gstore ? c->gstore[k].gp : nullptr));
             if (per_step) {

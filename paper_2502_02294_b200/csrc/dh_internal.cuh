@@ -70,6 +70,12 @@ struct GravStore {
     float* gp[3] = {nullptr, nullptr, nullptr};
 };
 
+// The particles entering one step of a checkpointed run, kept from the forward pass for the reverse pass.
+struct PartStore {
+    float* buf = nullptr;   // 6 n_part floats
+    float* p[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+};
+
 }  // namespace dh
 
 struct dh_ctx {
@@ -139,6 +145,9 @@ struct dh_ctx {
     std::vector<dh::GravStore> gstore;   // per-step g' of the last checkpointed dh_run
     int tune_gstore = 1;                 // 0: never keep g' from the forward pass
     bool run_gstore = false;             // the last dh_run filled gstore[0 .. run_n)
+    std::vector<dh::PartStore> pstore;   // particles entering step k = 1 .. run_n - 1 of the last checkpointed dh_run
+    int tune_pstore = 1;                 // 0: never keep them (the segment re-run repeats kick + drift)
+    bool run_pstore = false;             // the last dh_run filled pstore[1 .. run_n)
     std::vector<double> run_a, run_dt;
     int run_n = 0, run_stride = 0;
     double run_a0 = 0, run_dtprev0 = 0;

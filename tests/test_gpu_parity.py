@@ -711,16 +711,16 @@ CFG2_DGAMMA_TOL = 5e-3             # B200: 1e-4 ... 1.6e-3; the oracle moves its
 
 
 def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
-    """dh_run_vjp may keep g' of every step from the forward pass ("gstore") and each segment step's sweep inputs
-    ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
+    """dh_run_vjp may keep g' of every step ("gstore") and the particles entering it ("pstore") from the forward pass, and
+    each segment step's sweep inputs ("tape"), or recompute them (include/diffhydro.h, dh_tune): storage policy only, the arithmetic is the same.  Two
     policies differ by the order of the deposit's fp32 atomics in the recomputed g' (last-bit), nothing more."""
     cfg = W.scaled_config(0, 32, n_steps=7, a1=0.03)
     delta, gas, part = IC.coupled_ic(W, cfg)
     a_s, dt_s = api.dh_schedule_lna(cfg.a0, cfg.a1, cfg.n_steps)
     out = []
-    for tape, gstore in ((1, 1), (0, 1), (1, 0), (0, 0)):
+    for tape, gstore, pstore in ((1, 1, 1), (0, 1, 1), (1, 0, 1), (0, 0, 1), (1, 1, 0), (0, 0, 0)):
         ctx = api.context_for(cfg)
-        ctx.dh_tune("tape", tape); ctx.dh_tune("gstore", gstore)
+        ctx.dh_tune("tape", tape); ctx.dh_tune("gstore", gstore); ctx.dh_tune("pstore", pstore)
         sg = api.State(gas, part, cfg.a0)
         ctx.dh_run(sg, a_s[1:], dt_s, 3)
         cg = torch_.zeros_like(sg.gas); cg[0] = sg.gas[0]
@@ -750,8 +750,10 @@ def test_reverse_pass_storage_policies_agree(api, torch_, O, W, IC):
     for g, p_, dg, n in out[1:]:
         assert PT.rel_l2(g, g0) < tol_g and PT.rel_l2(p_, p0) < tol_p and abs(dg / dg0 - 1) < 1e-4, (sens_g, sens_p)
         assert PT.rel_l2_trimmed(g, g0, frac=1e-2) < TOL_GRAD
-    # keeping g' removes deposit + Poisson from the segment re-run: fewer launches than recomputing it
+    # keeping g' removes deposit + Poisson from the segment re-run: fewer launches than recomputing it; keeping the
+    # particles removes the re-run's kick + drift (7 steps in segments of 3, 3, 1: four of them are not a segment's last)
     assert out[0][3] < out[2][3] and out[1][3] < out[3][3]
+    assert out[4][3] - out[0][3] == 4 and out[5][3] - out[3][3] == 4
 
 
 def test_want_dsched_off_changes_only_the_schedule_cotangents(api, torch_, W, IC):
