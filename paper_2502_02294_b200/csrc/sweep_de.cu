@@ -333,8 +333,26 @@ __device__ __forceinline__ void ld2(const float* p, float& a, float& b) {
     a = t.x; b = t.y;
 }
 
-// x sweep: block = (N/2 chain threads, R rows); grid.x = ceil(N^2 / R)
-template <bool HAS_G>
+// K consecutive floats (K = 2 or 4) of one row as one 8 / 16-byte access
+template <int K>
+__device__ __forceinline__ void ldK(const float* p, float (&v)[K]) {
+    if (K == 4) {
+        const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[K - 1] = t.w;
+    } else {
+        ld2(p, v[0], v[1]);
+    }
+}
+template <int K>
+__device__ __forceinline__ void stK(float* p, const float (&v)[K]) {
+    if (K == 4) *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[K - 1]);
+    else *reinterpret_cast<float2*>(p) = make_float2(v[0], v[1]);
+}
+
+// x sweep: block = (N/K chain threads, R rows); grid.x = ceil(N^2 / R).  Forward K = 4 (64 - 77 registers at K = 2 leave the
+// room; the exchanges and barriers are per thread, so twice the cells per thread halve them), adjoint K = KD = 2.
+constexpr int KDF = 4;
+template <bool HAS_G, int K>
 __global__ void __launch_bounds__(512) sweep_de_x_fwd_kernel(Ptr6 in, const float* __restrict__ gfield, MPtr6s outp,
                                                              float* cmax, SweepConst sc, long nrows) {
     extern __shared__ float smem[];
@@ -345,19 +363,35 @@ __global__ void __launch_bounds__(512) sweep_de_x_fwd_kernel(Ptr6 in, const floa
     long row = (long)blockIdx.x * blockDim.y + r;
     const bool valid = row < nrows;
     if (!valid) row = nrows - 1;
-    const long base = row * sc.N + (long)cx * KD;
-    float u[KD][6], g[KD] = {0.f, 0.f}, out[KD][6], cin[KD];
+    const long base = row * sc.N + (long)cx * K;
+    float u[K][6], g[K], out[K][6], cin[K];
 #pragma unroll
-    for (int k = 0; k < 6; ++k) ld2(in.p[k] + base, u[0][k], u[1][k]);
-    if (HAS_G) ld2(gfield + base, g[0], g[1]);
+    for (int k = 0; k < 6; ++k) {
+        float v[K];
+        ldK<K>(in.p[k] + base, v);
+#pragma unroll
+        for (int j = 0; j < K; ++j) u[j][k] = v[j];
+    }
+    if (HAS_G) ldK<K>(gfield + base, g);
+    else {
+#pragma unroll
+        for (int j = 0; j < K; ++j) g[j] = 0.f;
+    }
     ChainDE ch{smem, nthr, r * Cx + cx, r * Cx + (cx == 0 ? Cx - 1 : cx - 1), r * Cx + (cx == Cx - 1 ? 0 : cx + 1)};
-    de_forward_core<KD, HAS_G>(u, g, ch, sc, out, cin);
+    de_forward_core<K, HAS_G>(u, g, ch, sc, out, cin);
     if (valid) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k) *reinterpret_cast<float2*>(outp.p[k] + base) = make_float2(out[0][k], out[1][k]);
+        for (int k = 0; k < 6; ++k) {
+            float v[K];
+#pragma unroll
+            for (int j = 0; j < K; ++j) v[j] = out[j][k];
+            stK<K>(outp.p[k] + base, v);
+        }
     }
     if (cmax) {
-        const float cm = (cin[1] > cin[0] || cin[1] != cin[1]) ? cin[1] : cin[0];
+        float cm = cin[0];
+#pragma unroll
+        for (int j = 1; j < K; ++j) cm = (cin[j] > cm || cin[j] != cin[j]) ? cin[j] : cm;
         block_max_to_global(cm, cmax, &s_max);
     }
 }
@@ -493,9 +527,9 @@ static void permute6(int d, float* const f[6], const float* out[6]) {
     out[0] = f[0]; out[1] = f[1 + d]; out[2] = f[1 + (d + 1) % 3]; out[3] = f[1 + (d + 2) % 3]; out[4] = f[4]; out[5] = f[5];
 }
 
-static void de_x_geometry(int N, dim3& block, unsigned& grid, long nrows) {
-    // N/2 chain threads per row, rows per block so that blocks are whole warps of about 64 threads (see sweep.cu)
-    const int Cx = N / KD;
+static void de_x_geometry(int N, int K, dim3& block, unsigned& grid, long nrows) {
+    // N/K chain threads per row, rows per block so that blocks are whole warps of about 64 threads (see sweep.cu)
+    const int Cx = N / K;
     int g = Cx, b = 32;
     while (b) { int t = g % b; g = b; b = t; }
     const int unit = 32 / g;
@@ -530,10 +564,10 @@ int launch_sweep_de(dh_ctx* c, int d, float* const in[6], const float* g, float 
     for (int k = 0; k < 6; ++k) pout.p[k] = const_cast<float*>(tmp[k]);
     if (d == 0) {
         dim3 block; unsigned grid; const long nrows = (long)N * N;
-        de_x_geometry(N, block, grid, nrows);
+        de_x_geometry(N, KDF, block, grid, nrows);
         const size_t sm = (size_t)DE_FWD_SLOTS * block.x * block.y * sizeof(float);
-        if (g) DE_LAUNCH((sweep_de_x_fwd_kernel<true>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
-        else DE_LAUNCH((sweep_de_x_fwd_kernel<false>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
+        if (g) DE_LAUNCH((sweep_de_x_fwd_kernel<true, KDF>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
+        else DE_LAUNCH((sweep_de_x_fwd_kernel<false, KDF>), grid, block, sm, c->stream, pin, g, pout, cmax, sc, nrows);
     } else if (c->tune_de_march) {
         // y / z forward: the marching pipeline with the sixth component (sweep_march.cu), 3.2 x faster than the chain tile
         float* outm[6];
@@ -572,7 +606,7 @@ int launch_sweep_de_vjp(dh_ctx* c, int d, float* const in[6], const float* g, fl
     for (int k = 0; k < 6; ++k) pci.p[k] = const_cast<float*>(tmp[k]);
     if (d == 0) {
         dim3 block; unsigned grid; const long nrows = (long)N * N;
-        de_x_geometry(N, block, grid, nrows);
+        de_x_geometry(N, KD, block, grid, nrows);
         const size_t sm = (size_t)DE_ADJ_SLOTS * block.x * block.y * sizeof(float);
         if (g) DE_LAUNCH((sweep_de_x_adj_kernel<true>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
         else DE_LAUNCH((sweep_de_x_adj_kernel<false>), grid, block, sm, c->stream, pin, g, pco, pci, g_bar, scal_bar, sc, nrows);
