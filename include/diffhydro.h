@@ -125,8 +125,10 @@ int dh_step_vjp(dh_ctx* ctx, const dh_state* state_checkpoint, double dt, double
 
 /* n_steps forward steps; a_sched[k] = scale factor at the END of step k, dt_sched[k] = its cosmic-time length (host
  * arrays).  checkpoint_stride > 0: a snapshot of the state is stored in the context before steps 0, stride,
- * 2 stride, ... for dh_run_vjp; <= 0: none.  The per-sweep CFL maxima are kept in the context
- * (dh_get_cmax).  Synchronises at the end and returns DH_ERR_NONFINITE if any maximum is NaN/Inf. */
+ * 2 stride, ... for dh_run_vjp; <= 0: none.  With a stride, and while the device has the room, every
+ * step's g' and the particles entering it are kept too (dh_tune "gstore", "pstore": 12 + 24 bytes per cell and step),
+ * which the reverse pass then does not recompute; the caller's particle arrays receive the final particles from the
+ * last step (they are not updated step by step).  The per-sweep CFL maxima are kept in the context (dh_get_cmax).  Synchronises at the end and returns DH_ERR_NONFINITE if any maximum is NaN/Inf. */
 int dh_run(dh_ctx* ctx, dh_state* state, const double* a_sched, const double* dt_sched, int n_steps,
            int checkpoint_stride);
 
@@ -137,7 +139,9 @@ int dh_run(dh_ctx* ctx, dh_state* state, const double* a_sched, const double* dt
 int dh_run_vjp(dh_ctx* ctx, const dh_cot* cot_final, dh_cot* cot_initial, dh_dparams* dparams);
 
 /* Optional: allocate now everything a dh_run(n_steps, checkpoint_stride) + dh_run_vjp pair will need (snapshot pool,
- * in-segment states, adjoint scratch, CFL log), so that neither call allocates.  Errors: DH_ERR_OOM. */
+ * in-segment states, adjoint scratch, CFL log, and -- each only if the device can hold it, see dh_tune -- the tapes of
+ * one segment, the per-step g' store and the per-step particle store), so that neither call allocates.  Invalidates the
+ * last run (dh_run_vjp then needs a new dh_run).  Errors: DH_ERR_OOM. */
 int dh_reserve(dh_ctx* ctx, int n_steps, int checkpoint_stride);
 
 /* ---- host-buffer variants (end-to-end path: host <-> device copies inside the call) ------------------------- */
